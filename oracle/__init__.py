@@ -1,0 +1,210 @@
+"""ORACLE -- test infrastructure, not the product.
+
+ctypes front end of ``qdp_oracle.c``: a plain single-threaded fp64 CPU
+implementation of the lattice expressions (definitions 1-6).
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
+/ ``--impl reference`` leg may import this package.  It imports nothing from
+``paper_1111_5596_b200`` and shares no code with the CUDA path.
+
+Arrays: host, lexicographic sites (x0 fastest), complex128,
+gauge [V,4,3,3], fermion [V,4,3], colour matrix [V,3,3].
+For fp32 parity the caller passes the fp32-rounded inputs converted back to
+complex128 (reading A13): the oracle always computes in fp64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "qdp_oracle.c")
+_LIB = os.path.join(_HERE, "libqdp_oracle.so")
+
+ALL, EVEN, ODD = 0, 1, 2
+CFLAGS = ["-O2", "-ffp-contract=off"]
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", *CFLAGS, "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+
+
+def _get():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        P, I, Z, D = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_double
+        sig = {
+            "orc_neighbor_table": ([P, I, I, P], None),
+            "orc_parity_mask": ([P, P], None),
+            "orc_shift_bytes": ([P, Z, P, P, I, I, I], None),
+            "orc_plaquette_site": ([P, P, Z, P], None),
+            "orc_plaquette": ([P, P, I, P], None),
+            "orc_polar_unitary": ([P, P], None),
+            "orc_proj_su3": ([P, P], None),
+            "orc_min_eig_vdv": ([P], D),
+            "orc_staple_site": ([P, P, Z, I, I, P], I),
+            "orc_ape_blend_site": ([P, P, Z, I, D, I, P], None),
+            "orc_ape_site": ([P, P, Z, I, D, I, P], None),
+            "orc_ape_smear_step": ([P, P, P, D, I, I], None),
+            "orc_hop_site": ([P, P, P, Z, P], None),
+            "orc_hop": ([P, P, P, P, I], None),
+            "orc_axpy_hop": ([P, D, D, P, P, P, I], None),
+            "orc_norm2": ([P, I, P, I], D),
+            "orc_inner": ([P, I, P, P, I, P], None),
+            "orc_sum": ([P, I, P, I, P], None),
+        }
+        for name, (args, res) in sig.items():
+            f = getattr(lib, name)
+            f.argtypes, f.restype = args, res
+        _lib = lib
+    return _lib
+
+
+def _dims(dims):
+    return (ctypes.c_int * 4)(*[int(d) for d in dims])
+
+
+def _c128(a):
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    return a
+
+
+def volume(dims):
+    return int(np.prod([int(d) for d in dims]))
+
+
+def neighbor_table(dims, mu, sign):
+    out = np.empty(volume(dims), dtype=np.int32)
+    _get().orc_neighbor_table(_dims(dims), mu, sign, out.ctypes.data)
+    return out
+
+
+def parity_mask(dims):
+    out = np.empty(volume(dims), dtype=np.uint8)
+    _get().orc_parity_mask(_dims(dims), out.ctypes.data)
+    return out
+
+
+def shift(dims, src, mu, sign, subset=ALL, dst=None):
+    """dst(x) = src(x + sign*mu) on the subset; any dtype, moved as bytes."""
+    src = np.ascontiguousarray(src)
+    V = volume(dims)
+    dst = np.zeros_like(src) if dst is None else np.ascontiguousarray(dst).copy()
+    _get().orc_shift_bytes(_dims(dims), src.nbytes // V, src.ctypes.data, dst.ctypes.data,
+                           mu, sign, subset)
+    return dst
+
+
+def plaquette(dims, u, subset=ALL):
+    u = _c128(u)
+    out = np.empty(3)
+    _get().orc_plaquette(_dims(dims), u.ctypes.data, subset, out.ctypes.data)
+    return out
+
+
+def plaquette_site(dims, u, lex):
+    u = _c128(u)
+    out = np.empty(6)
+    _get().orc_plaquette_site(_dims(dims), u.ctypes.data, lex, out.ctypes.data)
+    return out
+
+
+def polar_unitary(V):
+    V = _c128(V)
+    out = np.empty((3, 3), dtype=np.complex128)
+    _get().orc_polar_unitary(V.ctypes.data, out.ctypes.data)
+    return out
+
+
+def proj_su3(V):
+    V = _c128(V)
+    out = np.empty((3, 3), dtype=np.complex128)
+    _get().orc_proj_su3(V.ctypes.data, out.ctypes.data)
+    return out
+
+
+def min_eig_vdv(V):
+    V = _c128(V)
+    return _get().orc_min_eig_vdv(V.ctypes.data)
+
+
+def staple_site(dims, u, lex, mu, t_dir=3):
+    u = _c128(u)
+    out = np.empty((3, 3), dtype=np.complex128)
+    n = _get().orc_staple_site(_dims(dims), u.ctypes.data, lex, mu, t_dir, out.ctypes.data)
+    return out, n
+
+
+def ape_blend_site(dims, u, lex, mu, alpha, t_dir=3):
+    u = _c128(u)
+    out = np.empty((3, 3), dtype=np.complex128)
+    _get().orc_ape_blend_site(_dims(dims), u.ctypes.data, lex, mu, alpha, t_dir, out.ctypes.data)
+    return out
+
+
+def ape_site(dims, u, lex, mu, alpha, t_dir=3):
+    u = _c128(u)
+    out = np.empty((3, 3), dtype=np.complex128)
+    _get().orc_ape_site(_dims(dims), u.ctypes.data, lex, mu, alpha, t_dir, out.ctypes.data)
+    return out
+
+
+def ape_smear_step(dims, u, alpha, t_dir=3, subset=ALL, u_out=None):
+    u = _c128(u)
+    out = np.zeros_like(u) if u_out is None else _c128(u_out).copy()
+    _get().orc_ape_smear_step(_dims(dims), u.ctypes.data, out.ctypes.data, alpha, t_dir, subset)
+    return out
+
+
+def hop_site(dims, u, psi, lex):
+    u, psi = _c128(u), _c128(psi)
+    out = np.empty((4, 3), dtype=np.complex128)
+    _get().orc_hop_site(_dims(dims), u.ctypes.data, psi.ctypes.data, lex, out.ctypes.data)
+    return out
+
+
+def hop(dims, u, psi, subset=ALL, chi=None):
+    u, psi = _c128(u), _c128(psi)
+    out = np.zeros_like(psi) if chi is None else _c128(chi).copy()
+    _get().orc_hop(_dims(dims), u.ctypes.data, psi.ctypes.data, out.ctypes.data, subset)
+    return out
+
+
+def axpy_hop(dims, a, b, u, psi, subset=ALL, chi=None):
+    u, psi = _c128(u), _c128(psi)
+    out = np.zeros_like(psi) if chi is None else _c128(chi).copy()
+    _get().orc_axpy_hop(_dims(dims), a, b, u.ctypes.data, psi.ctypes.data, out.ctypes.data, subset)
+    return out
+
+
+def _reals(dims, f):
+    return 2 * (f.size // volume(dims))
+
+
+def norm2(dims, f, subset=ALL):
+    f = _c128(f)
+    return _get().orc_norm2(_dims(dims), _reals(dims, f), f.ctypes.data, subset)
+
+
+def inner(dims, a, b, subset=ALL):
+    a, b = _c128(a), _c128(b)
+    out = np.empty(2)
+    _get().orc_inner(_dims(dims), _reals(dims, a), a.ctypes.data, b.ctypes.data, subset,
+                     out.ctypes.data)
+    return complex(out[0], out[1])
+
+
+def sum_field(dims, f, subset=ALL):
+    f = _c128(f)
+    n = _reals(dims, f)
+    out = np.empty(n)
+    _get().orc_sum(_dims(dims), n, f.ctypes.data, subset, out.ctypes.data)
+    return out[0::2] + 1j * out[1::2]

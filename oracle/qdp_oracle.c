@@ -1,0 +1,442 @@
+/*
+ * qdp_oracle.c -- ORACLE (test infrastructure, NOT the product).
+ *
+ * A plain, slow, single-threaded fp64 CPU implementation of the QDP++-style
+ * lattice expressions that arXiv:1111.5596 (F. Winter, "Accelerating
+ * QDP++/Chroma on GPUs") moves to the GPU: "data parallel types and
+ * expressions suitable for lattice field theory" (section 1),
+ * evaluated one expression at a time at every lattice site (PAPER.md:29,
+ * 88-90).  The paper names the expressions only by their use ("smearing",
+ * "residual calculation"); their mathematical definitions
+ * are the textbook ones fixed by BASELINE.json:north_star and restated in
+ * SURVEY.md section 8(c), definitions 1-6.  Each function below cites the
+ * definition it writes out.
+ *
+ * Rules this file obeys:
+ *   - Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ *     --impl reference leg may build, load or call it.
+ *   - It shares no code, header, table or constant with the CUDA path under
+ *     paper_1111_5596_b200/csrc/.  Neighbours are recomputed from coordinates
+ *     with % at every use; there are no index tables.
+ *   - No blocking, fusion or reordering: every quantity is the definition,
+ *     evaluated site by site in nested loops, in the paper's host layout
+ *     (site-outermost array of structures, PAPER.md:116 -- the layout the
+ *     paper found un-coalesced on the device is fine for a host oracle).
+ *   - Built with -O2 -ffp-contract=off: no FMA contraction, no fast-math.
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"): unit gauge field gives
+ * plaquette exactly 1 and is a fixed point of the APE step; gauge
+ * invariance / covariance under random site-local SU(3); abelian closed
+ * forms; plane-wave eigenvalues of hop on the unit field; hermiticity of
+ * hop; scipy.linalg.polar and a Newton iteration for the projection;
+ * U U^dag = 1, det U = 1 after projection; shift round trips and coordinate
+ * fields; numpy brute force on 2^4 and (4,2,6,4).  Nothing here is "parity
+ * unpinned".
+ *
+ * Host layout (the paper gives none):
+ *   lex(x)   = x0 + L0*(x1 + L1*(x2 + L2*x3))        (x0 fastest)
+ *   gauge    u[((lex*4 + mu)*3 + row)*3 + col]        complex = (re, im)
+ *   fermion  psi[(lex*4 + spin)*3 + colour]
+ *   matrix   m[(lex*3 + row)*3 + col]
+ *   (U psi)_row = sum_col U[row][col] psi[col]
+ * Subsets: 0 = all, 1 = even, 2 = odd; parity = (x0+x1+x2+x3) & 1
+ * (SURVEY.md 8(c) reading A2).
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <string.h>
+
+typedef struct { double re, im; } cplx;
+
+static cplx c_add(cplx a, cplx b) { cplx r = { a.re + b.re, a.im + b.im }; return r; }
+static cplx c_mul(cplx a, cplx b) {
+    cplx r = { a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re };
+    return r;
+}
+static cplx c_conj(cplx a) { cplx r = { a.re, -a.im }; return r; }
+static cplx c_scale(double s, cplx a) { cplx r = { s * a.re, s * a.im }; return r; }
+
+/* 3x3 complex matrices, row-major m[row*3+col]. */
+static void m_mul(const cplx *a, const cplx *b, cplx *out) {
+    cplx t[9];
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) {
+            cplx s = { 0.0, 0.0 };
+            for (int k = 0; k < 3; k++) s = c_add(s, c_mul(a[i * 3 + k], b[k * 3 + j]));
+            t[i * 3 + j] = s;
+        }
+    memcpy(out, t, sizeof t);
+}
+static void m_adj(const cplx *a, cplx *out) {
+    cplx t[9];
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) t[i * 3 + j] = c_conj(a[j * 3 + i]);
+    memcpy(out, t, sizeof t);
+}
+static cplx m_trace(const cplx *a) { return c_add(c_add(a[0], a[4]), a[8]); }
+static cplx m_det(const cplx *a) {
+    cplx t0 = c_mul(a[0], c_add(c_mul(a[4], a[8]), c_scale(-1.0, c_mul(a[5], a[7]))));
+    cplx t1 = c_mul(a[1], c_add(c_mul(a[3], a[8]), c_scale(-1.0, c_mul(a[5], a[6]))));
+    cplx t2 = c_mul(a[2], c_add(c_mul(a[3], a[7]), c_scale(-1.0, c_mul(a[4], a[6]))));
+    return c_add(c_add(t0, c_scale(-1.0, t1)), t2);
+}
+
+/* ---- geometry ---------------------------------------------------------- */
+
+static size_t volume(const int *L) { return (size_t)L[0] * L[1] * L[2] * L[3]; }
+static void coords_of(const int *L, size_t lex, int *x) {
+    x[0] = (int)(lex % L[0]); lex /= L[0];
+    x[1] = (int)(lex % L[1]); lex /= L[1];
+    x[2] = (int)(lex % L[2]); lex /= L[2];
+    x[3] = (int)lex;
+}
+static size_t lex_of(const int *L, const int *x) {
+    return (size_t)x[0] + (size_t)L[0] * (x[1] + (size_t)L[1] * (x[2] + (size_t)L[2] * x[3]));
+}
+/* lex index of x + step*mu_hat, coordinates mod L (periodic). Definition 1. */
+static size_t hop_lex(const int *L, const int *x, int mu, int step) {
+    int y[4] = { x[0], x[1], x[2], x[3] };
+    y[mu] = ((x[mu] + step) % L[mu] + L[mu]) % L[mu];
+    return lex_of(L, y);
+}
+static int parity_of(const int *x) { return (x[0] + x[1] + x[2] + x[3]) & 1; }
+static int in_subset(const int *x, int subset) {
+    if (subset == 0) return 1;
+    return parity_of(x) == (subset == 1 ? 0 : 1);
+}
+
+/* out[lex(x)] = lex(x + sign*mu_hat).  SURVEY.md Appendix A "Neighbour tables". */
+void orc_neighbor_table(const int *L, int mu, int sign, int32_t *out) {
+    size_t V = volume(L);
+    for (size_t s = 0; s < V; s++) {
+        int x[4]; coords_of(L, s, x);
+        out[s] = (int32_t)hop_lex(L, x, mu, sign);
+    }
+}
+/* mask[lex(x)] = (x0+x1+x2+x3) & 1.  Reading A2. */
+void orc_parity_mask(const int *L, uint8_t *out) {
+    size_t V = volume(L);
+    for (size_t s = 0; s < V; s++) {
+        int x[4]; coords_of(L, s, x);
+        out[s] = (uint8_t)parity_of(x);
+    }
+}
+
+/* ---- shift (definition 1) --------------------------------------------------
+ * dst(x) = src(x + sign*mu_hat) for x in subset; other sites of dst untouched.
+ * Pure data movement on opaque per-site records so it is bit-exact for any
+ * element type. */
+void orc_shift_bytes(const int *L, size_t bytes_per_site, const void *src, void *dst,
+                     int mu, int sign, int subset) {
+    size_t V = volume(L);
+    const char *s = (const char *)src;
+    char *d = (char *)dst;
+    for (size_t i = 0; i < V; i++) {
+        int x[4]; coords_of(L, i, x);
+        if (!in_subset(x, subset)) continue;
+        size_t j = hop_lex(L, x, mu, sign);
+        memcpy(d + i * bytes_per_site, s + j * bytes_per_site, bytes_per_site);
+    }
+}
+
+/* ---- plaquette (definition 2) ------------------------------------------- */
+
+static const cplx *link_at(const double *u, size_t lex, int mu) {
+    return (const cplx *)(u + ((lex * 4 + (size_t)mu) * 9) * 2);
+}
+
+/* Re tr P_{mu nu}(x), P = U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag. */
+static double plaq_retr(const int *L, const double *u, const int *x, int mu, int nu) {
+    size_t s = lex_of(L, x);
+    cplx a[9], b[9], t[9];
+    m_mul(link_at(u, s, mu), link_at(u, hop_lex(L, x, mu, +1), nu), a);
+    m_adj(link_at(u, hop_lex(L, x, nu, +1), mu), b);
+    m_mul(a, b, t);
+    m_adj(link_at(u, s, nu), b);
+    m_mul(t, b, a);
+    return m_trace(a).re;
+}
+
+/* out6 = Re tr P_{mu nu}(x) for (mu,nu) = (0,1),(0,2),(1,2),(0,3),(1,3),(2,3). */
+void orc_plaquette_site(const int *L, const double *u, size_t lex, double *out6) {
+    static const int pl[6][2] = { {0,1}, {0,2}, {1,2}, {0,3}, {1,3}, {2,3} };
+    int x[4]; coords_of(L, lex, x);
+    for (int p = 0; p < 6; p++) out6[p] = plaq_retr(L, u, x, pl[p][0], pl[p][1]);
+}
+
+/* Compensated (Neumaier) accumulator: the oracle's global sums do not depend
+ * on summation order to the precision the parity bar needs (reading A12). */
+typedef struct { double s, c; } ksum;
+static void k_add(ksum *k, double v) {
+    double t = k->s + v;
+    if (fabs(k->s) >= fabs(v)) k->c += (k->s - t) + v; else k->c += (v - t) + k->s;
+    k->s = t;
+}
+static double k_val(const ksum *k) { return k->s + k->c; }
+
+/* out[0] = (1/(6*3*N)) sum_{x in sub} sum_{mu<nu} Re tr P_{mu nu}(x)
+ * out[1] = the 3 spatial planes (mu<nu<3), normalised 1/(3*3*N)
+ * out[2] = the 3 temporal planes (nu=3),   normalised 1/(3*3*N)
+ * N = number of sites in the subset (reading A4, A5). */
+void orc_plaquette(const int *L, const double *u, int subset, double *out3) {
+    size_t V = volume(L), n = 0;
+    ksum ss = { 0, 0 }, st = { 0, 0 };
+    for (size_t s = 0; s < V; s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        n++;
+        for (int mu = 0; mu < 4; mu++)
+            for (int nu = mu + 1; nu < 4; nu++) {
+                double v = plaq_retr(L, u, x, mu, nu);
+                if (nu == 3) k_add(&st, v); else k_add(&ss, v);
+            }
+    }
+    double sp = k_val(&ss), tp = k_val(&st), N = (double)n;
+    out3[0] = (sp + tp) / (6.0 * 3.0 * N);
+    out3[1] = sp / (3.0 * 3.0 * N);
+    out3[2] = tp / (3.0 * 3.0 * N);
+}
+
+/* ---- SU(3) projection (definition 4, Appendix B) -------------------------- */
+
+/* Cyclic complex Jacobi on a 3x3 Hermitian H: H = Q diag(lam) Q^dag.
+ * Each rotation is applied as plain J^dag H J, Q <- Q J with full 3x3 products. */
+static void herm_eig3(const cplx *Hin, double *lam, cplx *Q) {
+    cplx H[9];
+    memcpy(H, Hin, sizeof H);
+    for (int i = 0; i < 9; i++) { Q[i].re = (i % 4 == 0) ? 1.0 : 0.0; Q[i].im = 0.0; }
+    double tr = H[0].re + H[4].re + H[8].re;
+    for (int sweep = 0; sweep < 100; sweep++) {
+        double off = 0.0;
+        for (int p = 0; p < 3; p++)
+            for (int q = p + 1; q < 3; q++)
+                off += H[p * 3 + q].re * H[p * 3 + q].re + H[p * 3 + q].im * H[p * 3 + q].im;
+        if (sqrt(off) <= 1e-17 * fabs(tr)) break;
+        for (int p = 0; p < 3; p++)
+            for (int q = p + 1; q < 3; q++) {
+                cplx g = H[p * 3 + q];
+                double ag = sqrt(g.re * g.re + g.im * g.im);
+                if (ag == 0.0) continue;
+                double a = H[p * 3 + p].re, b = H[q * 3 + q].re;
+                /* phase e^{i phi} of g, then a real 2x2 Jacobi rotation */
+                cplx eph = { g.re / ag, g.im / ag };
+                double tau = (b - a) / (2.0 * ag);
+                double t = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+                double c = 1.0 / sqrt(1.0 + t * t), s = t * c;
+                cplx J[9], Jd[9], T[9];
+                for (int i = 0; i < 9; i++) { J[i].re = (i % 4 == 0) ? 1.0 : 0.0; J[i].im = 0.0; }
+                /* J = D R, D = diag(1, e^{-i phi}) on (p,q), R = [[c, s], [-s, c]] */
+                J[p * 3 + p].re = c;  J[p * 3 + p].im = 0.0;
+                J[p * 3 + q].re = s;  J[p * 3 + q].im = 0.0;
+                J[q * 3 + p] = c_scale(-s, c_conj(eph));
+                J[q * 3 + q] = c_scale(c, c_conj(eph));
+                m_adj(J, Jd);
+                m_mul(Jd, H, T);
+                m_mul(T, J, H);
+                m_mul(Q, J, Q);
+                /* the rotated pair is annihilated up to rounding: set it to exactly 0
+                 * (standard Jacobi practice) and keep H exactly Hermitian */
+                H[p * 3 + q].re = 0.0; H[p * 3 + q].im = 0.0;
+                for (int i = 0; i < 3; i++) {
+                    H[i * 3 + i].im = 0.0;
+                    for (int j = i + 1; j < 3; j++) H[j * 3 + i] = c_conj(H[i * 3 + j]);
+                }
+            }
+    }
+    lam[0] = H[0].re; lam[1] = H[4].re; lam[2] = H[8].re;
+}
+
+/* W = V (V^dag V)^{-1/2}: the unitary polar factor (definition 4). */
+void orc_polar_unitary(const double *Vin, double *Wout) {
+    const cplx *V = (const cplx *)Vin;
+    cplx Vd[9], H[9], Q[9], Qd[9], D[9], R[9], T[9], W[9];
+    double lam[3];
+    m_adj(V, Vd);
+    m_mul(Vd, V, H);
+    herm_eig3(H, lam, Q);
+    memset(D, 0, sizeof D);
+    for (int k = 0; k < 3; k++) D[k * 4].re = 1.0 / sqrt(lam[k]);
+    m_adj(Q, Qd);
+    m_mul(Q, D, T);
+    m_mul(T, Qd, R);
+    m_mul(V, R, W);
+    memcpy(Wout, W, sizeof W);
+}
+
+/* Proj(V) = W e^{-i theta/3}, theta = arg det V in (-pi, pi] (readings A8, A9). */
+void orc_proj_su3(const double *Vin, double *out) {
+    cplx W[9];
+    orc_polar_unitary(Vin, (double *)W);
+    cplx d = m_det((const cplx *)Vin);
+    double theta = atan2(d.im, d.re);
+    cplx ph = { cos(theta / 3.0), -sin(theta / 3.0) };
+    cplx *o = (cplx *)out;
+    for (int i = 0; i < 9; i++) o[i] = c_mul(W[i], ph);
+}
+
+/* smallest singular value^2 of V (lambda_min of V^dag V), for reading A10 */
+double orc_min_eig_vdv(const double *Vin) {
+    const cplx *V = (const cplx *)Vin;
+    cplx Vd[9], H[9], Q[9];
+    double lam[3];
+    m_adj(V, Vd);
+    m_mul(Vd, V, H);
+    herm_eig3(H, lam, Q);
+    double m = lam[0];
+    if (lam[1] < m) m = lam[1];
+    if (lam[2] < m) m = lam[2];
+    return m;
+}
+
+/* ---- staples and the APE step (definition 3) ------------------------------ */
+
+/* S_mu(x) = sum_{nu in smeared set, nu != mu}
+ *   [ U_nu(x) U_mu(x+nu) U_nu(x+mu)^dag + U_nu(x-nu)^dag U_mu(x-nu) U_nu(x-nu+mu) ]
+ * smeared set = {0,1,2} if t_dir == 3, {0,1,2,3} if t_dir == -1.
+ * Returns the number of staples n = 2*(|set|-1). */
+int orc_staple_site(const int *L, const double *u, size_t lex, int mu, int t_dir, double *S18) {
+    int x[4]; coords_of(L, lex, x);
+    cplx S[9];
+    memset(S, 0, sizeof S);
+    int n = 0;
+    for (int nu = 0; nu < 4; nu++) {
+        if (nu == mu || nu == t_dir) continue;
+        cplx a[9], b[9], t[9];
+        /* upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dag */
+        m_mul(link_at(u, lex, nu), link_at(u, hop_lex(L, x, nu, +1), mu), a);
+        m_adj(link_at(u, hop_lex(L, x, mu, +1), nu), b);
+        m_mul(a, b, t);
+        for (int i = 0; i < 9; i++) S[i] = c_add(S[i], t[i]);
+        /* lower: U_nu(x-nu)^dag U_mu(x-nu) U_nu(x-nu+mu) */
+        int y[4] = { x[0], x[1], x[2], x[3] };
+        y[nu] = ((x[nu] - 1) % L[nu] + L[nu]) % L[nu];
+        size_t ly = lex_of(L, y);
+        m_adj(link_at(u, ly, nu), b);
+        m_mul(b, link_at(u, ly, mu), a);
+        m_mul(a, link_at(u, hop_lex(L, y, mu, +1), nu), t);
+        for (int i = 0; i < 9; i++) S[i] = c_add(S[i], t[i]);
+        n += 2;
+    }
+    memcpy(S18, S, sizeof S);
+    return n;
+}
+
+/* V_mu(x) = (1-alpha) U_mu(x) + (alpha/n) S_mu(x)  (reading A6), before projection. */
+void orc_ape_blend_site(const int *L, const double *u, size_t lex, int mu, double alpha,
+                        int t_dir, double *V18) {
+    cplx S[9];
+    int n = orc_staple_site(L, u, lex, mu, t_dir, (double *)S);
+    const cplx *U = link_at(u, lex, mu);
+    cplx *V = (cplx *)V18;
+    for (int i = 0; i < 9; i++)
+        V[i] = c_add(c_scale(1.0 - alpha, U[i]), c_scale(alpha / (double)n, S[i]));
+}
+
+/* U'_mu(x) = Proj(V_mu(x)); if mu == t_dir the link is copied unchanged (A7). */
+void orc_ape_site(const int *L, const double *u, size_t lex, int mu, double alpha, int t_dir,
+                  double *out18) {
+    if (mu == t_dir) { memcpy(out18, link_at(u, lex, mu), 18 * sizeof(double)); return; }
+    double V[18];
+    orc_ape_blend_site(L, u, lex, mu, alpha, t_dir, V);
+    orc_proj_su3(V, out18);
+}
+
+void orc_ape_smear_step(const int *L, const double *u_in, double *u_out, double alpha, int t_dir,
+                        int subset) {
+    size_t V = volume(L);
+    for (size_t s = 0; s < V; s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        for (int mu = 0; mu < 4; mu++)
+            orc_ape_site(L, u_in, s, mu, alpha, t_dir, u_out + ((s * 4 + (size_t)mu) * 9) * 2);
+    }
+}
+
+/* ---- hop (definition 5) ---------------------------------------------------
+ * chi(x)_{s a} = sum_mu sum_b [ U_mu(x)_{ab} psi(x+mu)_{sb}
+ *                             + conj(U_mu(x-mu)_{ba}) psi(x-mu)_{sb} ]      */
+void orc_hop_site(const int *L, const double *u, const double *psi, size_t lex, double *out24) {
+    int x[4]; coords_of(L, lex, x);
+    cplx chi[12];
+    memset(chi, 0, sizeof chi);
+    for (int mu = 0; mu < 4; mu++) {
+        size_t lf = hop_lex(L, x, mu, +1), lb = hop_lex(L, x, mu, -1);
+        const cplx *Uf = link_at(u, lex, mu), *Ub = link_at(u, lb, mu);
+        const cplx *pf = (const cplx *)(psi + lf * 24), *pb = (const cplx *)(psi + lb * 24);
+        for (int s = 0; s < 4; s++)
+            for (int a = 0; a < 3; a++)
+                for (int b = 0; b < 3; b++) {
+                    chi[s * 3 + a] = c_add(chi[s * 3 + a], c_mul(Uf[a * 3 + b], pf[s * 3 + b]));
+                    chi[s * 3 + a] = c_add(chi[s * 3 + a], c_mul(c_conj(Ub[b * 3 + a]), pb[s * 3 + b]));
+                }
+    }
+    memcpy(out24, chi, sizeof chi);
+}
+
+void orc_hop(const int *L, const double *u, const double *psi, double *chi, int subset) {
+    size_t V = volume(L);
+    for (size_t s = 0; s < V; s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        orc_hop_site(L, u, psi, s, chi + s * 24);
+    }
+}
+
+/* chi = a psi + b hop(psi) on the subset (definition 6, axpy_hop). */
+void orc_axpy_hop(const int *L, double a, double b, const double *u, const double *psi,
+                  double *chi, int subset) {
+    size_t V = volume(L);
+    for (size_t s = 0; s < V; s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        double h[24];
+        orc_hop_site(L, u, psi, s, h);
+        for (int i = 0; i < 24; i++) chi[s * 24 + i] = a * psi[s * 24 + i] + b * h[i];
+    }
+}
+
+/* ---- global reductions (definition 6) -------------------------------------
+ * reals = 2 * (complex components per site). Lexicographic order, compensated. */
+double orc_norm2(const int *L, int reals, const double *f, int subset) {
+    size_t V = volume(L);
+    ksum k = { 0, 0 };
+    for (size_t s = 0; s < V; s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        for (int i = 0; i < reals; i++) k_add(&k, f[s * reals + i] * f[s * reals + i]);
+    }
+    return k_val(&k);
+}
+
+/* out = sum_x sum_c conj(a_c(x)) b_c(x)  (conjugates its FIRST argument, A12). */
+void orc_inner(const int *L, int reals, const double *a, const double *b, int subset, double *out2) {
+    size_t V = volume(L);
+    ksum kr = { 0, 0 }, ki = { 0, 0 };
+    for (size_t s = 0; s < V; s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        for (int c = 0; c < reals / 2; c++) {
+            cplx p = c_mul(c_conj(((const cplx *)a)[s * (reals / 2) + c]),
+                           ((const cplx *)b)[s * (reals / 2) + c]);
+            k_add(&kr, p.re);
+            k_add(&ki, p.im);
+        }
+    }
+    out2[0] = k_val(&kr);
+    out2[1] = k_val(&ki);
+}
+
+/* out[c] = sum_x f_c(x), per real component (re, im interleaved like f). */
+void orc_sum(const int *L, int reals, const double *f, int subset, double *out) {
+    size_t V = volume(L);
+    for (int i = 0; i < reals; i++) {
+        ksum k = { 0, 0 };
+        for (size_t s = 0; s < V; s++) {
+            int x[4]; coords_of(L, s, x);
+            if (!in_subset(x, subset)) continue;
+            k_add(&k, f[s * reals + i]);
+        }
+        out[i] = k_val(&k);
+    }
+}
