@@ -1,0 +1,194 @@
+/*
+ * qdp_b200.h -- C ABI of libqdp_b200.so: site-parallel evaluation of QDP++-style
+ * lattice-field expressions on one NVIDIA B200 (sm_100a).
+ *
+ * This is the hot path arXiv:1111.5596 (F. Winter, "Accelerating QDP++/Chroma on
+ * GPUs", PoS Lattice 2011) moves to the GPU: "data parallel types and
+ * expressions suitable for lattice field theory" (sec. 1), one
+ * device kernel per expression with no lattice-sized temporaries (PAPER.md:27,
+ * 88-90), for the "non-kernel routines like smearing" (sec. 3) and
+ * the "residual calculation and solution reconstruction" around the solver
+ * (sec. 4.3).  The paper defines none of the expressions
+ * mathematically; the definitions are the textbook ones fixed by
+ * BASELINE.json:north_star and written out in SURVEY.md sec. 8(c) (cited below
+ * as "def. N") and DESIGN.md.  The paper's run-time code generator and software
+ * LRU cache are prior art and are not part of this library: fields live in
+ * device memory for their whole lifetime, in a site-fastest structure-of-arrays
+ * complex layout -- the coalesced layout PAPER.md:118 (sec. 6) found 6-10x
+ * faster than the host-native one.
+ *
+ * Conventions
+ *   - Every function returns a status (QDP_OK or a negative error); no C++
+ *     exception crosses the ABI.  qdp_last_error() returns a thread-local
+ *     message for the last failure on the calling thread.
+ *   - "host" pointers are ordinary host memory owned by the caller (pinned memory
+ *     makes the copies faster, it is not required).  "device" pointers are CUDA
+ *     device memory on the lattice's device.
+ *   - Public site order (host buffers, exported tables):
+ *         lex(x) = x0 + L0*(x1 + L1*(x2 + L2*x3)),  x = (x0,x1,x2,x3), x0 fastest.
+ *     The device-internal site order is private.
+ *   - Host field layout, array of structures, element type = field precision,
+ *     complex = (re, im) adjacent:
+ *         QDP_COLOR_MATRIX  host[(lex*3 + row)*3 + col]
+ *         QDP_GAUGE         host[((lex*4 + mu)*3 + row)*3 + col]
+ *         QDP_FERMION       host[(lex*4 + spin)*3 + colour]
+ *     (U psi)_row = sum_col U[row][col] psi[col].
+ *   - Subsets: parity(x) = (x0+x1+x2+x3) & 1; QDP_EVEN = parity 0.  An operation
+ *     under a subset writes only the subset's sites of its destination (all
+ *     other sites keep their previous contents) and reductions sum only the
+ *     subset's sites.  Neighbours are read from wherever they are.
+ *   - Kernels are enqueued on the lattice's stream (default: the legacy default
+ *     stream).  Field->field calls are asynchronous with respect to the host;
+ *     calls that return host scalars synchronise that stream before returning.
+ *   - Neighbour-reading operations are out of place: passing the destination as
+ *     a neighbour-read source returns QDP_ERR_ALIAS.
+ *   - There is no CPU fallback anywhere: a missing device is an error.
+ */
+#ifndef QDP_B200_H
+#define QDP_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    QDP_OK = 0,
+    QDP_ERR_ARG = -1,      /* null pointer, bad enum value, bad mu/sign            */
+    QDP_ERR_DIMS = -2,     /* an extent is odd or < 2, or the volume is too large  */
+    QDP_ERR_KIND = -3,     /* a field has the wrong kind for this operation        */
+    QDP_ERR_PREC = -4,     /* operands of different precision                      */
+    QDP_ERR_LATTICE = -5,  /* operands belong to different lattices                */
+    QDP_ERR_ALIAS = -6,    /* destination aliases a neighbour-read source          */
+    QDP_ERR_OOM = -7,      /* device allocation failed                             */
+    QDP_ERR_CUDA = -8      /* any other CUDA runtime error (message has details)   */
+};
+
+typedef enum { QDP_ALL = 0, QDP_EVEN = 1, QDP_ODD = 2 } qdp_subset;
+typedef enum { QDP_F32 = 0, QDP_F64 = 1 } qdp_prec;
+typedef enum {
+    QDP_COLOR_MATRIX = 0,  /* 3x3 complex per site (9 complex)          */
+    QDP_GAUGE = 1,         /* 4 colour matrices per site (36 complex)   */
+    QDP_FERMION = 2        /* 4 spin x 3 colour per site (12 complex)   */
+} qdp_kind;
+
+typedef struct qdp_lattice qdp_lattice;   /* opaque */
+typedef struct qdp_field qdp_field;       /* opaque */
+
+/* ---- lattice ------------------------------------------------------------- */
+
+/* Create a periodic 4-D lattice on CUDA device `device`.
+ * dims (host, 4 ints): extents (L0,L1,L2,L3) = (x,y,z,t).  Every extent must be
+ * even and >= 2 (red/black colouring needs it, reading A2) and the volume must
+ * be below 2^31/36 sites; otherwise QDP_ERR_DIMS.  *out is owned by the caller
+ * until qdp_lattice_destroy.  Fields must be freed before their lattice. */
+int qdp_lattice_create(const int dims[4], int device, qdp_lattice** out);
+int qdp_lattice_destroy(qdp_lattice* lat);
+
+/* Use `cuda_stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream;
+ * NULL = legacy default stream) for every later call on this lattice. */
+int qdp_lattice_set_stream(qdp_lattice* lat, void* cuda_stream);
+
+/* Replace the device allocator used by qdp_field_alloc and the library's scratch
+ * buffers (default cudaMalloc/cudaFree).  alloc(bytes, ctx) returns a device
+ * pointer aligned to >= 256 bytes or NULL; free_(ptr, ctx) releases it.  Lets
+ * PyTorch's caching allocator own the memory.  Process-wide; set it before
+ * creating lattices.  Passing alloc = NULL restores the default. */
+int qdp_set_allocator(void* (*alloc)(size_t bytes, void* ctx),
+                      void (*free_)(void* ptr, void* ctx), void* ctx);
+
+/* Export geometry in the PUBLIC numbering for parity checks (def. 1, App. A):
+ *   out[lex(x)] = lex(x + sign*mu_hat)   (V int32, host)
+ *   out[lex(x)] = parity(x)              (V bytes, host)
+ * Both are produced on the device by the same index arithmetic the kernels use
+ * and converted to the public numbering.  Synchronous. */
+int qdp_lattice_neighbor_table(qdp_lattice* lat, int mu, int sign, int32_t* host_out);
+int qdp_lattice_parity_mask(qdp_lattice* lat, uint8_t* host_out);
+int qdp_lattice_volume(const qdp_lattice* lat, int64_t* out);
+
+/* ---- fields -------------------------------------------------------------- */
+
+/* Allocate a field on the lattice's device (library-owned, contents undefined). */
+int qdp_field_alloc(qdp_lattice* lat, qdp_kind kind, qdp_prec prec, qdp_field** out);
+/* Wrap caller-owned device memory (e.g. a torch tensor) as a field.  `bytes` must
+ * be at least qdp_field_bytes(); dev_ptr must be 256-byte aligned and must stay
+ * valid until qdp_field_free, which does not free it. */
+int qdp_field_wrap(qdp_lattice* lat, qdp_kind kind, qdp_prec prec, void* dev_ptr, size_t bytes,
+                   qdp_field** out);
+int qdp_field_free(qdp_field* f);
+/* Bytes of device memory a field of this kind/precision occupies (= host bytes). */
+int qdp_field_bytes(const qdp_lattice* lat, qdp_kind kind, qdp_prec prec, size_t* out);
+
+/* Host (layout above) <-> device (private layout).  Synchronous: the host buffer
+ * may be reused as soon as the call returns.  Bit-exact round trip. */
+int qdp_field_upload(qdp_field* f, const void* host_aos_lex);
+int qdp_field_download(const qdp_field* f, void* host_aos_lex);
+/* dst = src on the device (same kind and precision); asynchronous. */
+int qdp_field_copy(qdp_field* dst, const qdp_field* src);
+
+/* ---- expressions --------------------------------------------------------- */
+
+/* def. 1: dst(x) = src(x + sign*mu_hat) for x in subset, coordinates mod L.
+ * mu in 0..3, sign = +1 or -1; dst and src of the same kind and precision;
+ * dst == src is QDP_ERR_ALIAS.  Pure data movement: bit-exact. */
+int qdp_shift(qdp_field* dst, const qdp_field* src, int mu, int sign, qdp_subset subset);
+
+/* def. 2: with P_{mu nu}(x) = U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag and N
+ * the number of sites in the subset,
+ *   out[0] = 1/(6*3*N) sum_{x in subset} sum_{mu<nu} Re tr P_{mu nu}(x)
+ *   out[1] = 1/(3*3*N) ... over the 3 spatial planes (mu < nu < 3)
+ *   out[2] = 1/(3*3*N) ... over the 3 temporal planes (nu = 3)
+ * u: QDP_GAUGE.  out: 3 doubles on the host.  Per-site arithmetic in the field
+ * precision, sums accumulated in fp64 by a fixed-shape tree (bit-identical from
+ * run to run).  Synchronous. */
+int qdp_plaquette(const qdp_field* u, qdp_subset subset, double out[3]);
+
+/* def. 3-4: one APE smearing step with SU(3) reprojection.  For x in subset,
+ * mu in the smeared set S ({0,1,2} if t_dir == 3, {0,1,2,3} if t_dir == -1):
+ *   V = (1-alpha) U_mu(x) + (alpha/n) sum_{nu in S, nu != mu}
+ *         [ U_nu(x) U_mu(x+nu) U_nu(x+mu)^dag
+ *         + U_nu(x-nu)^dag U_mu(x-nu) U_nu(x-nu+mu) ],      n = 2(|S|-1)
+ *   u_out_mu(x) = V (V^dag V)^{-1/2} exp(-i arg(det V)/3),   arg in (-pi, pi]
+ * and u_out_3(x) = u_in_3(x) (bit-exact copy) when t_dir == 3.  V must be
+ * non-singular (reading A10).  u_in, u_out: QDP_GAUGE, same precision;
+ * u_out == u_in is QDP_ERR_ALIAS.  alpha is cast to the field precision.
+ * Asynchronous. */
+int qdp_ape_smear_step(qdp_field* u_out, const qdp_field* u_in, double alpha, int t_dir,
+                       qdp_subset subset);
+
+/* def. 5: chi(x)_{s a} = sum_mu sum_b [ U_mu(x)_{ab} psi(x+mu)_{s b}
+ *                                      + conj(U_mu(x-mu)_{ba}) psi(x-mu)_{s b} ]
+ * for x in subset (no gamma matrices, no kappa, periodic in all directions).
+ * chi, psi: QDP_FERMION; u: QDP_GAUGE; chi == psi is QDP_ERR_ALIAS.  Asynchronous. */
+int qdp_hop(qdp_field* chi, const qdp_field* u, const qdp_field* psi, qdp_subset subset);
+
+/* def. 6: chi = a*psi + b*hop(psi) on the subset, one fused kernel.  If norm2_out
+ * is not NULL it receives sum_{x in subset} |chi(x)|^2 accumulated in the same
+ * pass (fp64) and the call is synchronous; otherwise asynchronous.  a, b are cast
+ * to the field precision. */
+int qdp_axpy_hop(qdp_field* chi, double a, double b, const qdp_field* u, const qdp_field* psi,
+                 qdp_subset subset, double* norm2_out);
+
+/* def. 6: global reductions over the subset, any kind; accumulated and returned
+ * in fp64 for both precisions; fixed-shape tree.  Synchronous.
+ *   qdp_norm2: out[0]   = sum_x sum_c |f_c(x)|^2
+ *   qdp_inner: out[0,1] = (re, im) of sum_x sum_c conj(a_c(x)) b_c(x)
+ *   qdp_sum:   out[2c], out[2c+1] = (re, im) of sum_x f_c(x), c < ncomp (9/36/12) */
+int qdp_norm2(const qdp_field* f, qdp_subset subset, double* out);
+int qdp_inner(const qdp_field* a, const qdp_field* b, qdp_subset subset, double out[2]);
+int qdp_sum(const qdp_field* f, qdp_subset subset, double* out);
+
+/* Block the host until every call enqueued on the lattice's stream has finished. */
+int qdp_lattice_sync(qdp_lattice* lat);
+
+/* Number of kernels this library has launched in this process (all lattices). */
+int64_t qdp_kernel_launch_count(void);
+
+const char* qdp_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QDP_B200_H */

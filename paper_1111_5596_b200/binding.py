@@ -1,0 +1,285 @@
+"""ctypes binding of include/qdp_b200.h: argument marshalling only.
+
+Function names are those of the C ABI.  Handles are small Python objects that own
+the C handle (and, for fields, the torch tensor that provides the device memory).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+__all__ = [
+    "QdpError", "Lattice", "Field", "LIB_PATH", "DECLARED_SYMBOLS",
+    "QDP_ALL", "QDP_EVEN", "QDP_ODD", "QDP_F32", "QDP_F64",
+    "QDP_COLOR_MATRIX", "QDP_GAUGE", "QDP_FERMION",
+    "qdp_lattice_create", "qdp_lattice_destroy", "qdp_lattice_set_stream", "qdp_lattice_volume",
+    "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
+    "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
+    "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
+    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop",
+    "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
+    "qdp_set_allocator", "field_from_host", "field_to_host",
+]
+
+QDP_ALL, QDP_EVEN, QDP_ODD = 0, 1, 2
+QDP_F32, QDP_F64 = 0, 1
+QDP_COLOR_MATRIX, QDP_GAUGE, QDP_FERMION = 0, 1, 2
+_NCOMP = {QDP_COLOR_MATRIX: 9, QDP_GAUGE: 36, QDP_FERMION: 12}
+_SHAPE = {QDP_COLOR_MATRIX: (3, 3), QDP_GAUGE: (4, 3, 3), QDP_FERMION: (4, 3)}
+
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libqdp_b200.so")
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_1111_5596_b200.build` "
+        "(there is no CPU fallback)")
+_lib = ctypes.CDLL(LIB_PATH)
+
+_P, _I, _D, _Z = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+_PP = ctypes.POINTER(ctypes.c_void_p)
+ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+FREE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
+
+# every symbol include/qdp_b200.h declares: (argtypes, restype)
+DECLARED_SYMBOLS = {
+    "qdp_lattice_create": ([_P, _I, _PP], _I),
+    "qdp_lattice_destroy": ([_P], _I),
+    "qdp_lattice_set_stream": ([_P, _P], _I),
+    "qdp_set_allocator": ([_P, _P, _P], _I),
+    "qdp_lattice_neighbor_table": ([_P, _I, _I, _P], _I),
+    "qdp_lattice_parity_mask": ([_P, _P], _I),
+    "qdp_lattice_volume": ([_P, ctypes.POINTER(ctypes.c_int64)], _I),
+    "qdp_field_alloc": ([_P, _I, _I, _PP], _I),
+    "qdp_field_wrap": ([_P, _I, _I, _P, _Z, _PP], _I),
+    "qdp_field_free": ([_P], _I),
+    "qdp_field_bytes": ([_P, _I, _I, ctypes.POINTER(_Z)], _I),
+    "qdp_field_upload": ([_P, _P], _I),
+    "qdp_field_download": ([_P, _P], _I),
+    "qdp_field_copy": ([_P, _P], _I),
+    "qdp_shift": ([_P, _P, _I, _I, _I], _I),
+    "qdp_plaquette": ([_P, _I, _P], _I),
+    "qdp_ape_smear_step": ([_P, _P, _D, _I, _I], _I),
+    "qdp_hop": ([_P, _P, _P, _I], _I),
+    "qdp_axpy_hop": ([_P, _D, _D, _P, _P, _I, _P], _I),
+    "qdp_norm2": ([_P, _I, _P], _I),
+    "qdp_inner": ([_P, _P, _I, _P], _I),
+    "qdp_sum": ([_P, _I, _P], _I),
+    "qdp_lattice_sync": ([_P], _I),
+    "qdp_kernel_launch_count": ([], ctypes.c_int64),
+    "qdp_last_error": ([], ctypes.c_char_p),
+}
+for _name, (_args, _res) in DECLARED_SYMBOLS.items():
+    _f = getattr(_lib, _name)
+    _f.argtypes, _f.restype = _args, _res
+
+
+class QdpError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"qdp error {code}: {msg}")
+        self.code = code
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise QdpError(rc, _lib.qdp_last_error().decode(errors="replace"))
+
+
+def qdp_last_error() -> str:
+    return _lib.qdp_last_error().decode(errors="replace")
+
+
+def qdp_kernel_launch_count() -> int:
+    return int(_lib.qdp_kernel_launch_count())
+
+
+class Lattice:
+    def __init__(self, handle: int, dims, device: int):
+        self.handle, self.dims, self.device = handle, tuple(int(d) for d in dims), device
+        self.volume = int(np.prod(self.dims))
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h and _lib is not None:      # _lib is None during interpreter shutdown
+            _lib.qdp_lattice_destroy(h)
+
+
+class Field:
+    def __init__(self, handle: int, lat: Lattice, kind: int, prec: int, storage=None):
+        self.handle, self.lat, self.kind, self.prec, self.storage = handle, lat, kind, prec, storage
+
+    @property
+    def host_dtype(self):
+        return np.complex128 if self.prec == QDP_F64 else np.complex64
+
+    @property
+    def host_shape(self):
+        return (self.lat.volume,) + _SHAPE[self.kind]
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h and _lib is not None:
+            _lib.qdp_field_free(h)
+        self.storage = None
+
+
+def qdp_lattice_create(dims, device: int = 0) -> Lattice:
+    out = ctypes.c_void_p()
+    _check(_lib.qdp_lattice_create((ctypes.c_int * 4)(*[int(d) for d in dims]), device, ctypes.byref(out)))
+    return Lattice(out.value, dims, device)
+
+
+def qdp_lattice_destroy(lat: Lattice) -> None:
+    h, lat.handle = lat.handle, None
+    if h:
+        _check(_lib.qdp_lattice_destroy(h))
+
+
+def qdp_lattice_set_stream(lat: Lattice, cuda_stream: int | None) -> None:
+    _check(_lib.qdp_lattice_set_stream(lat.handle, cuda_stream))
+
+
+def qdp_lattice_sync(lat: Lattice) -> None:
+    _check(_lib.qdp_lattice_sync(lat.handle))
+
+
+def qdp_lattice_volume(lat: Lattice) -> int:
+    out = ctypes.c_int64()
+    _check(_lib.qdp_lattice_volume(lat.handle, ctypes.byref(out)))
+    return out.value
+
+
+def qdp_lattice_neighbor_table(lat: Lattice, mu: int, sign: int) -> np.ndarray:
+    out = np.empty(lat.volume, dtype=np.int32)
+    _check(_lib.qdp_lattice_neighbor_table(lat.handle, mu, sign, out.ctypes.data))
+    return out
+
+
+def qdp_lattice_parity_mask(lat: Lattice) -> np.ndarray:
+    out = np.empty(lat.volume, dtype=np.uint8)
+    _check(_lib.qdp_lattice_parity_mask(lat.handle, out.ctypes.data))
+    return out
+
+
+def qdp_set_allocator(alloc, free_, ctx=None) -> None:
+    """alloc/free_: ctypes callbacks of type ALLOC_FN / FREE_FN (keep them alive), or None."""
+    _check(_lib.qdp_set_allocator(ctypes.cast(alloc, _P) if alloc else None,
+                                  ctypes.cast(free_, _P) if free_ else None, ctx))
+
+
+def qdp_field_bytes(lat: Lattice, kind: int, prec: int) -> int:
+    out = _Z()
+    _check(_lib.qdp_field_bytes(lat.handle, kind, prec, ctypes.byref(out)))
+    return out.value
+
+
+def qdp_field_wrap(lat: Lattice, kind: int, prec: int, dev_ptr: int, nbytes: int, storage=None) -> Field:
+    out = ctypes.c_void_p()
+    _check(_lib.qdp_field_wrap(lat.handle, kind, prec, dev_ptr, nbytes, ctypes.byref(out)))
+    return Field(out.value, lat, kind, prec, storage)
+
+
+def qdp_field_alloc(lat: Lattice, kind: int, prec: int, use_torch: bool = True) -> Field:
+    """Device memory comes from PyTorch's caching allocator (a uint8 tensor wrapped with
+    qdp_field_wrap); use_torch=False lets the library allocate (qdp_field_alloc in C)."""
+    if use_torch:
+        import torch
+        nbytes = qdp_field_bytes(lat, kind, prec)
+        buf = torch.empty(nbytes, dtype=torch.uint8, device=f"cuda:{lat.device}")
+        return qdp_field_wrap(lat, kind, prec, buf.data_ptr(), nbytes, storage=buf)
+    out = ctypes.c_void_p()
+    _check(_lib.qdp_field_alloc(lat.handle, kind, prec, ctypes.byref(out)))
+    return Field(out.value, lat, kind, prec)
+
+
+def qdp_field_free(f: Field) -> None:
+    h, f.handle = f.handle, None
+    if h:
+        _check(_lib.qdp_field_free(h))
+    f.storage = None
+
+
+def _host_ptr(f: Field, host) -> int:
+    """host: numpy array (complex64/128, C-contiguous) or a CPU torch tensor (e.g. pinned)."""
+    if isinstance(host, np.ndarray):
+        if host.dtype != f.host_dtype or not host.flags.c_contiguous:
+            raise TypeError(f"host array must be C-contiguous {f.host_dtype}")
+        if host.size != int(np.prod(f.host_shape)):
+            raise ValueError("host array has the wrong number of elements")
+        return host.ctypes.data
+    nbytes = host.numel() * host.element_size()
+    if nbytes != qdp_field_bytes(f.lat, f.kind, f.prec) or not host.is_contiguous() or host.is_cuda:
+        raise ValueError("host tensor must be a contiguous CPU tensor of the field's byte size")
+    return host.data_ptr()
+
+
+def qdp_field_upload(f: Field, host) -> None:
+    _check(_lib.qdp_field_upload(f.handle, _host_ptr(f, host)))
+
+
+def qdp_field_download(f: Field, host=None):
+    if host is None:
+        host = np.empty(f.host_shape, dtype=f.host_dtype)
+    _check(_lib.qdp_field_download(f.handle, _host_ptr(f, host)))
+    return host
+
+
+def qdp_field_copy(dst: Field, src: Field) -> None:
+    _check(_lib.qdp_field_copy(dst.handle, src.handle))
+
+
+def field_from_host(lat: Lattice, kind: int, host: np.ndarray) -> Field:
+    prec = QDP_F64 if host.dtype == np.complex128 else QDP_F32
+    f = qdp_field_alloc(lat, kind, prec)
+    qdp_field_upload(f, np.ascontiguousarray(host))
+    return f
+
+
+def field_to_host(f: Field) -> np.ndarray:
+    return qdp_field_download(f)
+
+
+def qdp_shift(dst: Field, src: Field, mu: int, sign: int, subset: int = QDP_ALL) -> None:
+    _check(_lib.qdp_shift(dst.handle, src.handle, mu, sign, subset))
+
+
+def qdp_plaquette(u: Field, subset: int = QDP_ALL) -> np.ndarray:
+    out = np.empty(3)
+    _check(_lib.qdp_plaquette(u.handle, subset, out.ctypes.data))
+    return out
+
+
+def qdp_ape_smear_step(u_out: Field, u_in: Field, alpha: float, t_dir: int = 3, subset: int = QDP_ALL) -> None:
+    _check(_lib.qdp_ape_smear_step(u_out.handle, u_in.handle, float(alpha), t_dir, subset))
+
+
+def qdp_hop(chi: Field, u: Field, psi: Field, subset: int = QDP_ALL) -> None:
+    _check(_lib.qdp_hop(chi.handle, u.handle, psi.handle, subset))
+
+
+def qdp_axpy_hop(chi: Field, a: float, b: float, u: Field, psi: Field, subset: int = QDP_ALL,
+                 want_norm2: bool = False):
+    if want_norm2:
+        out = ctypes.c_double()
+        _check(_lib.qdp_axpy_hop(chi.handle, float(a), float(b), u.handle, psi.handle, subset, ctypes.addressof(out)))
+        return out.value
+    _check(_lib.qdp_axpy_hop(chi.handle, float(a), float(b), u.handle, psi.handle, subset, None))
+    return None
+
+
+def qdp_norm2(f: Field, subset: int = QDP_ALL) -> float:
+    out = ctypes.c_double()
+    _check(_lib.qdp_norm2(f.handle, subset, ctypes.addressof(out)))
+    return out.value
+
+
+def qdp_inner(a: Field, b: Field, subset: int = QDP_ALL) -> complex:
+    out = np.empty(2)
+    _check(_lib.qdp_inner(a.handle, b.handle, subset, out.ctypes.data))
+    return complex(out[0], out[1])
+
+
+def qdp_sum(f: Field, subset: int = QDP_ALL) -> np.ndarray:
+    out = np.empty(2 * _NCOMP[f.kind])
+    _check(_lib.qdp_sum(f.handle, subset, out.ctypes.data))
+    return (out[0::2] + 1j * out[1::2]).reshape(_SHAPE[f.kind])

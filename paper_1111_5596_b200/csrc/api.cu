@@ -1,0 +1,460 @@
+// api.cu -- the C ABI of include/qdp_b200.h: handles, argument validation, memory,
+// host<->device transfers and kernel dispatch.  No arithmetic of the method lives
+// here; every step of the path runs in the kernels of the other translation units.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/qdp_b200.h"
+#include "internal.h"
+
+using namespace qdp;
+
+// ---- error reporting ---------------------------------------------------------
+static thread_local char t_err[512] = "";
+
+static int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_err, sizeof t_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+#define CUDA_TRY(expr)                                                                     \
+    do {                                                                                   \
+        cudaError_t e_ = (expr);                                                           \
+        if (e_ != cudaSuccess)                                                             \
+            return fail(e_ == cudaErrorMemoryAllocation ? QDP_ERR_OOM : QDP_ERR_CUDA,      \
+                        "%s: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+// ---- allocator hook ----------------------------------------------------------
+static void* (*g_alloc)(size_t, void*) = nullptr;
+static void (*g_free)(void*, void*) = nullptr;
+static void* g_alloc_ctx = nullptr;
+
+static int dev_alloc(size_t bytes, void** out) {
+    if (g_alloc) {
+        *out = g_alloc(bytes, g_alloc_ctx);
+        if (!*out) return fail(QDP_ERR_OOM, "allocator hook returned NULL for %zu bytes", bytes);
+        return QDP_OK;
+    }
+    CUDA_TRY(cudaMalloc(out, bytes));
+    return QDP_OK;
+}
+static void dev_free(void* p, bool from_hook) {
+    if (!p) return;
+    if (from_hook && g_free) g_free(p, g_alloc_ctx);
+    else cudaFree(p);
+}
+
+// ---- handles -------------------------------------------------------------------
+static const uint32_t kLatMagic = 0x51445031u, kFieldMagic = 0x51445032u;
+static const int kStageSites = 1 << 15;   // sites per upload/download chunk
+
+struct qdp_lattice {
+    uint32_t magic;
+    int device;
+    int dims[4];
+    Geom geom;
+    cudaStream_t stream;
+    // scratch, all allocated at create time
+    double* partials;        // device: 4 * kMaxPartialBlocks, also 2*36*64 for sum
+    unsigned int* counter;   // device
+    double* result_dev;      // device: 72 doubles
+    double* result_host;     // pinned: 72 doubles
+    void* stage[2];          // device staging chunks for upload/download
+    size_t stage_bytes;
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_copied[2], ev_done[2];
+    bool scratch_from_hook;
+    int live_fields;
+};
+
+struct qdp_field {
+    uint32_t magic;
+    qdp_lattice* lat;
+    int kind, prec, ncomp;
+    void* data;
+    size_t bytes;
+    bool owned, from_hook;
+};
+
+static int kind_ncomp(int kind) {
+    switch (kind) {
+        case QDP_COLOR_MATRIX: return 9;
+        case QDP_GAUGE: return 36;
+        case QDP_FERMION: return 12;
+        default: return 0;
+    }
+}
+static size_t elem_bytes(int prec) { return prec == QDP_F64 ? 16 : 8; }
+
+static bool ok_lat(const qdp_lattice* l) { return l && l->magic == kLatMagic; }
+static bool ok_field(const qdp_field* f) { return f && f->magic == kFieldMagic && ok_lat(f->lat); }
+static bool ok_subset(int s) { return s == QDP_ALL || s == QDP_EVEN || s == QDP_ODD; }
+
+static ReduceBuf reduce_buf(qdp_lattice* l) {
+    ReduceBuf rb;
+    rb.partials = l->partials;
+    rb.counter = l->counter;
+    rb.result = l->result_dev;
+    return rb;
+}
+// copy n doubles of the device result to `out` and wait for them
+static int fetch_result(qdp_lattice* l, int n, double* out) {
+    CUDA_TRY(cudaMemcpyAsync(l->result_host, l->result_dev, n * sizeof(double), cudaMemcpyDeviceToHost, l->stream));
+    CUDA_TRY(cudaStreamSynchronize(l->stream));
+    memcpy(out, l->result_host, n * sizeof(double));
+    return QDP_OK;
+}
+
+struct DeviceGuard {
+    int prev;
+    bool ok;
+    explicit DeviceGuard(int dev) : prev(-1), ok(false) {
+        if (cudaGetDevice(&prev) != cudaSuccess) return;
+        ok = prev == dev || cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (ok && prev >= 0) cudaSetDevice(prev); }
+};
+#define ENTER(lat)                                                        \
+    DeviceGuard guard_((lat)->device);                                    \
+    if (!guard_.ok) return fail(QDP_ERR_CUDA, "cannot select CUDA device %d", (lat)->device)
+
+// ---- lattice -------------------------------------------------------------------
+extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** out) {
+    if (!dims || !out) return fail(QDP_ERR_ARG, "qdp_lattice_create: null argument");
+    long long V = 1;
+    for (int i = 0; i < 4; i++) {
+        if (dims[i] < 2 || (dims[i] & 1)) return fail(QDP_ERR_DIMS, "extent L%d = %d must be even and >= 2", i, dims[i]);
+        V *= dims[i];
+        if (V > (1ll << 31) / 36) return fail(QDP_ERR_DIMS, "volume too large for 32-bit site indices");
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(QDP_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+    if (device < 0 || device >= ndev) return fail(QDP_ERR_ARG, "device %d out of range (%d devices)", device, ndev);
+    qdp_lattice* l = new (std::nothrow) qdp_lattice();
+    if (!l) return fail(QDP_ERR_OOM, "host allocation failed");
+    memset(l, 0, sizeof *l);
+    l->magic = kLatMagic;
+    l->device = device;
+    memcpy(l->dims, dims, sizeof l->dims);
+    l->geom = Geom::make(dims);
+    ENTER(l);
+    l->scratch_from_hook = g_alloc != nullptr;
+    size_t npart = (size_t)4 * kMaxPartialBlocks;
+    if (npart < (size_t)2 * 36 * 64) npart = (size_t)2 * 36 * 64;
+    int rc;
+    void* p = nullptr;
+    if ((rc = dev_alloc(npart * sizeof(double), &p)) != QDP_OK) { delete l; return rc; }
+    l->partials = (double*)p;
+    if ((rc = dev_alloc(256, &p)) != QDP_OK) { delete l; return rc; }
+    l->counter = (unsigned int*)p;
+    if ((rc = dev_alloc(72 * sizeof(double), &p)) != QDP_OK) { delete l; return rc; }
+    l->result_dev = (double*)p;
+    CUDA_TRY(cudaMemset(l->counter, 0, 256));
+    CUDA_TRY(cudaMallocHost((void**)&l->result_host, 72 * sizeof(double)));
+    l->stage_bytes = (size_t)kStageSites * 36 * 16;
+    for (int i = 0; i < 2; i++) {
+        if ((rc = dev_alloc(l->stage_bytes, &l->stage[i])) != QDP_OK) { delete l; return rc; }
+        CUDA_TRY(cudaEventCreateWithFlags(&l->ev_copied[i], cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&l->ev_done[i], cudaEventDisableTiming));
+    }
+    CUDA_TRY(cudaStreamCreateWithFlags(&l->copy_stream, cudaStreamNonBlocking));
+    *out = l;
+    return QDP_OK;
+}
+
+extern "C" int qdp_lattice_destroy(qdp_lattice* l) {
+    if (!ok_lat(l)) return fail(QDP_ERR_ARG, "qdp_lattice_destroy: not a lattice");
+    if (l->live_fields) return fail(QDP_ERR_ARG, "qdp_lattice_destroy: %d fields still alive", l->live_fields);
+    ENTER(l);
+    cudaStreamSynchronize(l->stream);
+    cudaStreamSynchronize(l->copy_stream);
+    dev_free(l->partials, l->scratch_from_hook);
+    dev_free(l->counter, l->scratch_from_hook);
+    dev_free(l->result_dev, l->scratch_from_hook);
+    cudaFreeHost(l->result_host);
+    for (int i = 0; i < 2; i++) {
+        dev_free(l->stage[i], l->scratch_from_hook);
+        cudaEventDestroy(l->ev_copied[i]);
+        cudaEventDestroy(l->ev_done[i]);
+    }
+    cudaStreamDestroy(l->copy_stream);
+    l->magic = 0;
+    delete l;
+    return QDP_OK;
+}
+
+extern "C" int qdp_lattice_set_stream(qdp_lattice* l, void* cuda_stream) {
+    if (!ok_lat(l)) return fail(QDP_ERR_ARG, "qdp_lattice_set_stream: not a lattice");
+    l->stream = (cudaStream_t)cuda_stream;
+    return QDP_OK;
+}
+
+extern "C" int qdp_set_allocator(void* (*alloc)(size_t, void*), void (*free_)(void*, void*), void* ctx) {
+    if ((alloc == nullptr) != (free_ == nullptr)) return fail(QDP_ERR_ARG, "qdp_set_allocator: need both alloc and free");
+    g_alloc = alloc; g_free = free_; g_alloc_ctx = ctx;
+    return QDP_OK;
+}
+
+extern "C" int qdp_lattice_volume(const qdp_lattice* l, int64_t* out) {
+    if (!ok_lat(l) || !out) return fail(QDP_ERR_ARG, "qdp_lattice_volume: bad argument");
+    *out = l->geom.V;
+    return QDP_OK;
+}
+
+extern "C" int qdp_lattice_neighbor_table(qdp_lattice* l, int mu, int sign, int32_t* host_out) {
+    if (!ok_lat(l) || !host_out) return fail(QDP_ERR_ARG, "qdp_lattice_neighbor_table: bad argument");
+    if (mu < 0 || mu > 3 || (sign != 1 && sign != -1)) return fail(QDP_ERR_ARG, "mu must be 0..3 and sign +-1");
+    ENTER(l);
+    void* tmp = nullptr;
+    CUDA_TRY(cudaMalloc(&tmp, (size_t)l->geom.V * sizeof(int32_t)));
+    cudaError_t e = launch_neighbor_table(l->geom, mu, sign, (int32_t*)tmp, l->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(host_out, tmp, (size_t)l->geom.V * sizeof(int32_t), cudaMemcpyDeviceToHost, l->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(l->stream);
+    cudaFree(tmp);
+    CUDA_TRY(e);
+    return QDP_OK;
+}
+
+extern "C" int qdp_lattice_parity_mask(qdp_lattice* l, uint8_t* host_out) {
+    if (!ok_lat(l) || !host_out) return fail(QDP_ERR_ARG, "qdp_lattice_parity_mask: bad argument");
+    ENTER(l);
+    void* tmp = nullptr;
+    CUDA_TRY(cudaMalloc(&tmp, (size_t)l->geom.V));
+    cudaError_t e = launch_parity_mask(l->geom, (uint8_t*)tmp, l->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(host_out, tmp, (size_t)l->geom.V, cudaMemcpyDeviceToHost, l->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(l->stream);
+    cudaFree(tmp);
+    CUDA_TRY(e);
+    return QDP_OK;
+}
+
+extern "C" int qdp_lattice_sync(qdp_lattice* l) {
+    if (!ok_lat(l)) return fail(QDP_ERR_ARG, "qdp_lattice_sync: not a lattice");
+    ENTER(l);
+    CUDA_TRY(cudaStreamSynchronize(l->stream));
+    return QDP_OK;
+}
+
+// ---- fields --------------------------------------------------------------------
+extern "C" int qdp_field_bytes(const qdp_lattice* l, qdp_kind kind, qdp_prec prec, size_t* out) {
+    if (!ok_lat(l) || !out) return fail(QDP_ERR_ARG, "qdp_field_bytes: bad argument");
+    int nc = kind_ncomp(kind);
+    if (!nc) return fail(QDP_ERR_KIND, "unknown field kind %d", (int)kind);
+    if (prec != QDP_F32 && prec != QDP_F64) return fail(QDP_ERR_PREC, "unknown precision %d", (int)prec);
+    *out = (size_t)l->geom.V * nc * elem_bytes(prec);
+    return QDP_OK;
+}
+
+static int make_field(qdp_lattice* l, int kind, int prec, void* ptr, bool owned, qdp_field** out) {
+    qdp_field* f = new (std::nothrow) qdp_field();
+    if (!f) return fail(QDP_ERR_OOM, "host allocation failed");
+    f->magic = kFieldMagic;
+    f->lat = l; f->kind = kind; f->prec = prec; f->ncomp = kind_ncomp(kind);
+    f->bytes = (size_t)l->geom.V * f->ncomp * elem_bytes(prec);
+    f->data = ptr; f->owned = owned; f->from_hook = owned && g_alloc != nullptr;
+    l->live_fields++;
+    *out = f;
+    return QDP_OK;
+}
+
+extern "C" int qdp_field_alloc(qdp_lattice* l, qdp_kind kind, qdp_prec prec, qdp_field** out) {
+    size_t bytes;
+    int rc = qdp_field_bytes(l, kind, prec, &bytes);
+    if (rc != QDP_OK) return rc;
+    if (!out) return fail(QDP_ERR_ARG, "qdp_field_alloc: null out");
+    ENTER(l);
+    void* p = nullptr;
+    if ((rc = dev_alloc(bytes, &p)) != QDP_OK) return rc;
+    return make_field(l, kind, prec, p, true, out);
+}
+
+extern "C" int qdp_field_wrap(qdp_lattice* l, qdp_kind kind, qdp_prec prec, void* dev_ptr, size_t bytes,
+                              qdp_field** out) {
+    size_t need;
+    int rc = qdp_field_bytes(l, kind, prec, &need);
+    if (rc != QDP_OK) return rc;
+    if (!out || !dev_ptr) return fail(QDP_ERR_ARG, "qdp_field_wrap: null argument");
+    if (bytes < need) return fail(QDP_ERR_ARG, "qdp_field_wrap: %zu bytes given, %zu needed", bytes, need);
+    if ((uintptr_t)dev_ptr % 256) return fail(QDP_ERR_ARG, "qdp_field_wrap: pointer not 256-byte aligned");
+    return make_field(l, kind, prec, dev_ptr, false, out);
+}
+
+extern "C" int qdp_field_free(qdp_field* f) {
+    if (!ok_field(f)) return fail(QDP_ERR_ARG, "qdp_field_free: not a field");
+    ENTER(f->lat);
+    if (f->owned) {
+        cudaStreamSynchronize(f->lat->stream);
+        dev_free(f->data, f->from_hook);
+    }
+    f->lat->live_fields--;
+    f->magic = 0;
+    delete f;
+    return QDP_OK;
+}
+
+// Upload: chunks of kStageSites sites; the H2D copy of chunk k+1 (copy stream)
+// overlaps the transpose of chunk k (lattice stream); two staging buffers.
+extern "C" int qdp_field_upload(qdp_field* f, const void* host) {
+    if (!ok_field(f) || !host) return fail(QDP_ERR_ARG, "qdp_field_upload: bad argument");
+    qdp_lattice* l = f->lat;
+    ENTER(l);
+    const size_t site_bytes = (size_t)f->ncomp * elem_bytes(f->prec);
+    const int V = l->geom.V;
+    int k = 0;
+    for (int begin = 0; begin < V; begin += kStageSites, k ^= 1) {
+        int n = V - begin < kStageSites ? V - begin : kStageSites;
+        // staging buffer k is free once the transpose that last read it is done
+        CUDA_TRY(cudaStreamWaitEvent(l->copy_stream, l->ev_done[k], 0));
+        CUDA_TRY(cudaMemcpyAsync(l->stage[k], (const char*)host + (size_t)begin * site_bytes, (size_t)n * site_bytes,
+                                 cudaMemcpyHostToDevice, l->copy_stream));
+        CUDA_TRY(cudaEventRecord(l->ev_copied[k], l->copy_stream));
+        CUDA_TRY(cudaStreamWaitEvent(l->stream, l->ev_copied[k], 0));
+        CUDA_TRY(launch_aos_to_soa(f->prec, l->geom, f->ncomp, l->stage[k], f->data, begin, n, l->stream));
+        CUDA_TRY(cudaEventRecord(l->ev_done[k], l->stream));
+    }
+    CUDA_TRY(cudaStreamSynchronize(l->stream));
+    return QDP_OK;
+}
+
+extern "C" int qdp_field_download(const qdp_field* f, void* host) {
+    if (!ok_field(f) || !host) return fail(QDP_ERR_ARG, "qdp_field_download: bad argument");
+    qdp_lattice* l = f->lat;
+    ENTER(l);
+    const size_t site_bytes = (size_t)f->ncomp * elem_bytes(f->prec);
+    const int V = l->geom.V;
+    int k = 0;
+    for (int begin = 0; begin < V; begin += kStageSites, k ^= 1) {
+        int n = V - begin < kStageSites ? V - begin : kStageSites;
+        // staging buffer k is free once the D2H copy that last read it is done
+        CUDA_TRY(cudaStreamWaitEvent(l->stream, l->ev_copied[k], 0));
+        CUDA_TRY(launch_soa_to_aos(f->prec, l->geom, f->ncomp, f->data, l->stage[k], begin, n, l->stream));
+        CUDA_TRY(cudaEventRecord(l->ev_done[k], l->stream));
+        CUDA_TRY(cudaStreamWaitEvent(l->copy_stream, l->ev_done[k], 0));
+        CUDA_TRY(cudaMemcpyAsync((char*)host + (size_t)begin * site_bytes, l->stage[k], (size_t)n * site_bytes,
+                                 cudaMemcpyDeviceToHost, l->copy_stream));
+        CUDA_TRY(cudaEventRecord(l->ev_copied[k], l->copy_stream));
+    }
+    CUDA_TRY(cudaStreamSynchronize(l->copy_stream));
+    CUDA_TRY(cudaStreamSynchronize(l->stream));
+    return QDP_OK;
+}
+
+static int check_pair(const char* who, const qdp_field* a, const qdp_field* b) {
+    if (a->lat != b->lat) return fail(QDP_ERR_LATTICE, "%s: fields belong to different lattices", who);
+    if (a->prec != b->prec) return fail(QDP_ERR_PREC, "%s: fields differ in precision", who);
+    return QDP_OK;
+}
+static bool overlaps(const qdp_field* a, const qdp_field* b) {
+    const char *pa = (const char*)a->data, *pb = (const char*)b->data;
+    return pa < pb + b->bytes && pb < pa + a->bytes;
+}
+
+extern "C" int qdp_field_copy(qdp_field* dst, const qdp_field* src) {
+    if (!ok_field(dst) || !ok_field(src)) return fail(QDP_ERR_ARG, "qdp_field_copy: not a field");
+    int rc = check_pair("qdp_field_copy", dst, src);
+    if (rc != QDP_OK) return rc;
+    if (dst->kind != src->kind) return fail(QDP_ERR_KIND, "qdp_field_copy: kinds differ");
+    ENTER(dst->lat);
+    if (dst->data != src->data)
+        CUDA_TRY(cudaMemcpyAsync(dst->data, src->data, src->bytes, cudaMemcpyDeviceToDevice, dst->lat->stream));
+    return QDP_OK;
+}
+
+// ---- expressions ---------------------------------------------------------------
+extern "C" int qdp_shift(qdp_field* dst, const qdp_field* src, int mu, int sign, qdp_subset subset) {
+    if (!ok_field(dst) || !ok_field(src)) return fail(QDP_ERR_ARG, "qdp_shift: not a field");
+    if (mu < 0 || mu > 3 || (sign != 1 && sign != -1) || !ok_subset(subset))
+        return fail(QDP_ERR_ARG, "qdp_shift: mu must be 0..3, sign +-1, subset 0..2");
+    int rc = check_pair("qdp_shift", dst, src);
+    if (rc != QDP_OK) return rc;
+    if (dst->kind != src->kind) return fail(QDP_ERR_KIND, "qdp_shift: kinds differ");
+    if (overlaps(dst, src)) return fail(QDP_ERR_ALIAS, "qdp_shift: dst aliases src");
+    ENTER(dst->lat);
+    CUDA_TRY(launch_shift(dst->prec, dst->lat->geom, dst->ncomp, dst->data, src->data, mu, sign, subset, dst->lat->stream));
+    return QDP_OK;
+}
+
+extern "C" int qdp_plaquette(const qdp_field* u, qdp_subset subset, double out[3]) {
+    if (!ok_field(u) || !out || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_plaquette: bad argument");
+    if (u->kind != QDP_GAUGE) return fail(QDP_ERR_KIND, "qdp_plaquette: u must be a gauge field");
+    qdp_lattice* l = u->lat;
+    ENTER(l);
+    CUDA_TRY(launch_plaquette(u->prec, l->geom, u->data, subset, reduce_buf(l), l->stream));
+    return fetch_result(l, 3, out);
+}
+
+extern "C" int qdp_ape_smear_step(qdp_field* u_out, const qdp_field* u_in, double alpha, int t_dir,
+                                  qdp_subset subset) {
+    if (!ok_field(u_out) || !ok_field(u_in) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_ape_smear_step: bad argument");
+    if (t_dir != 3 && t_dir != -1) return fail(QDP_ERR_ARG, "qdp_ape_smear_step: t_dir must be 3 or -1");
+    if (u_out->kind != QDP_GAUGE || u_in->kind != QDP_GAUGE) return fail(QDP_ERR_KIND, "qdp_ape_smear_step: gauge fields needed");
+    int rc = check_pair("qdp_ape_smear_step", u_out, u_in);
+    if (rc != QDP_OK) return rc;
+    if (overlaps(u_out, u_in)) return fail(QDP_ERR_ALIAS, "qdp_ape_smear_step: u_out aliases u_in");
+    qdp_lattice* l = u_out->lat;
+    ENTER(l);
+    CUDA_TRY(launch_ape(u_out->prec, l->geom, u_out->data, u_in->data, alpha, t_dir, subset, l->stream));
+    return QDP_OK;
+}
+
+static int hop_common(const char* who, qdp_field* chi, const qdp_field* u, const qdp_field* psi, qdp_subset subset,
+                      bool axpy, double a, double b, double* norm2_out) {
+    if (!ok_field(chi) || !ok_field(u) || !ok_field(psi) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "%s: bad argument", who);
+    if (chi->kind != QDP_FERMION || psi->kind != QDP_FERMION || u->kind != QDP_GAUGE)
+        return fail(QDP_ERR_KIND, "%s: need (fermion, gauge, fermion)", who);
+    int rc = check_pair(who, chi, psi);
+    if (rc == QDP_OK) rc = check_pair(who, chi, u);
+    if (rc != QDP_OK) return rc;
+    if (overlaps(chi, psi)) return fail(QDP_ERR_ALIAS, "%s: chi aliases psi", who);
+    qdp_lattice* l = chi->lat;
+    ENTER(l);
+    CUDA_TRY(launch_hop(chi->prec, l->geom, chi->data, u->data, psi->data, subset, axpy, a, b, norm2_out != nullptr,
+                        reduce_buf(l), l->stream));
+    if (norm2_out) return fetch_result(l, 1, norm2_out);
+    return QDP_OK;
+}
+
+extern "C" int qdp_hop(qdp_field* chi, const qdp_field* u, const qdp_field* psi, qdp_subset subset) {
+    return hop_common("qdp_hop", chi, u, psi, subset, false, 0.0, 1.0, nullptr);
+}
+extern "C" int qdp_axpy_hop(qdp_field* chi, double a, double b, const qdp_field* u, const qdp_field* psi,
+                            qdp_subset subset, double* norm2_out) {
+    return hop_common("qdp_axpy_hop", chi, u, psi, subset, true, a, b, norm2_out);
+}
+
+extern "C" int qdp_norm2(const qdp_field* f, qdp_subset subset, double* out) {
+    if (!ok_field(f) || !out || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_norm2: bad argument");
+    qdp_lattice* l = f->lat;
+    ENTER(l);
+    CUDA_TRY(launch_norm2(f->prec, l->geom, f->ncomp, f->data, subset, reduce_buf(l), l->stream));
+    return fetch_result(l, 1, out);
+}
+
+extern "C" int qdp_inner(const qdp_field* a, const qdp_field* b, qdp_subset subset, double out[2]) {
+    if (!ok_field(a) || !ok_field(b) || !out || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_inner: bad argument");
+    int rc = check_pair("qdp_inner", a, b);
+    if (rc != QDP_OK) return rc;
+    if (a->kind != b->kind) return fail(QDP_ERR_KIND, "qdp_inner: kinds differ");
+    qdp_lattice* l = a->lat;
+    ENTER(l);
+    CUDA_TRY(launch_inner(a->prec, l->geom, a->ncomp, a->data, b->data, subset, reduce_buf(l), l->stream));
+    return fetch_result(l, 2, out);
+}
+
+extern "C" int qdp_sum(const qdp_field* f, qdp_subset subset, double* out) {
+    if (!ok_field(f) || !out || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_sum: bad argument");
+    qdp_lattice* l = f->lat;
+    ENTER(l);
+    CUDA_TRY(launch_sum(f->prec, l->geom, f->ncomp, f->data, subset, l->partials, l->result_dev, l->stream));
+    return fetch_result(l, 2 * f->ncomp, out);
+}
+
+extern "C" int64_t qdp_kernel_launch_count(void) { return g_launch_count; }
+
+extern "C" const char* qdp_last_error(void) { return t_err; }

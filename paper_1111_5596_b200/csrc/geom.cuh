@@ -1,0 +1,159 @@
+// geom.cuh -- lattice geometry on the device: internal site order, coordinates,
+// nearest-neighbour index arithmetic.  (DESIGN.md "Layout".)
+//
+// Internal site order ("checkerboard-lex"):
+//     s = parity(x) * V/2 + (lex(x) >> 1),   lex(x) = x0 + L0*(x1 + L1*(x2 + L2*x3))
+// Because L0 is even, lex pairs (2k, 2k+1) differ only in x0 and hence in parity,
+// so h = lex >> 1 enumerates each parity half once.  EVEN subset = [0, V/2),
+// ODD = [V/2, V): red/black operations touch contiguous memory, and every
+// neighbour of a site lies in the other half.
+//
+// No neighbour tables are read by the kernels: a neighbour index is a handful of
+// integer instructions on the decoded coordinates, which is cheaper than the
+// 32 B/site of table traffic it would replace on an HBM-bound path.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace qdp {
+
+// Division of n < 2^31 by a run-time constant d < 2^31: q = (n * m) >> sh.
+// m = ceil(2^(31+l) / d), l = ceil(log2 d)   (Granlund-Montgomery, N = 31 bits)
+struct FastDiv {
+    uint32_t d, m, sh;
+    __host__ static FastDiv make(uint32_t d) {
+        FastDiv f;
+        f.d = d;
+        uint32_t l = 0;
+        while ((1ull << l) < d) ++l;
+        f.sh = 31 + l;
+        f.m = (uint32_t)(((1ull << f.sh) + d - 1) / d);
+        return f;
+    }
+    __host__ __device__ __forceinline__ uint32_t div(uint32_t n) const {
+        return (uint32_t)(((uint64_t)n * m) >> sh);
+    }
+};
+
+struct Geom {
+    int L0, L1, L2, L3;
+    int Lh0;         // L0 / 2
+    int V, Vh;       // sites, sites per parity
+    int s1, s2, s3;  // strides of x1, x2, x3 in the half index h
+    FastDiv dLh0, dL1, dL2;
+
+    __host__ static Geom make(const int* L) {
+        Geom g;
+        g.L0 = L[0]; g.L1 = L[1]; g.L2 = L[2]; g.L3 = L[3];
+        g.Lh0 = L[0] / 2;
+        g.V = L[0] * L[1] * L[2] * L[3];
+        g.Vh = g.V / 2;
+        g.s1 = g.Lh0; g.s2 = g.Lh0 * L[1]; g.s3 = g.Lh0 * L[1] * L[2];
+        g.dLh0 = FastDiv::make(g.Lh0);
+        g.dL1 = FastDiv::make(L[1]);
+        g.dL2 = FastDiv::make(L[2]);
+        return g;
+    }
+};
+
+// A decoded site.  odd0 = x0 & 1 = (p + x1 + x2 + x3) & 1;  x0 = 2*hx + odd0.
+struct Site {
+    int p, h, hx, x1, x2, x3, odd0;
+    __device__ __forceinline__ int index(const Geom& g) const { return p * g.Vh + h; }
+    __device__ __forceinline__ int x0() const { return 2 * hx + odd0; }
+};
+
+__device__ __forceinline__ Site site_decode(const Geom& g, int p, int h) {
+    Site x;
+    x.p = p; x.h = h;
+    uint32_t r1 = g.dLh0.div((uint32_t)h);
+    x.hx = h - (int)r1 * g.Lh0;
+    uint32_t r2 = g.dL1.div(r1);
+    x.x1 = (int)r1 - (int)r2 * g.L1;
+    uint32_t r3 = g.dL2.div(r2);
+    x.x2 = (int)r2 - (int)r3 * g.L2;
+    x.x3 = (int)r3;
+    x.odd0 = (p + x.x1 + x.x2 + x.x3) & 1;
+    return x;
+}
+
+// internal index s in [0, V) -> Site
+__device__ __forceinline__ Site site_from_index(const Geom& g, int s) {
+    int p = s >= g.Vh;
+    return site_decode(g, p, s - p * g.Vh);
+}
+
+// x + sign * mu_hat with periodic wrap; MU, SIGN compile-time so it unrolls away.
+template <int MU, int SIGN>
+__device__ __forceinline__ Site site_step(const Geom& g, Site x) {
+    if (MU == 0) {
+        if (SIGN > 0) {
+            if (x.odd0) {
+                bool wrap = x.hx == g.Lh0 - 1;
+                x.h += wrap ? -(g.Lh0 - 1) : 1;
+                x.hx = wrap ? 0 : x.hx + 1;
+            }
+        } else {
+            if (!x.odd0) {
+                bool wrap = x.hx == 0;
+                x.h += wrap ? (g.Lh0 - 1) : -1;
+                x.hx = wrap ? g.Lh0 - 1 : x.hx - 1;
+            }
+        }
+    } else if (MU == 1) {
+        bool wrap = SIGN > 0 ? x.x1 == g.L1 - 1 : x.x1 == 0;
+        x.h += SIGN * (wrap ? -(g.L1 - 1) * g.s1 : g.s1);
+        x.x1 = wrap ? (SIGN > 0 ? 0 : g.L1 - 1) : x.x1 + SIGN;
+    } else if (MU == 2) {
+        bool wrap = SIGN > 0 ? x.x2 == g.L2 - 1 : x.x2 == 0;
+        x.h += SIGN * (wrap ? -(g.L2 - 1) * g.s2 : g.s2);
+        x.x2 = wrap ? (SIGN > 0 ? 0 : g.L2 - 1) : x.x2 + SIGN;
+    } else {
+        bool wrap = SIGN > 0 ? x.x3 == g.L3 - 1 : x.x3 == 0;
+        x.h += SIGN * (wrap ? -(g.L3 - 1) * g.s3 : g.s3);
+        x.x3 = wrap ? (SIGN > 0 ? 0 : g.L3 - 1) : x.x3 + SIGN;
+    }
+    x.p ^= 1;
+    if (MU == 0) x.odd0 ^= 1;   // for MU != 0 both p and x_MU change parity: odd0 = (p+x1+x2+x3)&1 is unchanged
+    return x;
+}
+
+// run-time direction (used by shift and the table export)
+__device__ __forceinline__ Site site_step_rt(const Geom& g, const Site& x, int mu, int sign) {
+    switch (mu * 2 + (sign < 0)) {
+        case 0: return site_step<0, +1>(g, x);
+        case 1: return site_step<0, -1>(g, x);
+        case 2: return site_step<1, +1>(g, x);
+        case 3: return site_step<1, -1>(g, x);
+        case 4: return site_step<2, +1>(g, x);
+        case 5: return site_step<2, -1>(g, x);
+        case 6: return site_step<3, +1>(g, x);
+        default: return site_step<3, -1>(g, x);
+    }
+}
+
+__device__ __forceinline__ int site_lex(const Geom& g, const Site& x) {
+    return x.x0() + g.L0 * (x.x1 + g.L1 * (x.x2 + g.L2 * x.x3));
+}
+
+// public lex index -> internal index
+__device__ __forceinline__ int lex_to_index(const Geom& g, int lex) {
+    int h = lex >> 1;
+    uint32_t r1 = g.dLh0.div((uint32_t)h);
+    uint32_t r2 = g.dL1.div(r1);
+    uint32_t r3 = g.dL2.div(r2);
+    int x1 = (int)r1 - (int)r2 * g.L1, x2 = (int)r2 - (int)r3 * g.L2, x3 = (int)r3;
+    int p = ((lex & 1) + x1 + x2 + x3) & 1;
+    return p * g.Vh + h;
+}
+
+// Map a linear work item to a site of the subset: subset 0 -> all V sites (both
+// halves, in internal order), 1 -> even half, 2 -> odd half.
+__device__ __forceinline__ int subset_count(const Geom& g, int subset) {
+    return subset == 0 ? g.V : g.Vh;
+}
+__device__ __forceinline__ int subset_index(const Geom& g, int subset, int i) {
+    return subset == 2 ? i + g.Vh : i;
+}
+
+}  // namespace qdp

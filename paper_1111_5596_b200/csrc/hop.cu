@@ -1,0 +1,103 @@
+// hop.cu -- chi(x) = sum_mu [ U_mu(x) psi(x+mu) + U_mu(x-mu)^dag psi(x-mu) ]   (def. 5)
+// and the fused chi = a psi + b hop(psi) with optional fused norm2 (def. 6).
+// (SURVEY.md 8(a) rows a7, a8.)  One kernel per expression, no lattice-sized
+// temporaries -- the point of the paper's expression fusion.
+//
+// One thread per updated site.  Per direction a thread issues 2 x (9 + 12)
+// independent 128-bit loads (fp64), all coalesced along the site index; the 8-fold
+// reuse of each psi(y) and 2-fold reuse of each link is left to L1/L2.
+#include "internal.h"
+#include "su3.cuh"
+
+namespace qdp {
+
+constexpr int kHopThreads = 128;
+
+template <class T, int MU>
+__device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
+                                        const typename Vec2<T>::type* __restrict__ u,
+                                        const typename Vec2<T>::type* __restrict__ psi, Spinor<T>& acc) {
+    const size_t V = (size_t)g.V;
+    {   // forward: U_mu(x) psi(x+mu)
+        const int sf = site_step<MU, +1>(g, x).index(g);
+        Mat3<T> U = ld_mat<T>(u, V, MU, s);
+        Spinor<T> p = ld_spinor<T>(psi, V, sf);
+#pragma unroll
+        for (int sp = 0; sp < 4; sp++)
+#pragma unroll
+            for (int a = 0; a < 3; a++)
+#pragma unroll
+                for (int b = 0; b < 3; b++) cmad(acc.e[sp * 3 + a], U.e[a * 3 + b], p.e[sp * 3 + b]);
+    }
+    {   // backward: U_mu(x-mu)^dag psi(x-mu)
+        const int sb = site_step<MU, -1>(g, x).index(g);
+        Mat3<T> U = ld_mat<T>(u, V, MU, sb);
+        Spinor<T> p = ld_spinor<T>(psi, V, sb);
+#pragma unroll
+        for (int sp = 0; sp < 4; sp++)
+#pragma unroll
+            for (int a = 0; a < 3; a++)
+#pragma unroll
+                for (int b = 0; b < 3; b++) cmad_conj_a(acc.e[sp * 3 + a], U.e[b * 3 + a], p.e[sp * 3 + b]);
+    }
+}
+
+template <class T, bool AXPY, bool NORM>
+__global__ void __launch_bounds__(kHopThreads) hop_kernel(Geom g, typename Vec2<T>::type* __restrict__ chi,
+                                                         const typename Vec2<T>::type* __restrict__ u,
+                                                         const typename Vec2<T>::type* __restrict__ psi,
+                                                         int subset, T a, T b, ReduceBuf rb) {
+    const int i = blockIdx.x * kHopThreads + threadIdx.x;
+    const bool active = i < subset_count(g, subset);
+    double n2[1] = {0.0};
+    if (active) {
+        const int s = subset_index(g, subset, i);
+        const Site x = site_from_index(g, s);
+        const size_t V = (size_t)g.V;
+        Spinor<T> acc;
+#pragma unroll
+        for (int c = 0; c < 12; c++) acc.e[c] = cx<T>(0, 0);
+        hop_dir<T, 0>(g, x, s, u, psi, acc);
+        hop_dir<T, 1>(g, x, s, u, psi, acc);
+        hop_dir<T, 2>(g, x, s, u, psi, acc);
+        hop_dir<T, 3>(g, x, s, u, psi, acc);
+        if (AXPY) {
+            Spinor<T> p = ld_spinor<T>(psi, V, s);
+#pragma unroll
+            for (int c = 0; c < 12; c++) {
+                // a*psi + b*hop: two roundings per part, like the definition
+                acc.e[c].re = a * p.e[c].re + b * acc.e[c].re;
+                acc.e[c].im = a * p.e[c].im + b * acc.e[c].im;
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 12; c++) {
+            st_cx<T>(chi, V, c, s, acc.e[c]);
+            if (NORM) n2[0] += (double)acc.e[c].re * (double)acc.e[c].re + (double)acc.e[c].im * (double)acc.e[c].im;
+        }
+    }
+    if (NORM) grid_reduce<1, kHopThreads>(n2, rb, nullptr);
+}
+
+template <class T>
+static cudaError_t launch_hop_t(const Geom& g, void* chi, const void* u, const void* psi, int subset,
+                                bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb,
+                                cudaStream_t st) {
+    using T2 = typename Vec2<T>::type;
+    int n = subset == 0 ? g.V : g.Vh;
+    int grid = (n + kHopThreads - 1) / kHopThreads;
+    T2* c = (T2*)chi; const T2* uu = (const T2*)u; const T2* p = (const T2*)psi;
+    if (!axpy)            hop_kernel<T, false, false><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
+    else if (!want_norm2) hop_kernel<T, true, false><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
+    else                  hop_kernel<T, true, true><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
+    g_launch_count++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hop(int prec, const Geom& g, void* chi, const void* u, const void* psi, int subset,
+                       bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb, cudaStream_t st) {
+    return prec ? launch_hop_t<double>(g, chi, u, psi, subset, axpy, a, b, want_norm2, rb, st)
+                : launch_hop_t<float>(g, chi, u, psi, subset, axpy, a, b, want_norm2, rb, st);
+}
+
+}  // namespace qdp

@@ -1,0 +1,51 @@
+// internal.h -- declarations shared by api.cu and the kernel translation units.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "geom.cuh"
+#include "reduce.cuh"
+
+namespace qdp {
+
+extern long long g_launch_count;   // kernels launched by this library
+
+// All launchers enqueue on `st` and return cudaGetLastError().
+// prec: 0 = fp32, 1 = fp64 (qdp_prec).  subset: 0 all, 1 even, 2 odd.
+
+// layout.cu
+cudaError_t launch_aos_to_soa(int prec, const Geom& g, int ncomp, const void* stage, void* field,
+                              int lex_begin, int nsites, cudaStream_t st);
+cudaError_t launch_soa_to_aos(int prec, const Geom& g, int ncomp, const void* field, void* stage,
+                              int lex_begin, int nsites, cudaStream_t st);
+cudaError_t launch_neighbor_table(const Geom& g, int mu, int sign, int32_t* out_lex, cudaStream_t st);
+cudaError_t launch_parity_mask(const Geom& g, uint8_t* out_lex, cudaStream_t st);
+
+// shift.cu
+cudaError_t launch_shift(int prec, const Geom& g, int ncomp, void* dst, const void* src, int mu,
+                         int sign, int subset, cudaStream_t st);
+
+// reduce.cu
+cudaError_t launch_norm2(int prec, const Geom& g, int ncomp, const void* f, int subset,
+                         const ReduceBuf& rb, cudaStream_t st);
+cudaError_t launch_inner(int prec, const Geom& g, int ncomp, const void* a, const void* b, int subset,
+                         const ReduceBuf& rb, cudaStream_t st);
+// out_dev: 2*ncomp doubles on the device; partials: scratch of 2*ncomp*nblk doubles
+cudaError_t launch_sum(int prec, const Geom& g, int ncomp, const void* f, int subset,
+                       double* partials, double* out_dev, cudaStream_t st);
+
+// hop.cu
+cudaError_t launch_hop(int prec, const Geom& g, void* chi, const void* u, const void* psi, int subset,
+                       bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb,
+                       cudaStream_t st);
+
+// plaquette.cu
+cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb,
+                             cudaStream_t st);
+
+// ape.cu
+cudaError_t launch_ape(int prec, const Geom& g, void* u_out, const void* u_in, double alpha, int t_dir,
+                       int subset, cudaStream_t st);
+
+}  // namespace qdp

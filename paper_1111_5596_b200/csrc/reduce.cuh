@@ -1,0 +1,78 @@
+// reduce.cuh -- deterministic global sums (hard part H4).
+//
+// Every reducing kernel ends in grid_reduce<K>(): warp shuffles, then a fixed
+// shared-memory tree over the warps of the block, then one partial per block in
+// a device buffer.  The last block to finish (ticket from an atomic counter)
+// sums the partials in block-index order with the same fixed tree and writes the
+// K results.  No floating-point atomics: the value depends only on the launch
+// shape, so repeated runs are bit-identical.  All accumulation is fp64.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace qdp {
+
+constexpr int kReduceThreads = 256;   // default block size of the reducing kernels
+constexpr int kMaxPartialBlocks = 148 * 16;
+
+struct ReduceBuf {
+    double* partials;        // [K][number of blocks], K <= 4
+    unsigned int* counter;   // zero between launches
+    double* result;          // [K] (device)
+};
+
+// NT = threads per block (multiple of 32, <= 1024)
+template <int K, int NT>
+__device__ __forceinline__ void block_tree(double (&v)[K], double (*sm)[NT / 32]) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < K; k++) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_down_sync(0xffffffffu, v[k], o);
+        if (lane == 0) sm[k][warp] = v[k];
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int k = 0; k < K; k++) {
+            double t = lane < NT / 32 ? sm[k][lane] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+            v[k] = t;   // valid in thread 0
+        }
+    }
+    __syncthreads();
+}
+
+// scale[k] multiplies result k (normalisation), applied once by the last block.
+template <int K, int NT = kReduceThreads>
+__device__ __forceinline__ void grid_reduce(double (&v)[K], const ReduceBuf& rb, const double* scale) {
+    __shared__ double sm[K][NT / 32];
+    __shared__ bool is_last;
+    const unsigned int nblk = gridDim.x * gridDim.y, bid = blockIdx.y * gridDim.x + blockIdx.x;
+    block_tree<K, NT>(v, sm);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < K; k++) rb.partials[k * nblk + bid] = v[k];
+        __threadfence();
+        unsigned int ticket = atomicAdd(rb.counter, 1u);
+        is_last = ticket == nblk - 1;
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    double t[K];
+#pragma unroll
+    for (int k = 0; k < K; k++) {
+        t[k] = 0.0;
+        for (unsigned int b = threadIdx.x; b < nblk; b += NT)
+            t[k] += __ldcg(&rb.partials[k * nblk + b]);
+    }
+    block_tree<K, NT>(t, sm);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < K; k++) rb.result[k] = scale ? t[k] * scale[k] : t[k];
+        *rb.counter = 0u;
+    }
+}
+
+}  // namespace qdp

@@ -1,0 +1,298 @@
+"""GPU-vs-oracle parity through the C ABI on the small configs (C1 4^4, 2^4, anisotropic
+extras, C2 16^3x32): element by element on the same seeded inputs.
+Bars (BASELINE.json:north_star): bit-exact for shifts / tables / masks / round trips;
+per-site relative error <= 1e-12 (fp64) / 2e-5 (fp32); global sums <= 1e-10 (fp64)."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from parity import TOL_SITE, TOL_SUM, links, site_rel_err, z3_fix
+
+pytestmark = pytest.mark.gpu
+
+SMALL = [(2, 2, 2, 2), (4, 4, 4, 4), (4, 2, 6, 4), (6, 4, 2, 8), (10, 6, 4, 2)]
+C2 = synth.CONFIGS["C2"]
+PRECS = ["f64", "f32"]
+SUBSETS = [0, 1, 2]
+KINDS = {"matrix": 0, "gauge": 1, "fermion": 2}
+
+
+def _seed(dims):
+    return synth.BASE_SEED + sum(dims)
+
+
+def _field(dims, kind, seed):
+    if kind == "matrix":
+        return synth.color_matrix(dims, seed)
+    if kind == "gauge":
+        return synth.gauge_hot(dims, seed)
+    return synth.spinor(dims, seed)
+
+
+def _as64(a):
+    return a.astype(np.complex128)
+
+
+@pytest.fixture(scope="module")
+def lat_cache(qdp):
+    cache = {}
+
+    def get(dims):
+        if dims not in cache:
+            cache[dims] = qdp.qdp_lattice_create(dims)
+        return cache[dims]
+    yield get
+    cache.clear()
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+def test_tables_and_masks_bit_exact(qdp, lat_cache, dims):
+    lat = lat_cache(dims)
+    assert qdp.qdp_lattice_volume(lat) == synth.volume(dims)
+    assert np.array_equal(qdp.qdp_lattice_parity_mask(lat), oracle.parity_mask(dims))
+    for mu in range(4):
+        for sign in (+1, -1):
+            assert np.array_equal(qdp.qdp_lattice_neighbor_table(lat, mu, sign),
+                                  oracle.neighbor_table(dims, mu, sign))
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_upload_download_round_trip_bit_exact(qdp, lat_cache, dims, prec):
+    lat = lat_cache(dims)
+    V = synth.volume(dims)
+    for kind, k in KINDS.items():
+        host = synth.round_to(_field(dims, kind, _seed(dims)), prec)
+        f = qdp.field_from_host(lat, k, host)
+        assert np.array_equal(qdp.field_to_host(f), host)
+    # a field filled with its own lex index pins the private permutation (A21)
+    idx = np.zeros((V, 3, 3), dtype=np.complex128)
+    idx[:] = np.arange(V)[:, None, None]
+    f = qdp.field_from_host(lat, 0, idx)
+    assert np.array_equal(qdp.field_to_host(f), idx)
+    s = qdp.qdp_sum(f)
+    assert np.array_equal(s, np.full((3, 3), V * (V - 1) / 2 + 0j))
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_shift_bit_exact(qdp, lat_cache, dims, prec):
+    lat = lat_cache(dims)
+    kinds = KINDS if dims != C2 else {"fermion": 2}
+    for kind, k in kinds.items():
+        host = synth.round_to(_field(dims, kind, _seed(dims) + 1), prec)
+        sentinel = synth.round_to(_field(dims, kind, _seed(dims) + 2), prec)
+        src = qdp.field_from_host(lat, k, host)
+        for mu in range(4):
+            for sign in (+1, -1):
+                for sub in SUBSETS:
+                    dst = qdp.field_from_host(lat, k, sentinel)
+                    qdp.qdp_shift(dst, src, mu, sign, sub)
+                    want = oracle.shift(dims, host, mu, sign, sub, dst=sentinel)
+                    assert np.array_equal(qdp.field_to_host(dst), want), (kind, mu, sign, sub)
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_reductions(qdp, lat_cache, dims, prec):
+    lat = lat_cache(dims)
+    tol = TOL_SUM[prec] if prec == "f64" else 1e-12   # fp32 inputs are exact in fp64: same bar applies
+    for kind, k in KINDS.items():
+        ha = synth.round_to(_field(dims, kind, _seed(dims) + 3), prec)
+        hb = synth.round_to(_field(dims, kind, _seed(dims) + 4), prec)
+        a, b = qdp.field_from_host(lat, k, ha), qdp.field_from_host(lat, k, hb)
+        for sub in SUBSETS:
+            n2 = oracle.norm2(dims, _as64(ha), sub)
+            got = qdp.qdp_norm2(a, sub)
+            assert abs(got - n2) <= tol * n2
+            assert got == qdp.qdp_norm2(a, sub)                       # run-to-run bit-identical
+            ip = oracle.inner(dims, _as64(ha), _as64(hb), sub)
+            scale = np.sqrt(n2 * oracle.norm2(dims, _as64(hb), sub))
+            assert abs(qdp.qdp_inner(a, b, sub) - ip) <= tol * scale
+            sm = oracle.sum_field(dims, _as64(ha), sub)
+            assert np.abs(qdp.qdp_sum(a, sub).ravel() - sm).max() <= tol * np.sqrt(n2 * synth.volume(dims))
+        assert abs(qdp.qdp_inner(a, a).real - qdp.qdp_norm2(a)) <= 1e-12 * qdp.qdp_norm2(a)
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_plaquette(qdp, lat_cache, dims, prec):
+    lat = lat_cache(dims)
+    variants = [synth.gauge_hot(dims, _seed(dims) + 5), synth.gauge_unit(dims)]
+    if dims == C2:
+        variants.append(synth.gauge_warm(dims, _seed(dims) + 5, 0.2))
+    for hu64 in variants:
+        hu = synth.round_to(hu64, prec)
+        u = qdp.field_from_host(lat, 1, hu)
+        for sub in SUBSETS:
+            want = oracle.plaquette(dims, _as64(hu), sub)
+            got = qdp.qdp_plaquette(u, sub)
+            # sums of O(V) terms of size <= 3, normalised by 9N or 18N: absolute bar
+            assert np.abs(got - want).max() <= TOL_SUM[prec], (sub, got, want)
+            assert np.array_equal(got, qdp.qdp_plaquette(u, sub))
+    unit = qdp.field_from_host(lat, 1, synth.round_to(synth.gauge_unit(dims), prec))
+    assert np.array_equal(qdp.qdp_plaquette(unit), [1.0, 1.0, 1.0])
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_hop_and_axpy_hop(qdp, lat_cache, dims, prec):
+    lat = lat_cache(dims)
+    hu = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 6), prec)
+    hp = synth.round_to(synth.spinor(dims, _seed(dims) + 7), prec)
+    sentinel = synth.round_to(synth.spinor(dims, _seed(dims) + 8, 1), prec)
+    u, psi = qdp.field_from_host(lat, 1, hu), qdp.field_from_host(lat, 2, hp)
+    a, b = synth.scalars_ab(_seed(dims))
+    if prec == "f32":
+        a, b = float(np.float32(a)), float(np.float32(b))
+    full = None
+    for sub in SUBSETS:
+        chi = qdp.field_from_host(lat, 2, sentinel)
+        qdp.qdp_hop(chi, u, psi, sub)
+        got = qdp.field_to_host(chi)
+        want = oracle.hop(dims, _as64(hu), _as64(hp), sub, chi=_as64(sentinel))
+        assert site_rel_err(got, want).max() <= TOL_SITE[prec], sub
+        if sub == 0:
+            full = got
+        chi2 = qdp.field_from_host(lat, 2, sentinel)
+        n2 = qdp.qdp_axpy_hop(chi2, a, b, u, psi, sub, want_norm2=True)
+        got2 = qdp.field_to_host(chi2)
+        want2 = oracle.axpy_hop(dims, a, b, _as64(hu), _as64(hp), sub, chi=_as64(sentinel))
+        assert site_rel_err(got2, want2).max() <= TOL_SITE[prec], sub
+        # fused norm2 == separate norm2 of the output (deterministic trees may differ in shape)
+        sep = qdp.qdp_norm2(chi2, sub)
+        assert abs(n2 - sep) <= 1e-12 * sep
+        assert abs(n2 - oracle.norm2(dims, want2, sub)) <= TOL_SUM[prec] * n2
+    # A17: even call then odd call into the same chi == full call, bit-exact
+    chi = qdp.field_from_host(lat, 2, sentinel)
+    qdp.qdp_hop(chi, u, psi, 1)
+    qdp.qdp_hop(chi, u, psi, 2)
+    assert np.array_equal(qdp.field_to_host(chi), full)
+    # inner(psi, hop psi) is real (A19: absolute bar 1e-10 * 8 * norm2)
+    ip = qdp.qdp_inner(psi, chi)
+    want_ip = oracle.inner(dims, _as64(hp), _as64(full))
+    n2p = oracle.norm2(dims, _as64(hp))
+    assert abs(ip - want_ip) <= 1e-10 * 8 * n2p
+    if prec == "f64":
+        assert abs(ip.imag) <= 1e-10 * 8 * n2p
+    # b = 0: chi = a psi exactly; a = 0, b = 1: hop exactly
+    chi3 = qdp.field_from_host(lat, 2, sentinel)
+    qdp.qdp_axpy_hop(chi3, a, 0.0, u, psi)
+    assert np.array_equal(qdp.field_to_host(chi3), (hp * hp.real.dtype.type(a)).astype(hp.dtype))
+    qdp.qdp_axpy_hop(chi3, 0.0, 1.0, u, psi)
+    assert np.array_equal(qdp.field_to_host(chi3), full)
+
+
+@pytest.mark.parametrize("dims", SMALL)
+@pytest.mark.parametrize("prec", PRECS)
+@pytest.mark.parametrize("t_dir", [3, -1])
+def test_ape_step(qdp, lat_cache, dims, prec, t_dir):
+    lat = lat_cache(dims)
+    hu = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 9), prec)
+    sentinel = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 10), prec)
+    u = qdp.field_from_host(lat, 1, hu)
+    for sub in SUBSETS:
+        out = qdp.field_from_host(lat, 1, sentinel)
+        qdp.qdp_ape_smear_step(out, u, 0.5, t_dir, sub)
+        got = qdp.field_to_host(out)
+        want = oracle.ape_smear_step(dims, _as64(hu), 0.5, t_dir, sub, u_out=_as64(sentinel))
+        fixed, n_centre = z3_fix(links(got).astype(np.complex128), links(want))
+        assert n_centre == 0                                      # A9: cut not hit on these inputs
+        assert site_rel_err(fixed, links(want)).max() <= TOL_SITE[prec], (sub, t_dir)
+        if t_dir == 3 and sub == 0:
+            assert np.array_equal(got[:, 3], hu[:, 3])            # A7: bit-exact copy
+    # unit field is a fixed point, exactly
+    unit = synth.round_to(synth.gauge_unit(dims), prec)
+    uu, out = qdp.field_from_host(lat, 1, unit), qdp.field_from_host(lat, 1, sentinel)
+    qdp.qdp_ape_smear_step(out, uu, 0.5, t_dir)
+    assert np.array_equal(qdp.field_to_host(out), unit)
+    # alpha = 0 is the identity
+    qdp.qdp_ape_smear_step(out, u, 0.0, t_dir)
+    assert site_rel_err(links(qdp.field_to_host(out)), links(_as64(hu))).max() <= TOL_SITE[prec]
+
+
+@pytest.mark.parametrize("prec", PRECS)
+def test_c2_ten_ape_steps_warm_and_hot(qdp, lat_cache, prec):
+    """BASELINE.json:configs[1]: 10 APE steps, plaquette after each (A16), hot + warm."""
+    dims = C2
+    lat = lat_cache(dims)
+    for name, hu64 in (("warm", synth.gauge_warm(dims, _seed(dims) + 11, 0.2)),
+                       ("hot", synth.gauge_hot(dims, _seed(dims) + 11))):
+        hu = synth.round_to(hu64, prec)
+        bufs = [qdp.field_from_host(lat, 1, hu), qdp.qdp_field_alloc(lat, 1, 1 if prec == "f64" else 0)]
+        ref = _as64(hu)
+        worst = 0.0
+        prev = None
+        for step in range(10):
+            qdp.qdp_ape_smear_step(bufs[1], bufs[0], 0.5, 3)
+            bufs.reverse()
+            ref = oracle.ape_smear_step(dims, ref, 0.5, 3)
+            pg, po = qdp.qdp_plaquette(bufs[0]), oracle.plaquette(dims, ref)
+            assert np.abs(pg - po).max() <= (1e-10 if prec == "f64" else 1e-5), (name, step)
+            if prev is not None:
+                assert pg[1] > prev                                 # smearing raises the plaquette
+            prev = pg[1]
+            if step in (0, 9):
+                got = links(qdp.field_to_host(bufs[0])).astype(np.complex128)
+                fixed, n_centre = z3_fix(got, links(ref))
+                assert n_centre == 0
+                worst = max(worst, site_rel_err(fixed, links(ref)).max())
+                eye = np.eye(3)
+                unit_bar = 1e-12 if prec == "f64" else 1e-5
+                assert np.abs(got @ np.conj(np.swapaxes(got, 1, 2)) - eye).max() <= unit_bar
+                assert np.abs(np.linalg.det(got) - 1).max() <= unit_bar
+        # error may grow over 10 chained steps; each step is within the bar, the chain within 10x
+        assert worst <= 10 * TOL_SITE[prec], (name, worst)
+
+
+def test_error_codes(qdp, lat_cache):
+    lat, lat2 = lat_cache((4, 4, 4, 4)), lat_cache((4, 2, 6, 4))
+    u = qdp.qdp_field_alloc(lat, 1, 1)
+    u32 = qdp.qdp_field_alloc(lat, 1, 0)
+    psi = qdp.qdp_field_alloc(lat, 2, 1)
+    chi = qdp.qdp_field_alloc(lat, 2, 1)
+    other = qdp.qdp_field_alloc(lat2, 2, 1)
+
+    def code(fn, *a):
+        with pytest.raises(qdp.QdpError) as e:
+            fn(*a)
+        return e.value.code
+
+    assert code(qdp.qdp_shift, psi, psi, 0, 1, 0) == -6
+    assert code(qdp.qdp_hop, psi, u, psi, 0) == -6
+    assert code(qdp.qdp_ape_smear_step, u, u, 0.5, 3, 0) == -6
+    assert code(qdp.qdp_hop, chi, u, other, 0) == -5
+    assert code(qdp.qdp_hop, chi, u32, psi, 0) == -4
+    assert code(qdp.qdp_hop, chi, psi, psi, 0) == -3
+    assert code(qdp.qdp_plaquette, psi, 0) == -3
+    assert code(qdp.qdp_shift, chi, psi, 4, 1, 0) == -1
+    assert code(qdp.qdp_shift, chi, psi, 0, 2, 0) == -1
+    assert code(qdp.qdp_shift, chi, psi, 0, 1, 3) == -1
+    assert code(qdp.qdp_ape_smear_step, u32, u32, 0.5, 2, 0) == -1
+    # library-owned allocation and the allocator hook
+    import ctypes, torch
+    f = qdp.qdp_field_alloc(lat, 2, 1, use_torch=False)
+    qdp.qdp_field_upload(f, synth.spinor((4, 4, 4, 4), 1))
+    assert qdp.qdp_norm2(f) > 0
+    qdp.qdp_field_free(f)
+    held = {}
+
+    def _alloc(n, ctx):
+        t = torch.empty(n, dtype=torch.uint8, device="cuda:0")
+        held[t.data_ptr()] = t
+        return t.data_ptr()
+
+    def _free(p, ctx):
+        held.pop(p, None)
+    a_cb, f_cb = qdp.binding.ALLOC_FN(_alloc), qdp.binding.FREE_FN(_free)
+    qdp.qdp_set_allocator(a_cb, f_cb)
+    try:
+        g = qdp.qdp_field_alloc(lat, 2, 1, use_torch=False)
+        assert len(held) == 1
+        qdp.qdp_field_upload(g, synth.spinor((4, 4, 4, 4), 1))
+        assert qdp.qdp_norm2(g) > 0
+        qdp.qdp_field_free(g)
+        assert len(held) == 0
+    finally:
+        qdp.qdp_set_allocator(None, None)
