@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- site-updates/s and achieved HBM GB/s of the hot path on one B200.
+
+A "step" is one pass of the whole hot path over one seeded
+synthetic lattice of BASELINE.json:configs[3] (C4, 32^3x64 fp64 -- the config the
+north_star quotes its 70 % target on):
+
+    shift(psi,+mu) | plaquette(u) | APE step u -> u' | hop on EVEN, hop on ODD |
+    inner(psi, chi) | chi = a psi + b hop(psi) with fused norm2 | norm2(chi)
+
+= 7 V site-updates.  `value` is site-updates/s with all inputs resident in HBM, timed with
+CUDA events on the lattice's stream; `e2e` is the same pass through the C ABI from pinned
+HOST buffers (upload u, psi; download u', chi inside the timed region).  Every field is
+larger than the 126 MB L2, so no explicit L2 flush is needed between iterations.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+N > 1 (torchrun): the path is single-GPU by contract ("replicas only"): every
+rank runs an independent replica; value = N * units / max-over-ranks time, scaling "weak".
+--impl reference times the oracle (plain single-threaded C, as it stands) on host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "site-updates/s"
+UNIT = "site-updates/s"
+OPS_PER_STEP = 7          # shift, plaquette, ape, hop(even+odd), inner, axpy_hop+norm2, norm2
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
+
+
+def algorithmic_bytes(V: int, eb: int) -> dict:
+    """every operand element read once, every result element written once.
+    eb = bytes per complex (16 fp64, 8 fp32).  Per launch on V sites."""
+    return {
+        "shift": V * 24 * eb,              # spinor: r 12 + w 12
+        "plaquette": V * 36 * eb,          # every link once
+        "ape": V * 72 * eb,                # full u_out contract: 36 r + 36 w (U_3 copied through)
+        "hop_even": (V // 2) * 96 * eb,    # 8 links (72) + psi 12 + chi 12 per updated site
+        "hop_odd": (V // 2) * 96 * eb,
+        "inner": V * 24 * eb,
+        "axpy_hop_norm2": V * 60 * eb,     # u 36 + psi 12 + chi 12
+        "norm2": V * 12 * eb,
+    }
+
+
+def measured_peak() -> tuple[float, str]:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(kernel)
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons during the timed region (pynvml)."""
+
+    def __init__(self, index: int, period: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._halt = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+        }
+        while not self._halt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self) -> dict:
+        self._halt.set()
+        self.join(timeout=1.0)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def run_ours(args) -> dict | None:
+    import torch
+    import synth
+    import paper_1111_5596_b200 as q
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    dims = synth.CONFIGS[args.config]
+    V = synth.volume(dims)
+    prec = args.prec
+    P = q.QDP_F64 if prec == "f64" else q.QDP_F32
+    eb = 16 if prec == "f64" else 8
+    seed = synth.BASE_SEED + 3 + rank
+    hu = synth.round_to(synth.gauge_hot(dims, seed), prec)
+    hp = synth.round_to(synth.spinor(dims, seed), prec)
+    a, b = synth.scalars_ab(seed)
+
+    stream = torch.cuda.Stream()
+    lat = q.qdp_lattice_create(dims, local)
+    q.qdp_lattice_set_stream(lat, stream.cuda_stream)
+    u, psi = q.field_from_host(lat, q.QDP_GAUGE, hu), q.field_from_host(lat, q.QDP_FERMION, hp)
+    u2 = q.qdp_field_alloc(lat, q.QDP_GAUGE, P)
+    chi, sh = q.qdp_field_alloc(lat, q.QDP_FERMION, P), q.qdp_field_alloc(lat, q.QDP_FERMION, P)
+
+    ops = [
+        ("shift", lambda k: q.qdp_shift(sh, psi, k % 4, 1 if (k // 4) % 2 == 0 else -1)),
+        ("plaquette", lambda k: q.qdp_plaquette(u)),
+        ("ape", lambda k: q.qdp_ape_smear_step(u2, u, 0.5, 3)),
+        ("hop_even", lambda k: q.qdp_hop(chi, u, psi, q.QDP_EVEN)),
+        ("hop_odd", lambda k: q.qdp_hop(chi, u, psi, q.QDP_ODD)),
+        ("inner", lambda k: q.qdp_inner(psi, chi)),
+        ("axpy_hop_norm2", lambda k: q.qdp_axpy_hop(chi, a, b, u, psi, q.QDP_ALL, want_norm2=True)),
+        ("norm2", lambda k: q.qdp_norm2(chi)),
+    ]
+    results = {}
+
+    def step(k, evs=None):
+        for i, (name, fn) in enumerate(ops):
+            if evs is not None:
+                evs[i].record(stream)
+            results[name] = fn(k)
+        if evs is not None:
+            evs[len(ops)].record(stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for k in range(args.warmup):
+        step(k)
+    K = args.steps
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(len(ops) + 1)] for _ in range(K)]
+    sampler = ClockSampler(local)
+    barrier()
+    launches0 = q.qdp_kernel_launch_count()
+    sampler.start()
+    for k in range(K):
+        step(k, evs[k])
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    launches = q.qdp_kernel_launch_count() - launches0
+    barrier()
+    total_ms = evs[0][0].elapsed_time(evs[K - 1][len(ops)])
+    per_op_ms = {name: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)]))
+                 for i, (name, _) in enumerate(ops)}
+
+    # ---- end to end through the C ABI from pinned host buffers ----------------------
+    ke = max(1, min(args.e2e_steps, K))
+    if args.no_e2e:
+        ke = 0
+    pin_u = torch.empty(hu.nbytes, dtype=torch.uint8, pin_memory=True)
+    pin_p = torch.empty(hp.nbytes, dtype=torch.uint8, pin_memory=True)
+    pin_u2 = torch.empty(hu.nbytes, dtype=torch.uint8, pin_memory=True)
+    pin_chi = torch.empty(hp.nbytes, dtype=torch.uint8, pin_memory=True)
+    pin_u.numpy()[:] = hu.view(np.uint8).ravel()
+    pin_p.numpy()[:] = hp.view(np.uint8).ravel()
+
+    def e2e_step(k):
+        q.qdp_field_upload(u, pin_u)
+        q.qdp_field_upload(psi, pin_p)
+        step(k)
+        q.qdp_field_download(u2, pin_u2)
+        q.qdp_field_download(chi, pin_chi)
+
+    e2e_s = 0.0
+    if ke:
+        e2e_step(0)
+        barrier()
+        t0 = time.perf_counter()
+        for k in range(ke):
+            e2e_step(k)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        barrier()
+
+    times = torch.tensor([total_ms, e2e_s * 1e3], dtype=torch.float64, device=f"cuda:{local}")
+    if dist is not None:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(times[0]), float(times[1])
+
+    out = None
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        alg = algorithmic_bytes(V, eb)
+        op_report = {}
+        for name, ms in per_op_ms.items():
+            gbs = alg[name] / ms / 1e6
+            sites = V // 2 if name.startswith("hop_") else V
+            op_report[name] = {"ms": round(ms, 5), "gbs": round(gbs, 1), "frac": round(gbs / peak, 4),
+                               "site_updates_per_s": sites / ms * 1e3}
+        dom = max(per_op_ms, key=per_op_ms.get)
+        dom_kernel = {"ape": "ape_kernel", "plaquette": "plaquette_kernel", "axpy_hop_norm2": "hop_kernel",
+                      "hop_even": "hop_kernel", "hop_odd": "hop_kernel"}.get(dom, dom + "_kernel")
+        units = OPS_PER_STEP * V * K * world
+        out = {
+            "metric": METRIC, "value": units / (total_ms * 1e-3), "unit": UNIT,
+            "n_gpus": world, "steps": K, "warmup": args.warmup, "ms_per_step": total_ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": prec, "data": "synthetic",
+            "config": {"workload": f"{args.config} {'x'.join(map(str, dims))} {prec}: shift, plaquette, "
+                                   "APE step (alpha=0.5, spatial) with SU(3) reprojection, hop even+odd, "
+                                   "inner, axpy_hop+norm2, norm2; hot (Haar) links",
+                       "sites": V, "site_updates_per_step": OPS_PER_STEP * V,
+                       "l2": "inputs larger than L2 (gauge 1.2 GB, spinor 0.4 GB vs 126 MB)",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "clocks": clocks,
+            "e2e": ({"value": OPS_PER_STEP * V * ke * world / (e2e_ms * 1e-3), "unit": UNIT,
+                     "h2d_bytes_per_step": int(hu.nbytes + hp.nbytes),
+                     "d2h_bytes_per_step": int(hu.nbytes + hp.nbytes),
+                     "steps": ke, "ms_per_step": e2e_ms / ke} if ke else None),
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "kernel": dom_kernel, "op": dom,
+                         "achieved": op_report[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                         "frac": op_report[dom]["frac"], "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": alg[dom], "traffic": ncu_traffic(dom_kernel)},
+            "ops": op_report,
+            "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(args, hu, hp, a, b, fraction=args.cpu_fraction)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return out
+
+
+def cpu_baseline(args, hu, hp, a, b, fraction: int) -> dict:
+    """The oracle as it stands, single-threaded, on a bounded sample: the first V/fraction
+    lex sites (whole time-slices) of the same lattice and inputs."""
+    import oracle
+    import synth
+    dims = synth.CONFIGS[args.config]
+    V = synth.volume(dims)
+    u = hu.astype(np.complex128, copy=False)
+    psi = hp.astype(np.complex128, copy=False)
+    chi, u_out, shifted = np.zeros_like(psi), np.zeros_like(u), np.zeros_like(psi)
+    n = V // fraction
+    t0 = time.perf_counter()
+    oracle.hot_path_sample(dims, u, psi, chi, u_out, shifted, a, b, 0, n)
+    dt = time.perf_counter() - t0
+    return {"value": OPS_PER_STEP * n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"lex sites [0, V/{fraction}) = {n} sites ({dims[3] // fraction} time-slices) of the same "
+                      f"lattice, one pass of the same 7 ops, {dt:.1f} s",
+            "host_cores_available": os.cpu_count()}
+
+
+def run_reference(args) -> dict | None:
+    """--impl reference: the oracle on host cores; each step is one time-slice-sized sample."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return None
+    import oracle
+    import synth
+    dims = synth.CONFIGS[args.config]
+    V = synth.volume(dims)
+    seed = synth.BASE_SEED + 3
+    hu = synth.round_to(synth.gauge_hot(dims, seed), args.prec).astype(np.complex128)
+    hp = synth.round_to(synth.spinor(dims, seed), args.prec).astype(np.complex128)
+    a, b = synth.scalars_ab(seed)
+    chi, u_out, shifted = np.zeros_like(hp), np.zeros_like(hu), np.zeros_like(hp)
+    n = V // dims[3]   # one time-slice per step
+    nslices = dims[3]
+
+    def step(k):
+        lo = (k % nslices) * n
+        oracle.hot_path_sample(dims, hu, hp, chi, u_out, shifted, a, b, lo, lo + n)
+
+    for k in range(args.warmup):
+        step(k)
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        step(args.warmup + k)
+    dt = time.perf_counter() - t0
+    value = OPS_PER_STEP * n * args.steps / dt
+    sample = f"one x3 time-slice ({n} sites) of {args.config} per step, 7 ops, single thread"
+    return {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.config} {'x'.join(map(str, dims))} {args.prec}: the same 7-op pass, "
+                               "oracle (plain C, fp64) on host cores, bounded sample per step",
+                   "sites": V, "sample_sites_per_step": n},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-fraction", type=int, default=4, help="cpu_baseline runs on V/fraction sites")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    out = run_reference(args) if args.impl == "reference" else run_ours(args)
+    if out is not None:
+        print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

@@ -60,6 +60,14 @@ def _get():
             "orc_norm2": ([P, I, P, I], D),
             "orc_inner": ([P, I, P, P, I, P], None),
             "orc_sum": ([P, I, P, I, P], None),
+            # the same loops over lex sites [begin, end): bounded samples for bench.py
+            "orc_shift_bytes_range": ([P, Z, P, P, I, I, I, Z, Z], None),
+            "orc_plaquette_range": ([P, P, I, Z, Z, P], None),
+            "orc_ape_smear_step_range": ([P, P, P, D, I, I, Z, Z], None),
+            "orc_hop_range": ([P, P, P, P, I, Z, Z], None),
+            "orc_axpy_hop_range": ([P, D, D, P, P, P, I, Z, Z], None),
+            "orc_norm2_range": ([P, I, P, I, Z, Z], D),
+            "orc_inner_range": ([P, I, P, P, I, Z, Z, P], None),
         }
         for name, (args, res) in sig.items():
             f = getattr(lib, name)
@@ -208,3 +216,23 @@ def sum_field(dims, f, subset=ALL):
     out = np.empty(n)
     _get().orc_sum(_dims(dims), n, f.ctypes.data, subset, out.ctypes.data)
     return out[0::2] + 1j * out[1::2]
+
+
+def hot_path_sample(dims, u, psi, chi, u_out, shifted, a, b, lex_begin, lex_end):
+    """One pass of the hot path restricted to the lex sites
+    [lex_begin, lex_end) of a large lattice: shift, plaquette, APE step, hop on even then
+    odd sites, axpy_hop, norm2, inner.  All arrays complex128 and preallocated; outputs are
+    written in place.  Returns (plaquette[3], norm2, inner).  For bench.py's cpu_baseline."""
+    lib, d = _get(), _dims(dims)
+    lo, hi = int(lex_begin), int(lex_end)
+    lib.orc_shift_bytes_range(d, psi.nbytes // volume(dims), psi.ctypes.data, shifted.ctypes.data, 0, 1, ALL, lo, hi)
+    plaq = np.empty(3)
+    lib.orc_plaquette_range(d, u.ctypes.data, ALL, lo, hi, plaq.ctypes.data)
+    lib.orc_ape_smear_step_range(d, u.ctypes.data, u_out.ctypes.data, 0.5, 3, ALL, lo, hi)
+    lib.orc_hop_range(d, u.ctypes.data, psi.ctypes.data, chi.ctypes.data, EVEN, lo, hi)
+    lib.orc_hop_range(d, u.ctypes.data, psi.ctypes.data, chi.ctypes.data, ODD, lo, hi)
+    ip = np.empty(2)
+    lib.orc_inner_range(d, 24, psi.ctypes.data, chi.ctypes.data, ALL, lo, hi, ip.ctypes.data)
+    lib.orc_axpy_hop_range(d, a, b, u.ctypes.data, psi.ctypes.data, chi.ctypes.data, ALL, lo, hi)
+    n2 = lib.orc_norm2_range(d, 24, chi.ctypes.data, ALL, lo, hi)
+    return plaq, n2, complex(ip[0], ip[1])

@@ -127,17 +127,20 @@ void orc_parity_mask(const int *L, uint8_t *out) {
  * dst(x) = src(x + sign*mu_hat) for x in subset; other sites of dst untouched.
  * Pure data movement on opaque per-site records so it is bit-exact for any
  * element type. */
-void orc_shift_bytes(const int *L, size_t bytes_per_site, const void *src, void *dst,
-                     int mu, int sign, int subset) {
-    size_t V = volume(L);
+void orc_shift_bytes_range(const int *L, size_t bytes_per_site, const void *src, void *dst,
+                           int mu, int sign, int subset, size_t lex_begin, size_t lex_end) {
     const char *s = (const char *)src;
     char *d = (char *)dst;
-    for (size_t i = 0; i < V; i++) {
+    for (size_t i = lex_begin; i < lex_end; i++) {
         int x[4]; coords_of(L, i, x);
         if (!in_subset(x, subset)) continue;
         size_t j = hop_lex(L, x, mu, sign);
         memcpy(d + i * bytes_per_site, s + j * bytes_per_site, bytes_per_site);
     }
+}
+void orc_shift_bytes(const int *L, size_t bytes_per_site, const void *src, void *dst,
+                     int mu, int sign, int subset) {
+    orc_shift_bytes_range(L, bytes_per_site, src, dst, mu, sign, subset, 0, volume(L));
 }
 
 /* ---- plaquette (definition 2) ------------------------------------------- */
@@ -179,10 +182,14 @@ static double k_val(const ksum *k) { return k->s + k->c; }
  * out[1] = the 3 spatial planes (mu<nu<3), normalised 1/(3*3*N)
  * out[2] = the 3 temporal planes (nu=3),   normalised 1/(3*3*N)
  * N = number of sites in the subset (reading A4, A5). */
-void orc_plaquette(const int *L, const double *u, int subset, double *out3) {
-    size_t V = volume(L), n = 0;
+/* The same sums restricted to lex sites [lex_begin, lex_end): out3 gets the three
+ * normalised values with N = subset sites in the range.  orc_plaquette is the full
+ * range.  (Used by bench.py to time a bounded sample of a large lattice.) */
+void orc_plaquette_range(const int *L, const double *u, int subset, size_t lex_begin,
+                         size_t lex_end, double *out3) {
+    size_t n = 0;
     ksum ss = { 0, 0 }, st = { 0, 0 };
-    for (size_t s = 0; s < V; s++) {
+    for (size_t s = lex_begin; s < lex_end; s++) {
         int x[4]; coords_of(L, s, x);
         if (!in_subset(x, subset)) continue;
         n++;
@@ -196,6 +203,9 @@ void orc_plaquette(const int *L, const double *u, int subset, double *out3) {
     out3[0] = (sp + tp) / (6.0 * 3.0 * N);
     out3[1] = sp / (3.0 * 3.0 * N);
     out3[2] = tp / (3.0 * 3.0 * N);
+}
+void orc_plaquette(const int *L, const double *u, int subset, double *out3) {
+    orc_plaquette_range(L, u, subset, 0, volume(L), out3);
 }
 
 /* ---- SU(3) projection (definition 4, Appendix B) -------------------------- */
@@ -342,15 +352,18 @@ void orc_ape_site(const int *L, const double *u, size_t lex, int mu, double alph
     orc_proj_su3(V, out18);
 }
 
-void orc_ape_smear_step(const int *L, const double *u_in, double *u_out, double alpha, int t_dir,
-                        int subset) {
-    size_t V = volume(L);
-    for (size_t s = 0; s < V; s++) {
+void orc_ape_smear_step_range(const int *L, const double *u_in, double *u_out, double alpha,
+                              int t_dir, int subset, size_t lex_begin, size_t lex_end) {
+    for (size_t s = lex_begin; s < lex_end; s++) {
         int x[4]; coords_of(L, s, x);
         if (!in_subset(x, subset)) continue;
         for (int mu = 0; mu < 4; mu++)
             orc_ape_site(L, u_in, s, mu, alpha, t_dir, u_out + ((s * 4 + (size_t)mu) * 9) * 2);
     }
+}
+void orc_ape_smear_step(const int *L, const double *u_in, double *u_out, double alpha, int t_dir,
+                        int subset) {
+    orc_ape_smear_step_range(L, u_in, u_out, alpha, t_dir, subset, 0, volume(L));
 }
 
 /* ---- hop (definition 5) ---------------------------------------------------
@@ -374,20 +387,22 @@ void orc_hop_site(const int *L, const double *u, const double *psi, size_t lex, 
     memcpy(out24, chi, sizeof chi);
 }
 
-void orc_hop(const int *L, const double *u, const double *psi, double *chi, int subset) {
-    size_t V = volume(L);
-    for (size_t s = 0; s < V; s++) {
+void orc_hop_range(const int *L, const double *u, const double *psi, double *chi, int subset,
+                   size_t lex_begin, size_t lex_end) {
+    for (size_t s = lex_begin; s < lex_end; s++) {
         int x[4]; coords_of(L, s, x);
         if (!in_subset(x, subset)) continue;
         orc_hop_site(L, u, psi, s, chi + s * 24);
     }
 }
+void orc_hop(const int *L, const double *u, const double *psi, double *chi, int subset) {
+    orc_hop_range(L, u, psi, chi, subset, 0, volume(L));
+}
 
 /* chi = a psi + b hop(psi) on the subset (definition 6, axpy_hop). */
-void orc_axpy_hop(const int *L, double a, double b, const double *u, const double *psi,
-                  double *chi, int subset) {
-    size_t V = volume(L);
-    for (size_t s = 0; s < V; s++) {
+void orc_axpy_hop_range(const int *L, double a, double b, const double *u, const double *psi,
+                        double *chi, int subset, size_t lex_begin, size_t lex_end) {
+    for (size_t s = lex_begin; s < lex_end; s++) {
         int x[4]; coords_of(L, s, x);
         if (!in_subset(x, subset)) continue;
         double h[24];
@@ -395,25 +410,32 @@ void orc_axpy_hop(const int *L, double a, double b, const double *u, const doubl
         for (int i = 0; i < 24; i++) chi[s * 24 + i] = a * psi[s * 24 + i] + b * h[i];
     }
 }
+void orc_axpy_hop(const int *L, double a, double b, const double *u, const double *psi,
+                  double *chi, int subset) {
+    orc_axpy_hop_range(L, a, b, u, psi, chi, subset, 0, volume(L));
+}
 
 /* ---- global reductions (definition 6) -------------------------------------
  * reals = 2 * (complex components per site). Lexicographic order, compensated. */
-double orc_norm2(const int *L, int reals, const double *f, int subset) {
-    size_t V = volume(L);
+double orc_norm2_range(const int *L, int reals, const double *f, int subset, size_t lex_begin,
+                       size_t lex_end) {
     ksum k = { 0, 0 };
-    for (size_t s = 0; s < V; s++) {
+    for (size_t s = lex_begin; s < lex_end; s++) {
         int x[4]; coords_of(L, s, x);
         if (!in_subset(x, subset)) continue;
         for (int i = 0; i < reals; i++) k_add(&k, f[s * reals + i] * f[s * reals + i]);
     }
     return k_val(&k);
 }
+double orc_norm2(const int *L, int reals, const double *f, int subset) {
+    return orc_norm2_range(L, reals, f, subset, 0, volume(L));
+}
 
 /* out = sum_x sum_c conj(a_c(x)) b_c(x)  (conjugates its FIRST argument, A12). */
-void orc_inner(const int *L, int reals, const double *a, const double *b, int subset, double *out2) {
-    size_t V = volume(L);
+void orc_inner_range(const int *L, int reals, const double *a, const double *b, int subset,
+                     size_t lex_begin, size_t lex_end, double *out2) {
     ksum kr = { 0, 0 }, ki = { 0, 0 };
-    for (size_t s = 0; s < V; s++) {
+    for (size_t s = lex_begin; s < lex_end; s++) {
         int x[4]; coords_of(L, s, x);
         if (!in_subset(x, subset)) continue;
         for (int c = 0; c < reals / 2; c++) {
@@ -425,6 +447,9 @@ void orc_inner(const int *L, int reals, const double *a, const double *b, int su
     }
     out2[0] = k_val(&kr);
     out2[1] = k_val(&ki);
+}
+void orc_inner(const int *L, int reals, const double *a, const double *b, int subset, double *out2) {
+    orc_inner_range(L, reals, a, b, subset, 0, volume(L), out2);
 }
 
 /* out[c] = sum_x f_c(x), per real component (re, im interleaved like f). */

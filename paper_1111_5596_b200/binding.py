@@ -29,7 +29,8 @@ QDP_COLOR_MATRIX, QDP_GAUGE, QDP_FERMION = 0, 1, 2
 _NCOMP = {QDP_COLOR_MATRIX: 9, QDP_GAUGE: 36, QDP_FERMION: 12}
 _SHAPE = {QDP_COLOR_MATRIX: (3, 3), QDP_GAUGE: (4, 3, 3), QDP_FERMION: (4, 3)}
 
-LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libqdp_b200.so")
+# QDP_B200_LIB selects another build of the same library (e.g. a debug or tuning build)
+LIB_PATH = os.environ.get("QDP_B200_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libqdp_b200.so")
 if not os.path.exists(LIB_PATH):
     raise ImportError(
         f"{LIB_PATH} is missing: build it with `python -m paper_1111_5596_b200.build` "

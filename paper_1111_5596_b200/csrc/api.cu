@@ -145,7 +145,10 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     l->geom = Geom::make(dims);
     ENTER(l);
     l->scratch_from_hook = g_alloc != nullptr;
+    // partials: K <= 4 values per block; the fused kernels launch one block per 64..256
+    // sites, the streaming reductions at most kMaxPartialBlocks, qdp_sum 2*36*64 values
     size_t npart = (size_t)4 * kMaxPartialBlocks;
+    if (npart < (size_t)4 * ((size_t)l->geom.V / 64 + 1)) npart = (size_t)4 * ((size_t)l->geom.V / 64 + 1);
     if (npart < (size_t)2 * 36 * 64) npart = (size_t)2 * 36 * 64;
     int rc;
     void* p = nullptr;

@@ -156,4 +156,25 @@ __device__ __forceinline__ int subset_index(const Geom& g, int subset, int i) {
     return subset == 2 ? i + g.Vh : i;
 }
 
+// Work-item order for the neighbour-reading kernels.  For the full lattice the two
+// parities are interleaved warp by warp over the same run of 32 half-indices:
+//     item i -> parity (i >> 5) & 1, h = (i >> 6) * 32 + (i & 31)
+// so a site and its neighbours (which lie in the other half) are processed by
+// adjacent warps at the same time and each link / spinor comes from DRAM once; walking
+// the even half and then the odd half would stream every field twice.
+// Returns false for padding items (Vh not a multiple of 32).
+__device__ __forceinline__ int work_items(const Geom& g, int subset) {
+    return subset == 0 ? 2 * ((g.Vh + 31) & ~31) : g.Vh;
+}
+__device__ __forceinline__ bool work_site(const Geom& g, int subset, int i, int& p, int& h) {
+    if (subset == 0) {
+        p = (i >> 5) & 1;
+        h = ((i >> 6) << 5) + (i & 31);
+    } else {
+        p = subset == 2;
+        h = i;
+    }
+    return h < g.Vh;
+}
+
 }  // namespace qdp

@@ -48,11 +48,12 @@ __global__ void __launch_bounds__(kHopThreads) hop_kernel(Geom g, typename Vec2<
                                                          const typename Vec2<T>::type* __restrict__ psi,
                                                          int subset, T a, T b, ReduceBuf rb) {
     const int i = blockIdx.x * kHopThreads + threadIdx.x;
-    const bool active = i < subset_count(g, subset);
+    int p, h;
+    const bool active = i < work_items(g, subset) && work_site(g, subset, i, p, h);
     double n2[1] = {0.0};
     if (active) {
-        const int s = subset_index(g, subset, i);
-        const Site x = site_from_index(g, s);
+        const Site x = site_decode(g, p, h);
+        const int s = x.index(g);
         const size_t V = (size_t)g.V;
         Spinor<T> acc;
 #pragma unroll
@@ -84,7 +85,7 @@ static cudaError_t launch_hop_t(const Geom& g, void* chi, const void* u, const v
                                 bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb,
                                 cudaStream_t st) {
     using T2 = typename Vec2<T>::type;
-    int n = subset == 0 ? g.V : g.Vh;
+    int n = subset == 0 ? 2 * ((g.Vh + 31) & ~31) : g.Vh;
     int grid = (n + kHopThreads - 1) / kHopThreads;
     T2* c = (T2*)chi; const T2* uu = (const T2*)u; const T2* p = (const T2*)psi;
     if (!axpy)            hop_kernel<T, false, false><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
