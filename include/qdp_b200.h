@@ -118,7 +118,9 @@ int qdp_field_alloc(qdp_lattice* lat, qdp_kind kind, qdp_prec prec, qdp_field** 
 int qdp_field_wrap(qdp_lattice* lat, qdp_kind kind, qdp_prec prec, void* dev_ptr, size_t bytes,
                    qdp_field** out);
 int qdp_field_free(qdp_field* f);
-/* Bytes of device memory a field of this kind/precision occupies (= host bytes). */
+/* Bytes of device memory a field of this kind/precision occupies.  Equal to the host
+ * buffer size V * ncomp * sizeof(complex) when V/2 is a multiple of 32 (all BASELINE
+ * configs); otherwise slightly larger (padding lanes of the blocked device layout). */
 int qdp_field_bytes(const qdp_lattice* lat, qdp_kind kind, qdp_prec prec, size_t* out);
 
 /* Host (layout above) <-> device (private layout).  Synchronous: the host buffer

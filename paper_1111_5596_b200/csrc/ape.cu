@@ -3,85 +3,121 @@
 // first example of a non-kernel routine that dominates once the solver is on the
 // GPU.
 //
-// One thread per (site, mu).  A 128-thread block is 4 warps = the 4 directions of one
-// group of 32 consecutive half-indices; consecutive blocks alternate parity over the
-// same run (full lattice), so all the links a neighbourhood needs are touched by
-// neighbouring blocks at one time and come from DRAM once.  With t_dir = 3 the mu = 3 warps
-// copy U_3 through unchanged (bit-exact).
+// One thread per site; the thread walks the smeared directions mu one after the other
+// (rolled loop: one copy of the matrix code, ~30 KB, stays in the instruction cache).
+// Per mu the 2(|S|-1) staples are straight-line code with an explicit software pipeline:
+// the third matrix of a staple is requested before its first product starts, and the
+// first two matrices of the next staple (or, at the end, of the next mu) before its
+// second product starts, so about one 3x3 product (108 DFMA) of work hides each
+// request.  In fp64 the kernel is bound by the fp64 pipe, so the
+// point of the pipeline is to keep that pipe fed from 8-12 resident warps per SM.
+//
+// Neighbour indices: the half-index offset of a step +-mu depends only on x_mu (and on
+// x0's parity for mu = 0), so the offsets of x-nu+mu are the sum of the two one-step
+// offsets (geom.cuh); eight ints per thread replace all coordinate arithmetic in the loop.
 #include "internal.h"
 #include "su3.cuh"
 
 namespace qdp {
 
-constexpr int kApeThreads = 128;
+#ifndef APE_THREADS
+#define APE_THREADS 128
+#endif
+#ifndef APE_MIN_BLOCKS
+#define APE_MIN_BLOCKS 3
+#endif
+constexpr int kApeThreads = APE_THREADS;
 
-// S += U_nu(x) U_mu(x+nu) U_nu(x+mu)^dag + U_nu(x-nu)^dag U_mu(x-nu) U_nu(x-nu+mu)
-// mu, nu are run-time values: one copy of the matrix code serves every (mu, nu) pair,
-// which keeps the kernel small enough to stay in the instruction cache while the four
-// mu-warps of a block run different directions.
-template <class T>
-__device__ __forceinline__ void add_staples(const Geom& g, const Site& x, int s, int mu, int nu,
-                                            const typename Vec2<T>::type* __restrict__ u, Mat3<T>& S) {
-    const size_t V = (size_t)g.V;
-    {
-        const int s_pnu = site_step_rt(g, x, nu, +1).index(g);
-        const int s_pmu = site_step_rt(g, x, mu, +1).index(g);
-        Mat3<T> t = mul(ld_mat<T>(u, V, nu, s), ld_mat<T>(u, V, mu, s_pnu));
-        mad_mul_adj(S, t, ld_mat<T>(u, V, nu, s_pmu));
-    }
-    {
-        const Site xm = site_step_rt(g, x, nu, -1);
-        const int s_mnu = xm.index(g);
-        const int s_mnu_pmu = site_step_rt(g, xm, mu, +1).index(g);
-        Mat3<T> t = adj_mul(ld_mat<T>(u, V, nu, s_mnu), ld_mat<T>(u, V, mu, s_mnu));
-        mad_mul(S, t, ld_mat<T>(u, V, nu, s_mnu_pmu));
-    }
+__device__ __forceinline__ int sel4(const int (&a)[4], int i) {
+    return i == 0 ? a[0] : (i == 1 ? a[1] : (i == 2 ? a[2] : a[3]));
 }
 
-#ifndef APE_MIN_BLOCKS
-#define APE_MIN_BLOCKS 4
-#endif
 template <class T, bool FOURD>
-__global__ void __launch_bounds__(kApeThreads, APE_MIN_BLOCKS) ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out,
-                                                         const typename Vec2<T>::type* __restrict__ u,
-                                                         T alpha, int subset) {
-    const int mu = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int i = blockIdx.x * 32 + lane;    // site work item
+__global__ void __launch_bounds__(kApeThreads, APE_MIN_BLOCKS)
+ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out, const typename Vec2<T>::type* __restrict__ u,
+           T alpha, int subset) {
+    using T2 = typename Vec2<T>::type;
+    constexpr int ND = FOURD ? 4 : 3;        // smeared directions
+    constexpr int NS = 2 * (ND - 1);         // staples per link
+    const int i = blockIdx.x * kApeThreads + threadIdx.x;
     int p, h;
     if (i >= work_items(g, subset) || !work_site(g, subset, i, p, h)) return;
     const Site x = site_decode(g, p, h);
-    const int s = x.index(g);
-    const size_t V = (size_t)g.V;
-    if (!FOURD && mu == 3) {   // time links pass through unchanged
+    const int sb = p * g.Vhp + h;            // this site
+    const int ob = (1 - p) * g.Vhp + h;      // same half-index in the other parity
+    int dp[4], dm[4];                        // half-index offsets of x+mu, x-mu
+    dp[0] = site_step<0, +1>(g, x).h - h; dm[0] = site_step<0, -1>(g, x).h - h;
+    dp[1] = site_step<1, +1>(g, x).h - h; dm[1] = site_step<1, -1>(g, x).h - h;
+    dp[2] = site_step<2, +1>(g, x).h - h; dm[2] = site_step<2, -1>(g, x).h - h;
+    dp[3] = site_step<3, +1>(g, x).h - h; dm[3] = site_step<3, -1>(g, x).h - h;
+
+    if (!FOURD) {   // time links pass through unchanged (bit-exact)
+        const T2* src = site_ptr(u, 36, 27, sb);
+        T2* dst = site_ptr(out, 36, 27, sb);
+        T2 t[9];
 #pragma unroll
-        for (int c = 27; c < 36; c++) out[(size_t)c * V + s] = __ldg(u + (size_t)c * V + s);
-        return;
+        for (int c = 0; c < 9; c++) t[c] = __ldg(src + c * kLane);
+#pragma unroll
+        for (int c = 0; c < 9; c++) dst[c * kLane] = t[c];
     }
-    Mat3<T> S = mat_zero<T>();
-    const int ndir = FOURD ? 4 : 3;
+    const T w_staple = alpha / T(NS), w_link = T(1) - alpha;
+
+    // operands of staple k of direction mu (nu = mu+1+k/2 mod ND):
+    //   upper (k even): A = U_nu(x),    B = U_mu(x+nu), C = U_nu(x+mu):    S += (A B) C^dag
+    //   lower (k odd):  A = U_nu(x-nu), B = U_mu(x-nu), C = U_nu(x-nu+mu): S += (A^dag B) C
+    auto ptrA = [&](int mu, int k) -> const T2* {
+        int nu = mu + 1 + (k >> 1); if (nu >= ND) nu -= ND;
+        return site_ptr(u, 36, nu * 9, (k & 1) ? ob + sel4(dm, nu) : sb);
+    };
+    auto ptrB = [&](int mu, int k) -> const T2* {
+        int nu = mu + 1 + (k >> 1); if (nu >= ND) nu -= ND;
+        return site_ptr(u, 36, mu * 9, ob + ((k & 1) ? sel4(dm, nu) : sel4(dp, nu)));
+    };
+    auto ptrC = [&](int mu, int k) -> const T2* {
+        int nu = mu + 1 + (k >> 1); if (nu >= ND) nu -= ND;
+        return site_ptr(u, 36, nu * 9, (k & 1) ? sb + sel4(dm, nu) + sel4(dp, mu) : ob + sel4(dp, mu));
+    };
+
+    Mat3<T> A = ld_mat_at<T>(ptrA(0, 0)), B = ld_mat_at<T>(ptrB(0, 0));
 #pragma unroll 1
-    for (int nu = 0; nu < ndir; nu++) {
-        if (nu == mu) continue;
-        add_staples<T>(g, x, s, mu, nu, u, S);
+    for (int mu = 0; mu < ND; mu++) {
+        Mat3<T> S = mat_zero<T>();
+        Mat3<T> U;
+#pragma unroll
+        for (int k = 0; k < NS; k++) {
+            Mat3<T> C = ld_mat_at<T>(ptrC(mu, k));
+            Mat3<T> Tm = (k & 1) ? adj_mul(A, B) : mul(A, B);
+            if (k + 1 < NS) {
+                A = ld_mat_at<T>(ptrA(mu, k + 1));
+                B = ld_mat_at<T>(ptrB(mu, k + 1));
+            } else {
+                U = ld_mat_at<T>(site_ptr(u, 36, mu * 9, sb));
+            }
+            if (k & 1) mad_mul(S, Tm, C); else mad_mul_adj(S, Tm, C);
+        }
+        if (mu + 1 < ND) {   // first operands of the next direction, in flight during the projection
+            A = ld_mat_at<T>(ptrA(mu + 1, 0));
+            B = ld_mat_at<T>(ptrB(mu + 1, 0));
+        }
+        // (1-alpha) U + (alpha/n) S, then the projection, always in fp64: for fp32 fields the
+        // closed form on an ill-conditioned V^dag V (hot links: cond ~ 100) would lose ~2e-5 in
+        // fp32, the whole fp32 error budget.
+        Mat3<double> Vd;
+#pragma unroll
+        for (int c = 0; c < 9; c++) {
+            T re = w_link * U.e[c].re + w_staple * S.e[c].re;
+            T im = w_link * U.e[c].im + w_staple * S.e[c].im;
+            Vd.e[c] = cx<double>((double)re, (double)im);
+        }
+        Mat3<double> Pd = proj_su3(Vd);
+        T2* o = site_ptr(out, 36, mu * 9, sb);
+#pragma unroll
+        for (int c = 0; c < 9; c++) {
+            T2 v;
+            v.x = (T)Pd.e[c].re; v.y = (T)Pd.e[c].im;
+            o[c * kLane] = v;
+        }
     }
-    const T w_staple = alpha / T(FOURD ? 6 : 4), w_link = T(1) - alpha;
-    Mat3<T> U = ld_mat<T>(u, V, mu, s);
-#pragma unroll
-    for (int i2 = 0; i2 < 9; i2++) {
-        // (1-alpha) U + (alpha/n) S
-        U.e[i2].re = w_link * U.e[i2].re + w_staple * S.e[i2].re;
-        U.e[i2].im = w_link * U.e[i2].im + w_staple * S.e[i2].im;
-    }
-    // The projection always runs in fp64: for fp32 fields the closed-form eigenvalues
-    // of an ill-conditioned V^dag V (hot links: cond ~ 100) would lose ~2e-5 in fp32,
-    // the whole fp32 error budget; fp64 is half the fp32 rate on B200, so this is cheap.
-    Mat3<double> Vd;
-#pragma unroll
-    for (int i2 = 0; i2 < 9; i2++) Vd.e[i2] = cx<double>((double)U.e[i2].re, (double)U.e[i2].im);
-    Mat3<double> Pd = proj_su3<double>(Vd);
-#pragma unroll
-    for (int i2 = 0; i2 < 9; i2++) U.e[i2] = cx<T>((T)Pd.e[i2].re, (T)Pd.e[i2].im);
-    st_mat<T>(out, V, mu, s, U);
 }
 
 template <class T>
@@ -89,7 +125,7 @@ static cudaError_t launch_ape_t(const Geom& g, void* out, const void* in, double
                                 cudaStream_t st) {
     using T2 = typename Vec2<T>::type;
     int items = subset == 0 ? 2 * ((g.Vh + 31) & ~31) : g.Vh;
-    dim3 grid((items + 31) / 32);
+    dim3 grid((items + kApeThreads - 1) / kApeThreads);
     if (t_dir == 3) ape_kernel<T, false><<<grid, kApeThreads, 0, st>>>(g, (T2*)out, (const T2*)in, (T)alpha, subset);
     else            ape_kernel<T, true><<<grid, kApeThreads, 0, st>>>(g, (T2*)out, (const T2*)in, (T)alpha, subset);
     g_launch_count++;

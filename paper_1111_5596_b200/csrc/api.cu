@@ -130,7 +130,7 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     for (int i = 0; i < 4; i++) {
         if (dims[i] < 2 || (dims[i] & 1)) return fail(QDP_ERR_DIMS, "extent L%d = %d must be even and >= 2", i, dims[i]);
         V *= dims[i];
-        if (V > (1ll << 31) / 36) return fail(QDP_ERR_DIMS, "volume too large for 32-bit site indices");
+        if (V + 64 > (1ll << 31) / 36) return fail(QDP_ERR_DIMS, "volume too large for 32-bit element indices");
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
@@ -250,7 +250,7 @@ extern "C" int qdp_field_bytes(const qdp_lattice* l, qdp_kind kind, qdp_prec pre
     int nc = kind_ncomp(kind);
     if (!nc) return fail(QDP_ERR_KIND, "unknown field kind %d", (int)kind);
     if (prec != QDP_F32 && prec != QDP_F64) return fail(QDP_ERR_PREC, "unknown precision %d", (int)prec);
-    *out = (size_t)l->geom.V * nc * elem_bytes(prec);
+    *out = field_elems(l->geom, nc) * elem_bytes(prec);   // includes the padding lanes of the blocked layout
     return QDP_OK;
 }
 
@@ -259,7 +259,7 @@ static int make_field(qdp_lattice* l, int kind, int prec, void* ptr, bool owned,
     if (!f) return fail(QDP_ERR_OOM, "host allocation failed");
     f->magic = kFieldMagic;
     f->lat = l; f->kind = kind; f->prec = prec; f->ncomp = kind_ncomp(kind);
-    f->bytes = (size_t)l->geom.V * f->ncomp * elem_bytes(prec);
+    f->bytes = field_elems(l->geom, f->ncomp) * elem_bytes(prec);
     f->data = ptr; f->owned = owned; f->from_hook = owned && g_alloc != nullptr;
     l->live_fields++;
     *out = f;

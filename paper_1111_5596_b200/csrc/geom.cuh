@@ -2,11 +2,20 @@
 // nearest-neighbour index arithmetic.  (DESIGN.md "Layout".)
 //
 // Internal site order ("checkerboard-lex"):
-//     s = parity(x) * V/2 + (lex(x) >> 1),   lex(x) = x0 + L0*(x1 + L1*(x2 + L2*x3))
+//     s = parity(x) * Vhp + (lex(x) >> 1),   lex(x) = x0 + L0*(x1 + L1*(x2 + L2*x3))
+// with Vhp = V/2 rounded up to a multiple of 32 (= V/2 for every BASELINE config).
 // Because L0 is even, lex pairs (2k, 2k+1) differ only in x0 and hence in parity,
 // so h = lex >> 1 enumerates each parity half once.  EVEN subset = [0, V/2),
-// ODD = [V/2, V): red/black operations touch contiguous memory, and every
+// ODD = [Vhp, Vhp + V/2): red/black operations touch contiguous memory, and every
 // neighbour of a site lies in the other half.
+//
+// Field storage ("blocked structure of arrays"): sites are grouped
+// in blocks of 32 consecutive indices; inside a block the components are planes of 32
+// complex numbers:
+//     element(c, s) = ((s >> 5) * ncomp + c) * 32 + (s & 31)
+// A warp still moves 32 consecutive complex numbers (512 B fp64) per component, but all
+// components of a site now sit at compile-time offsets (c * 32 elements) from one base
+// address, so a 3x3 matrix costs one address computation instead of nine.
 //
 // No neighbour tables are read by the kernels: a neighbour index is a handful of
 // integer instructions on the decoded coordinates, which is cheaper than the
@@ -39,6 +48,7 @@ struct Geom {
     int L0, L1, L2, L3;
     int Lh0;         // L0 / 2
     int V, Vh;       // sites, sites per parity
+    int Vhp;         // Vh rounded up to a multiple of 32: index stride between the parity halves
     int s1, s2, s3;  // strides of x1, x2, x3 in the half index h
     FastDiv dLh0, dL1, dL2;
 
@@ -48,6 +58,7 @@ struct Geom {
         g.Lh0 = L[0] / 2;
         g.V = L[0] * L[1] * L[2] * L[3];
         g.Vh = g.V / 2;
+        g.Vhp = (g.Vh + 31) & ~31;
         g.s1 = g.Lh0; g.s2 = g.Lh0 * L[1]; g.s3 = g.Lh0 * L[1] * L[2];
         g.dLh0 = FastDiv::make(g.Lh0);
         g.dL1 = FastDiv::make(L[1]);
@@ -59,7 +70,7 @@ struct Geom {
 // A decoded site.  odd0 = x0 & 1 = (p + x1 + x2 + x3) & 1;  x0 = 2*hx + odd0.
 struct Site {
     int p, h, hx, x1, x2, x3, odd0;
-    __device__ __forceinline__ int index(const Geom& g) const { return p * g.Vh + h; }
+    __device__ __forceinline__ int index(const Geom& g) const { return p * g.Vhp + h; }
     __device__ __forceinline__ int x0() const { return 2 * hx + odd0; }
 };
 
@@ -77,10 +88,13 @@ __device__ __forceinline__ Site site_decode(const Geom& g, int p, int h) {
     return x;
 }
 
-// internal index s in [0, V) -> Site
-__device__ __forceinline__ Site site_from_index(const Geom& g, int s) {
-    int p = s >= g.Vh;
-    return site_decode(g, p, s - p * g.Vh);
+// element index of component c of site s in a field of ncomp components per site
+__host__ __device__ __forceinline__ size_t field_elem(int ncomp, int c, int s) {
+    return ((size_t)(s >> 5) * ncomp + c) * 32 + (s & 31);
+}
+// complex elements a field of ncomp components occupies (including the padding lanes)
+__host__ __device__ __forceinline__ size_t field_elems(const Geom& g, int ncomp) {
+    return (size_t)2 * g.Vhp * ncomp;
 }
 
 // x + sign * mu_hat with periodic wrap; MU, SIGN compile-time so it unrolls away.
@@ -144,7 +158,7 @@ __device__ __forceinline__ int lex_to_index(const Geom& g, int lex) {
     uint32_t r3 = g.dL2.div(r2);
     int x1 = (int)r1 - (int)r2 * g.L1, x2 = (int)r2 - (int)r3 * g.L2, x3 = (int)r3;
     int p = ((lex & 1) + x1 + x2 + x3) & 1;
-    return p * g.Vh + h;
+    return p * g.Vhp + h;
 }
 
 // Map a linear work item to a site of the subset: subset 0 -> all V sites (both
@@ -152,8 +166,14 @@ __device__ __forceinline__ int lex_to_index(const Geom& g, int lex) {
 __device__ __forceinline__ int subset_count(const Geom& g, int subset) {
     return subset == 0 ? g.V : g.Vh;
 }
+// i-th site of the subset in work order -> internal index (subset 0: even half, then odd half)
 __device__ __forceinline__ int subset_index(const Geom& g, int subset, int i) {
-    return subset == 2 ? i + g.Vh : i;
+    if (subset == 0) return i < g.Vh ? i : i - g.Vh + g.Vhp;
+    return subset == 2 ? i + g.Vhp : i;
+}
+__device__ __forceinline__ Site subset_site(const Geom& g, int subset, int i) {
+    int p = subset == 0 ? (i >= g.Vh) : (subset == 2);
+    return site_decode(g, p, subset == 0 && p ? i - g.Vh : i);
 }
 
 // Work-item order for the neighbour-reading kernels.  For the full lattice the two

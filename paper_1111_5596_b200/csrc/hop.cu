@@ -17,11 +17,10 @@ template <class T, int MU>
 __device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
                                         const typename Vec2<T>::type* __restrict__ u,
                                         const typename Vec2<T>::type* __restrict__ psi, Spinor<T>& acc) {
-    const size_t V = (size_t)g.V;
     {   // forward: U_mu(x) psi(x+mu)
         const int sf = site_step<MU, +1>(g, x).index(g);
-        Mat3<T> U = ld_mat<T>(u, V, MU, s);
-        Spinor<T> p = ld_spinor<T>(psi, V, sf);
+        Mat3<T> U = ld_mat<T>(u, 36, MU, s);
+        Spinor<T> p = ld_spinor<T>(psi, sf);
 #pragma unroll
         for (int sp = 0; sp < 4; sp++)
 #pragma unroll
@@ -31,8 +30,8 @@ __device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
     }
     {   // backward: U_mu(x-mu)^dag psi(x-mu)
         const int sb = site_step<MU, -1>(g, x).index(g);
-        Mat3<T> U = ld_mat<T>(u, V, MU, sb);
-        Spinor<T> p = ld_spinor<T>(psi, V, sb);
+        Mat3<T> U = ld_mat<T>(u, 36, MU, sb);
+        Spinor<T> p = ld_spinor<T>(psi, sb);
 #pragma unroll
         for (int sp = 0; sp < 4; sp++)
 #pragma unroll
@@ -54,7 +53,6 @@ __global__ void __launch_bounds__(kHopThreads) hop_kernel(Geom g, typename Vec2<
     if (active) {
         const Site x = site_decode(g, p, h);
         const int s = x.index(g);
-        const size_t V = (size_t)g.V;
         Spinor<T> acc;
 #pragma unroll
         for (int c = 0; c < 12; c++) acc.e[c] = cx<T>(0, 0);
@@ -63,7 +61,7 @@ __global__ void __launch_bounds__(kHopThreads) hop_kernel(Geom g, typename Vec2<
         hop_dir<T, 2>(g, x, s, u, psi, acc);
         hop_dir<T, 3>(g, x, s, u, psi, acc);
         if (AXPY) {
-            Spinor<T> p = ld_spinor<T>(psi, V, s);
+            Spinor<T> p = ld_spinor<T>(psi, s);
 #pragma unroll
             for (int c = 0; c < 12; c++) {
                 // a*psi + b*hop: two roundings per part, like the definition
@@ -71,9 +69,12 @@ __global__ void __launch_bounds__(kHopThreads) hop_kernel(Geom g, typename Vec2<
                 acc.e[c].im = a * p.e[c].im + b * acc.e[c].im;
             }
         }
+        typename Vec2<T>::type* o = site_ptr(chi, 12, 0, s);
 #pragma unroll
         for (int c = 0; c < 12; c++) {
-            st_cx<T>(chi, V, c, s, acc.e[c]);
+            typename Vec2<T>::type v;
+            v.x = acc.e[c].re; v.y = acc.e[c].im;
+            o[c * kLane] = v;
             if (NORM) n2[0] += (double)acc.e[c].re * (double)acc.e[c].re + (double)acc.e[c].im * (double)acc.e[c].im;
         }
     }
@@ -85,7 +86,7 @@ static cudaError_t launch_hop_t(const Geom& g, void* chi, const void* u, const v
                                 bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb,
                                 cudaStream_t st) {
     using T2 = typename Vec2<T>::type;
-    int n = subset == 0 ? 2 * ((g.Vh + 31) & ~31) : g.Vh;
+    int n = subset == 0 ? 2 * g.Vhp : g.Vh;
     int grid = (n + kHopThreads - 1) / kHopThreads;
     T2* c = (T2*)chi; const T2* uu = (const T2*)u; const T2* p = (const T2*)psi;
     if (!axpy)            hop_kernel<T, false, false><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);

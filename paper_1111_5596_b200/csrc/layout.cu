@@ -25,7 +25,6 @@ __global__ void __launch_bounds__(256) transpose_kernel(Geom g, int ncomp, T2* _
     const int site0 = blockIdx.x * kTileSites;
     const int ns = min(kTileSites, nsites - site0);
     const int nelem = ns * ncomp;
-    const size_t V = (size_t)g.V;
     T2* st = stage + (size_t)site0 * ncomp;
     if (TO_SOA) {
         for (int e = threadIdx.x; e < nelem; e += blockDim.x) {
@@ -36,13 +35,13 @@ __global__ void __launch_bounds__(256) transpose_kernel(Geom g, int ncomp, T2* _
         for (int e = threadIdx.x; e < nelem; e += blockDim.x) {
             int c = e / ns, j = e - c * ns;
             int s = lex_to_index(g, lex_begin + site0 + j);
-            field[(size_t)c * V + s] = tile[c * pitch + j];
+            field[field_elem(ncomp, c, s)] = tile[c * pitch + j];
         }
     } else {
         for (int e = threadIdx.x; e < nelem; e += blockDim.x) {
             int c = e / ns, j = e - c * ns;
             int s = lex_to_index(g, lex_begin + site0 + j);
-            tile[c * pitch + j] = field[(size_t)c * V + s];
+            tile[c * pitch + j] = field[field_elem(ncomp, c, s)];
         }
         __syncthreads();
         for (int e = threadIdx.x; e < nelem; e += blockDim.x) {
@@ -79,14 +78,14 @@ cudaError_t launch_soa_to_aos(int prec, const Geom& g, int ncomp, const void* fi
 __global__ void neighbor_table_kernel(Geom g, int mu, int sign, int32_t* __restrict__ out) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= g.V) return;
-    Site x = site_from_index(g, s);
+    Site x = subset_site(g, 0, s);
     Site y = site_step_rt(g, x, mu, sign);
     out[site_lex(g, x)] = site_lex(g, y);
 }
 __global__ void parity_mask_kernel(Geom g, uint8_t* __restrict__ out) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= g.V) return;
-    Site x = site_from_index(g, s);
+    Site x = subset_site(g, 0, s);
     out[site_lex(g, x)] = (uint8_t)x.p;
 }
 

@@ -1,54 +1,86 @@
 // plaquette.cu -- sum_x sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag]
 // fused with its global sum (def. 2).
 //
-// Per plane the thread forms A = U_mu(x) U_nu(x+mu) and B = U_nu(x) U_mu(x+nu) and
-// takes Re tr(A B^dag) = sum_ij Re(A_ij conj(B_ij)): two 3x3 products and an
-// 18-term dot product instead of three products and a trace (1404 FMA per site).
+// Per plane the thread forms P = U_mu(x) U_nu(x+mu) and Q = U_nu(x) U_mu(x+nu) and
+// takes Re tr(P Q^dag) = sum_ij Re(P_ij conj(Q_ij)): two 3x3 products and an
+// 18-term dot product instead of three products and a trace (1404 FMA per site); Q is
+// never materialised, each entry goes straight into the dot product.
+//
+// One thread per site, rolled loop over the six planes (one copy of the matrix code) with an
+// explicit software pipeline: the operands of Q are requested before P is computed and
+// the operands of the next plane's P before Q is computed, so one 3x3 product (108 DFMA)
+// of work covers each request.  Neighbour indices are four precomputed half-index offsets.
 #include "internal.h"
 #include "su3.cuh"
 
 namespace qdp {
 
-constexpr int kPlaqThreads = 128;
-
-// Re tr P_{mu nu}(x); mu, nu run-time so that one copy of the matrix code serves all
-// six planes (small kernel, modest register count).
-template <class T>
-__device__ __forceinline__ T plaq_plane(const Geom& g, const Site& x, int s, int mu, int nu,
-                                        const typename Vec2<T>::type* __restrict__ u) {
-    const size_t V = (size_t)g.V;
-    const int s_pmu = site_step_rt(g, x, mu, +1).index(g);
-    const int s_pnu = site_step_rt(g, x, nu, +1).index(g);
-    Mat3<T> A = mul(ld_mat<T>(u, V, mu, s), ld_mat<T>(u, V, nu, s_pmu));
-    Mat3<T> B = mul(ld_mat<T>(u, V, nu, s), ld_mat<T>(u, V, mu, s_pnu));
-    return re_tr_mul_adj(A, B);
-}
+#ifndef PLAQ_THREADS
+#define PLAQ_THREADS 128
+#endif
+#ifndef PLAQ_MIN_BLOCKS
+#define PLAQ_MIN_BLOCKS 2
+#endif
+constexpr int kPlaqThreads = PLAQ_THREADS;
 
 struct PlaqScale { double s[3]; };
 
-#ifndef PLAQ_MIN_BLOCKS
-#define PLAQ_MIN_BLOCKS 3
-#endif
-#ifndef PLAQ_UNROLL
-#define PLAQ_UNROLL 1
-#endif
-constexpr int kPlaqUnroll = PLAQ_UNROLL;
+// sum_ij Re(P_ij conj((A B)_ij))
 template <class T>
-__global__ void __launch_bounds__(kPlaqThreads, PLAQ_MIN_BLOCKS) plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u,
-                                                                int subset, ReduceBuf rb, PlaqScale sc) {
+__device__ __forceinline__ T re_tr_p_adj_ab(const Mat3<T>& P, const Mat3<T>& a, const Mat3<T>& b) {
+    T s0 = 0, s1 = 0, s2 = 0;   // three chains (one per row) keep the fp64 pipe's latency covered
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        T acc = 0;
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            Cx<T> q = a.e[i * 3] * b.e[j];
+            cmad(q, a.e[i * 3 + 1], b.e[3 + j]);
+            cmad(q, a.e[i * 3 + 2], b.e[6 + j]);
+            acc = fma(P.e[i * 3 + j].re, q.re, acc);
+            acc = fma(P.e[i * 3 + j].im, q.im, acc);
+        }
+        if (i == 0) s0 = acc; else if (i == 1) s1 = acc; else s2 = acc;
+    }
+    return s0 + s1 + s2;
+}
+
+template <class T>
+__global__ void __launch_bounds__(kPlaqThreads, PLAQ_MIN_BLOCKS)
+plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u, int subset, ReduceBuf rb, PlaqScale sc) {
+    using T2 = typename Vec2<T>::type;
     const int i = blockIdx.x * kPlaqThreads + threadIdx.x;
     double acc[3] = {0.0, 0.0, 0.0};   // all, spatial, temporal
     int p, h;
     if (i < work_items(g, subset) && work_site(g, subset, i, p, h)) {
         const Site x = site_decode(g, p, h);
-        const int s = x.index(g);
+        const int sb = p * g.Vhp + h;            // this site
+        const int ob = (1 - p) * g.Vhp + h;      // same half-index in the other parity
+        int dp[4];                               // half-index offsets of x+mu
+        dp[0] = site_step<0, +1>(g, x).h - h;
+        dp[1] = site_step<1, +1>(g, x).h - h;
+        dp[2] = site_step<2, +1>(g, x).h - h;
+        dp[3] = site_step<3, +1>(g, x).h - h;
+        auto sel = [&](int d) { return d == 0 ? dp[0] : (d == 1 ? dp[1] : (d == 2 ? dp[2] : dp[3])); };
+        // planes (0,1) (0,2) (1,2) (0,3) (1,3) (2,3): the first three are spatial
+        auto plane_mu = [](int pl) { return pl < 3 ? (pl == 2) : pl - 3; };
+        auto plane_nu = [](int pl) { return pl < 3 ? (pl == 0 ? 1 : 2) : 3; };
+        const T2* here = site_ptr(u, 36, 0, sb);
+        Mat3<T> A = ld_mat_at<T>(here + plane_mu(0) * 9 * kLane);
+        Mat3<T> B = ld_mat_at<T>(site_ptr(u, 36, plane_nu(0) * 9, ob + sel(plane_mu(0))));
         T sp = 0, tp = 0;
-#pragma unroll kPlaqUnroll
+#pragma unroll 1
         for (int pl = 0; pl < 6; pl++) {
-            // planes (0,1) (0,2) (1,2) (0,3) (1,3) (2,3): the first three are spatial
-            const int mu = pl < 3 ? (pl == 2) : pl - 3;
-            const int nu = pl < 3 ? (pl == 0 ? 1 : 2) : 3;
-            const T v = plaq_plane<T>(g, x, s, mu, nu, u);
+            const int mu = plane_mu(pl), nu = plane_nu(pl);
+            Mat3<T> A2 = ld_mat_at<T>(here + nu * 9 * kLane);                        // U_nu(x)
+            Mat3<T> B2 = ld_mat_at<T>(site_ptr(u, 36, mu * 9, ob + sel(nu)));        // U_mu(x+nu)
+            Mat3<T> P = mul(A, B);                                                   // U_mu(x) U_nu(x+mu)
+            if (pl + 1 < 6) {
+                const int mu1 = plane_mu(pl + 1), nu1 = plane_nu(pl + 1);
+                A = ld_mat_at<T>(here + mu1 * 9 * kLane);
+                B = ld_mat_at<T>(site_ptr(u, 36, nu1 * 9, ob + sel(mu1)));
+            }
+            const T v = re_tr_p_adj_ab(P, A2, B2);
             if (pl < 3) sp += v; else tp += v;
         }
         acc[1] = (double)sp;
@@ -61,7 +93,7 @@ __global__ void __launch_bounds__(kPlaqThreads, PLAQ_MIN_BLOCKS) plaquette_kerne
 cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb,
                              cudaStream_t st) {
     int n = subset == 0 ? g.V : g.Vh;
-    int items = subset == 0 ? 2 * ((g.Vh + 31) & ~31) : g.Vh;
+    int items = subset == 0 ? 2 * g.Vhp : g.Vh;
     int grid = (items + kPlaqThreads - 1) / kPlaqThreads;
     PlaqScale sc;
     sc.s[0] = 1.0 / (18.0 * (double)n);

@@ -1,7 +1,9 @@
 // reduce.cu -- norm2, innerProduct, sum over a subset (def. 6).
-// HBM-bound streaming reads: 16 B (fp64) per complex component, accumulated in
-// fp64.  The subset's sites are a contiguous range of every component plane
-// (checkerboard order), so the reads are fully coalesced for even/odd too.
+// HBM-bound streaming reads: 16 B (fp64) per complex component, accumulated in fp64.
+// In the blocked layout (geom.cuh) a parity half of a field is one contiguous range of
+// memory, so norm2 and inner are plain 128-bit streaming loops over [begin, begin + n)
+// for all three subsets.  Only lattices whose half volume is not a multiple of 32 have
+// padding lanes; those use the RAGGED instantiation, which masks them.
 #include "internal.h"
 #include "su3.cuh"
 
@@ -9,81 +11,92 @@ namespace qdp {
 
 constexpr int kUnroll = 4;
 
-// grid = (blocks per plane, ncomp): blockIdx.y is the component plane, so no
-// per-element division is needed to find the plane.
-static dim3 reduce_grid(int n, int ncomp) {
-    int per_block = kReduceThreads * kUnroll;
-    int bx = (n + per_block - 1) / per_block;
-    int cap = kMaxPartialBlocks / ncomp;
-    if (bx > cap) bx = cap;
-    if (bx < 1) bx = 1;
-    return dim3(bx, ncomp);
+static int stream_grid(size_t n) {
+    size_t per_block = (size_t)kReduceThreads * kUnroll;
+    size_t b = (n + per_block - 1) / per_block;
+    if (b > (size_t)kMaxPartialBlocks) b = kMaxPartialBlocks;
+    if (b < 1) b = 1;
+    return (int)b;
 }
 
-template <class T2>
+// element e of the field (e counted from the start of the buffer) belongs to a real site?
+template <int NCOMP>
+__device__ __forceinline__ bool real_lane(const Geom& g, unsigned e) {
+    const unsigned half = (unsigned)g.Vhp * NCOMP;
+    const unsigned eh = e >= half ? e - half : e;
+    const unsigned hs = (eh / (NCOMP * 32u)) * 32u + (eh & 31u);
+    return hs < (unsigned)g.Vh;
+}
+
+template <class T2, int NCOMP, bool RAGGED>
 __global__ void __launch_bounds__(kReduceThreads) norm2_kernel(Geom g, const T2* __restrict__ f, int subset,
                                                               ReduceBuf rb) {
-    const int n = subset_count(g, subset);
-    const T2* plane = f + (size_t)blockIdx.y * g.V + subset_index(g, subset, 0);
-    const int stride = gridDim.x * kReduceThreads;
+    const unsigned half = (unsigned)g.Vhp * NCOMP;
+    const unsigned begin = subset == 2 ? half : 0u, n = subset == 0 ? 2u * half : half;
+    const T2* p = f + begin;
+    const unsigned stride = gridDim.x * kReduceThreads;
     double acc[1] = {0.0};
-    int i = blockIdx.x * kReduceThreads + threadIdx.x;
-    for (; i + (kUnroll - 1) * stride < n; i += kUnroll * stride) {
+    unsigned e = blockIdx.x * kReduceThreads + threadIdx.x;
+    for (; e + (kUnroll - 1) * stride < n; e += kUnroll * stride) {
         T2 v[kUnroll];
 #pragma unroll
-        for (int k = 0; k < kUnroll; k++) v[k] = __ldg(plane + i + k * stride);
+        for (int k = 0; k < kUnroll; k++) v[k] = __ldg(p + e + k * stride);
 #pragma unroll
         for (int k = 0; k < kUnroll; k++)
-            acc[0] += (double)v[k].x * (double)v[k].x + (double)v[k].y * (double)v[k].y;
+            if (!RAGGED || real_lane<NCOMP>(g, begin + e + k * stride))
+                acc[0] += (double)v[k].x * (double)v[k].x + (double)v[k].y * (double)v[k].y;
     }
-    for (; i < n; i += stride) {
-        T2 v = __ldg(plane + i);
-        acc[0] += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+    for (; e < n; e += stride) {
+        T2 v = __ldg(p + e);
+        if (!RAGGED || real_lane<NCOMP>(g, begin + e))
+            acc[0] += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
     }
     grid_reduce<1>(acc, rb, nullptr);
 }
 
-template <class T2>
+template <class T2, int NCOMP, bool RAGGED>
 __global__ void __launch_bounds__(kReduceThreads) inner_kernel(Geom g, const T2* __restrict__ a,
                                                               const T2* __restrict__ b, int subset, ReduceBuf rb) {
-    const int n = subset_count(g, subset);
-    const size_t off = (size_t)blockIdx.y * g.V + subset_index(g, subset, 0);
-    const T2 *pa = a + off, *pb = b + off;
-    const int stride = gridDim.x * kReduceThreads;
+    const unsigned half = (unsigned)g.Vhp * NCOMP;
+    const unsigned begin = subset == 2 ? half : 0u, n = subset == 0 ? 2u * half : half;
+    const T2 *pa = a + begin, *pb = b + begin;
+    const unsigned stride = gridDim.x * kReduceThreads;
     double acc[2] = {0.0, 0.0};
-    int i = blockIdx.x * kReduceThreads + threadIdx.x;
-    for (; i + (kUnroll - 1) * stride < n; i += kUnroll * stride) {
+    unsigned e = blockIdx.x * kReduceThreads + threadIdx.x;
+    for (; e + (kUnroll - 1) * stride < n; e += kUnroll * stride) {
         T2 va[kUnroll], vb[kUnroll];
 #pragma unroll
         for (int k = 0; k < kUnroll; k++) {
-            va[k] = __ldg(pa + i + k * stride);
-            vb[k] = __ldg(pb + i + k * stride);
+            va[k] = __ldg(pa + e + k * stride);
+            vb[k] = __ldg(pb + e + k * stride);
         }
 #pragma unroll
-        for (int k = 0; k < kUnroll; k++) {   // conj(a) * b
-            acc[0] += (double)va[k].x * (double)vb[k].x + (double)va[k].y * (double)vb[k].y;
-            acc[1] += (double)va[k].x * (double)vb[k].y - (double)va[k].y * (double)vb[k].x;
-        }
+        for (int k = 0; k < kUnroll; k++)   // conj(a) * b
+            if (!RAGGED || real_lane<NCOMP>(g, begin + e + k * stride)) {
+                acc[0] += (double)va[k].x * (double)vb[k].x + (double)va[k].y * (double)vb[k].y;
+                acc[1] += (double)va[k].x * (double)vb[k].y - (double)va[k].y * (double)vb[k].x;
+            }
     }
-    for (; i < n; i += stride) {
-        T2 va = __ldg(pa + i), vb = __ldg(pb + i);
-        acc[0] += (double)va.x * (double)vb.x + (double)va.y * (double)vb.y;
-        acc[1] += (double)va.x * (double)vb.y - (double)va.y * (double)vb.x;
+    for (; e < n; e += stride) {
+        T2 va = __ldg(pa + e), vb = __ldg(pb + e);
+        if (!RAGGED || real_lane<NCOMP>(g, begin + e)) {
+            acc[0] += (double)va.x * (double)vb.x + (double)va.y * (double)vb.y;
+            acc[1] += (double)va.x * (double)vb.y - (double)va.y * (double)vb.x;
+        }
     }
     grid_reduce<2>(acc, rb, nullptr);
 }
 
-// sum: blockIdx.y = component plane; two kernels (partials, then a fixed-order finish)
+// sum: blockIdx.y = component; two kernels (partials, then a fixed-order finish)
 constexpr int kSumBlocks = 64;
 template <class T2>
-__global__ void __launch_bounds__(kReduceThreads) sum_partial_kernel(Geom g, const T2* __restrict__ f, int subset,
-                                                                    double* __restrict__ partials) {
+__global__ void __launch_bounds__(kReduceThreads) sum_partial_kernel(Geom g, int ncomp, const T2* __restrict__ f,
+                                                                    int subset, double* __restrict__ partials) {
     __shared__ double sm[2][kReduceThreads / 32];
     const int n = subset_count(g, subset);
-    const T2* plane = f + (size_t)blockIdx.y * g.V + subset_index(g, subset, 0);
     double acc[2] = {0.0, 0.0};
     for (int i = blockIdx.x * kReduceThreads + threadIdx.x; i < n; i += gridDim.x * kReduceThreads) {
-        T2 v = __ldg(plane + i);
+        T2 v = __ldg(f + field_elem(ncomp, blockIdx.y, subset_index(g, subset, i)));
         acc[0] += (double)v.x;
         acc[1] += (double)v.y;
     }
@@ -100,27 +113,57 @@ __global__ void sum_finish_kernel(int nblk, const double* __restrict__ partials,
     out[c * 2 + k] = t;
 }
 
+template <class T2, int NCOMP>
+static void norm2_dispatch(const Geom& g, const void* f, int subset, const ReduceBuf& rb, cudaStream_t st) {
+    size_t n = (size_t)g.Vhp * NCOMP * (subset == 0 ? 2 : 1);
+    int grid = stream_grid(n);
+    if (g.Vh == g.Vhp) norm2_kernel<T2, NCOMP, false><<<grid, kReduceThreads, 0, st>>>(g, (const T2*)f, subset, rb);
+    else               norm2_kernel<T2, NCOMP, true><<<grid, kReduceThreads, 0, st>>>(g, (const T2*)f, subset, rb);
+}
+template <class T2, int NCOMP>
+static void inner_dispatch(const Geom& g, const void* a, const void* b, int subset, const ReduceBuf& rb,
+                           cudaStream_t st) {
+    size_t n = (size_t)g.Vhp * NCOMP * (subset == 0 ? 2 : 1);
+    int grid = stream_grid(n);
+    if (g.Vh == g.Vhp)
+        inner_kernel<T2, NCOMP, false><<<grid, kReduceThreads, 0, st>>>(g, (const T2*)a, (const T2*)b, subset, rb);
+    else
+        inner_kernel<T2, NCOMP, true><<<grid, kReduceThreads, 0, st>>>(g, (const T2*)a, (const T2*)b, subset, rb);
+}
+
 cudaError_t launch_norm2(int prec, const Geom& g, int ncomp, const void* f, int subset,
                          const ReduceBuf& rb, cudaStream_t st) {
-    dim3 grid = reduce_grid(subset == 0 ? g.V : g.Vh, ncomp);
-    if (prec) norm2_kernel<double2><<<grid, kReduceThreads, 0, st>>>(g, (const double2*)f, subset, rb);
-    else      norm2_kernel<float2><<<grid, kReduceThreads, 0, st>>>(g, (const float2*)f, subset, rb);
+    if (prec) {
+        if (ncomp == 9) norm2_dispatch<double2, 9>(g, f, subset, rb, st);
+        else if (ncomp == 12) norm2_dispatch<double2, 12>(g, f, subset, rb, st);
+        else norm2_dispatch<double2, 36>(g, f, subset, rb, st);
+    } else {
+        if (ncomp == 9) norm2_dispatch<float2, 9>(g, f, subset, rb, st);
+        else if (ncomp == 12) norm2_dispatch<float2, 12>(g, f, subset, rb, st);
+        else norm2_dispatch<float2, 36>(g, f, subset, rb, st);
+    }
     g_launch_count++;
     return cudaGetLastError();
 }
 cudaError_t launch_inner(int prec, const Geom& g, int ncomp, const void* a, const void* b, int subset,
                          const ReduceBuf& rb, cudaStream_t st) {
-    dim3 grid = reduce_grid(subset == 0 ? g.V : g.Vh, ncomp);
-    if (prec) inner_kernel<double2><<<grid, kReduceThreads, 0, st>>>(g, (const double2*)a, (const double2*)b, subset, rb);
-    else      inner_kernel<float2><<<grid, kReduceThreads, 0, st>>>(g, (const float2*)a, (const float2*)b, subset, rb);
+    if (prec) {
+        if (ncomp == 9) inner_dispatch<double2, 9>(g, a, b, subset, rb, st);
+        else if (ncomp == 12) inner_dispatch<double2, 12>(g, a, b, subset, rb, st);
+        else inner_dispatch<double2, 36>(g, a, b, subset, rb, st);
+    } else {
+        if (ncomp == 9) inner_dispatch<float2, 9>(g, a, b, subset, rb, st);
+        else if (ncomp == 12) inner_dispatch<float2, 12>(g, a, b, subset, rb, st);
+        else inner_dispatch<float2, 36>(g, a, b, subset, rb, st);
+    }
     g_launch_count++;
     return cudaGetLastError();
 }
 cudaError_t launch_sum(int prec, const Geom& g, int ncomp, const void* f, int subset,
                        double* partials, double* out_dev, cudaStream_t st) {
     dim3 grid(kSumBlocks, ncomp);
-    if (prec) sum_partial_kernel<double2><<<grid, kReduceThreads, 0, st>>>(g, (const double2*)f, subset, partials);
-    else      sum_partial_kernel<float2><<<grid, kReduceThreads, 0, st>>>(g, (const float2*)f, subset, partials);
+    if (prec) sum_partial_kernel<double2><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const double2*)f, subset, partials);
+    else      sum_partial_kernel<float2><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const float2*)f, subset, partials);
     sum_finish_kernel<<<ncomp, 2, 0, st>>>(kSumBlocks, partials, out_dev);
     g_launch_count += 2;
     return cudaGetLastError();
