@@ -3,8 +3,12 @@
 // first example of a non-kernel routine that dominates once the solver is on the
 // GPU.
 //
-// One thread per site; the thread walks the smeared directions mu one after the other
-// (rolled loop: one copy of the matrix code, ~30 KB, stays in the instruction cache).
+// One thread per site; the thread walks the smeared directions mu one after the other.  The
+// mu loop is unrolled: rolled, ptxas rotates the prefetched matrices of the next direction
+// through MOVs that wait for their loads (measured on C4 fp64: 0.83 ms rolled at 168
+// registers, 0.78 ms unrolled at 255; a variant that shares K = U_mu(x+nu) U_nu(x+mu)^dag
+// between the two upper staples of a plane needs 8 % fewer DFMA but two live staple sums,
+// spills, and measured 0.82 ms; persistent warps measured 0.99 ms -- DESIGN.md section 5).
 // Per mu the 2(|S|-1) staples are straight-line code with an explicit software pipeline:
 // the third matrix of a staple is requested before its first product starts, and the
 // first two matrices of the next staple (or, at the end, of the next mu) before its
@@ -23,17 +27,17 @@ namespace qdp {
 #ifndef APE_THREADS
 #define APE_THREADS 128
 #endif
-#ifndef APE_MIN_BLOCKS
-#define APE_MIN_BLOCKS 3
-#endif
 constexpr int kApeThreads = APE_THREADS;
+// fp64: 2 blocks of 128 threads per SM (255 registers, the software pipeline needs them);
+// fp32: 3 blocks (168 registers; the projection runs in fp64 for both)
+template <class T> struct ApeCfg { static constexpr int kMinBlocks = sizeof(T) == 8 ? 2 : 3; };
 
 __device__ __forceinline__ int sel4(const int (&a)[4], int i) {
     return i == 0 ? a[0] : (i == 1 ? a[1] : (i == 2 ? a[2] : a[3]));
 }
 
 template <class T, bool FOURD>
-__global__ void __launch_bounds__(kApeThreads, APE_MIN_BLOCKS)
+__global__ void __launch_bounds__(kApeThreads, ApeCfg<T>::kMinBlocks)
 ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out, const typename Vec2<T>::type* __restrict__ u,
            T alpha, int subset) {
     using T2 = typename Vec2<T>::type;
@@ -79,7 +83,7 @@ ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out, const typename Vec2
     };
 
     Mat3<T> A = ld_mat_at<T>(ptrA(0, 0)), B = ld_mat_at<T>(ptrB(0, 0));
-#pragma unroll 1
+#pragma unroll
     for (int mu = 0; mu < ND; mu++) {
         Mat3<T> S = mat_zero<T>();
         Mat3<T> U;

@@ -62,8 +62,8 @@ struct qdp_lattice {
     // scratch, all allocated at create time
     double* partials;        // device: 4 * kMaxPartialBlocks, also 2*36*64 for sum
     unsigned int* counter;   // device
-    double* result_dev;      // device: 72 doubles
-    double* result_host;     // pinned: 72 doubles
+    double* result_host;     // pinned, mapped: 72 doubles; the reducing kernels write their results here
+    double* result_dev;      // the device address of result_host
     void* stage[2];          // device staging chunks for upload/download
     size_t stage_bytes;
     cudaStream_t copy_stream;
@@ -102,9 +102,9 @@ static ReduceBuf reduce_buf(qdp_lattice* l) {
     rb.result = l->result_dev;
     return rb;
 }
-// copy n doubles of the device result to `out` and wait for them
+// The last block of a reducing kernel stores the n results straight into mapped pinned host
+// memory (no separate device-to-host copy to launch); wait for the kernel and hand them out.
 static int fetch_result(qdp_lattice* l, int n, double* out) {
-    CUDA_TRY(cudaMemcpyAsync(l->result_host, l->result_dev, n * sizeof(double), cudaMemcpyDeviceToHost, l->stream));
     CUDA_TRY(cudaStreamSynchronize(l->stream));
     memcpy(out, l->result_host, n * sizeof(double));
     return QDP_OK;
@@ -156,10 +156,9 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     l->partials = (double*)p;
     if ((rc = dev_alloc(256, &p)) != QDP_OK) { delete l; return rc; }
     l->counter = (unsigned int*)p;
-    if ((rc = dev_alloc(72 * sizeof(double), &p)) != QDP_OK) { delete l; return rc; }
-    l->result_dev = (double*)p;
     CUDA_TRY(cudaMemset(l->counter, 0, 256));
-    CUDA_TRY(cudaMallocHost((void**)&l->result_host, 72 * sizeof(double)));
+    CUDA_TRY(cudaHostAlloc((void**)&l->result_host, 72 * sizeof(double), cudaHostAllocMapped));
+    CUDA_TRY(cudaHostGetDevicePointer((void**)&l->result_dev, l->result_host, 0));
     l->stage_bytes = (size_t)kStageSites * 36 * 16;
     for (int i = 0; i < 2; i++) {
         if ((rc = dev_alloc(l->stage_bytes, &l->stage[i])) != QDP_OK) { delete l; return rc; }
@@ -179,7 +178,6 @@ extern "C" int qdp_lattice_destroy(qdp_lattice* l) {
     cudaStreamSynchronize(l->copy_stream);
     dev_free(l->partials, l->scratch_from_hook);
     dev_free(l->counter, l->scratch_from_hook);
-    dev_free(l->result_dev, l->scratch_from_hook);
     cudaFreeHost(l->result_host);
     for (int i = 0; i < 2; i++) {
         dev_free(l->stage[i], l->scratch_from_hook);

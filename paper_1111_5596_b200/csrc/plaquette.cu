@@ -6,10 +6,12 @@
 // 18-term dot product instead of three products and a trace (1404 FMA per site); Q is
 // never materialised, each entry goes straight into the dot product.
 //
-// One thread per site, rolled loop over the six planes (one copy of the matrix code) with an
-// explicit software pipeline: the operands of Q are requested before P is computed and
-// the operands of the next plane's P before Q is computed, so one 3x3 product (108 DFMA)
-// of work covers each request.  Neighbour indices are four precomputed half-index offsets.
+// One thread per site, the six planes fully unrolled (a rolled loop makes ptxas rotate the
+// prefetched matrices through MOVs that wait for the loads: measured 0.58 -> 0.42 ms on C4)
+// with an explicit software pipeline: the operands of Q are requested before P is computed
+// and the operands of the next plane's P before Q is computed, so one 3x3 product (108
+// DFMA) of work covers each request.  Neighbour indices are four precomputed half-index
+// offsets.  Warps are persistent (see the kernel) so the block reduction runs once.
 #include "internal.h"
 #include "su3.cuh"
 
@@ -22,6 +24,10 @@ namespace qdp {
 #define PLAQ_MIN_BLOCKS 2
 #endif
 constexpr int kPlaqThreads = PLAQ_THREADS;
+#ifndef PLAQ_UNROLL
+#define PLAQ_UNROLL 6
+#endif
+constexpr int kPlaqUnroll = PLAQ_UNROLL;
 
 struct PlaqScale { double s[3]; };
 
@@ -49,10 +55,18 @@ template <class T>
 __global__ void __launch_bounds__(kPlaqThreads, PLAQ_MIN_BLOCKS)
 plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u, int subset, ReduceBuf rb, PlaqScale sc) {
     using T2 = typename Vec2<T>::type;
-    const int i = blockIdx.x * kPlaqThreads + threadIdx.x;
+    // Persistent warps: warp w of the grid takes the 32-site work items w, w + W, w + 2W, ...
+    // (W = warps in the grid), so at any time the resident warps sweep one contiguous window
+    // of the lattice and the block-level reduction runs once per block, not once per 128 sites.
+    const int lane = threadIdx.x & 31;
+    const int nwarps = gridDim.x * (kPlaqThreads / 32);
+    const int nitems = (work_items(g, subset) + 31) >> 5;   // 32-site items (the last one may be ragged)
     double acc[3] = {0.0, 0.0, 0.0};   // all, spatial, temporal
-    int p, h;
-    if (i < work_items(g, subset) && work_site(g, subset, i, p, h)) {
+    for (int wi = blockIdx.x * (kPlaqThreads / 32) + (threadIdx.x >> 5); wi < nitems; wi += nwarps) {
+        const int i = wi * 32 + lane;
+        int p, h;
+        const bool live = i < work_items(g, subset) && work_site(g, subset, i, p, h);
+        if (!live) continue;
         const Site x = site_decode(g, p, h);
         const int sb = p * g.Vhp + h;            // this site
         const int ob = (1 - p) * g.Vhp + h;      // same half-index in the other parity
@@ -66,10 +80,10 @@ plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u, int subse
         auto plane_mu = [](int pl) { return pl < 3 ? (pl == 2) : pl - 3; };
         auto plane_nu = [](int pl) { return pl < 3 ? (pl == 0 ? 1 : 2) : 3; };
         const T2* here = site_ptr(u, 36, 0, sb);
+        T sp = 0, tp = 0;
         Mat3<T> A = ld_mat_at<T>(here + plane_mu(0) * 9 * kLane);
         Mat3<T> B = ld_mat_at<T>(site_ptr(u, 36, plane_nu(0) * 9, ob + sel(plane_mu(0))));
-        T sp = 0, tp = 0;
-#pragma unroll 1
+#pragma unroll kPlaqUnroll
         for (int pl = 0; pl < 6; pl++) {
             const int mu = plane_mu(pl), nu = plane_nu(pl);
             Mat3<T> A2 = ld_mat_at<T>(here + nu * 9 * kLane);                        // U_nu(x)
@@ -83,18 +97,30 @@ plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u, int subse
             const T v = re_tr_p_adj_ab(P, A2, B2);
             if (pl < 3) sp += v; else tp += v;
         }
-        acc[1] = (double)sp;
-        acc[2] = (double)tp;
-        acc[0] = acc[1] + acc[2];
+        acc[1] += (double)sp;
+        acc[2] += (double)tp;
     }
+    acc[0] = acc[1] + acc[2];
     grid_reduce<3, kPlaqThreads>(acc, rb, sc.s);
 }
+
+#ifndef PLAQ_CTAS_PER_SM
+#define PLAQ_CTAS_PER_SM PLAQ_MIN_BLOCKS
+#endif
 
 cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb,
                              cudaStream_t st) {
     int n = subset == 0 ? g.V : g.Vh;
     int items = subset == 0 ? 2 * g.Vhp : g.Vh;
     int grid = (items + kPlaqThreads - 1) / kPlaqThreads;
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (sms <= 0) sms = 148;
+    }
+    if (grid > sms * PLAQ_CTAS_PER_SM) grid = sms * PLAQ_CTAS_PER_SM;
     PlaqScale sc;
     sc.s[0] = 1.0 / (18.0 * (double)n);
     sc.s[1] = sc.s[2] = 1.0 / (9.0 * (double)n);

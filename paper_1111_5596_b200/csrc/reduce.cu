@@ -9,12 +9,18 @@
 
 namespace qdp {
 
-constexpr int kUnroll = 4;
+#ifndef RED_UNROLL
+#define RED_UNROLL 4
+#endif
+#ifndef RED_BLOCKS_PER_SM
+#define RED_BLOCKS_PER_SM 16
+#endif
+constexpr int kUnroll = RED_UNROLL;
 
 static int stream_grid(size_t n) {
     size_t per_block = (size_t)kReduceThreads * kUnroll;
     size_t b = (n + per_block - 1) / per_block;
-    if (b > (size_t)kMaxPartialBlocks) b = kMaxPartialBlocks;
+    if (b > (size_t)148 * RED_BLOCKS_PER_SM) b = (size_t)148 * RED_BLOCKS_PER_SM;
     if (b < 1) b = 1;
     return (int)b;
 }

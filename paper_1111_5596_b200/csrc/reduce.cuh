@@ -60,12 +60,24 @@ __device__ __forceinline__ void grid_reduce(double (&v)[K], const ReduceBuf& rb,
     __syncthreads();
     if (!is_last) return;
     __threadfence();
+    // Thread t sums partials t, t + NT, ... in that order; eight loads are kept in flight
+    // (a fused kernel has one partial per 128 sites, so a thread of the last block walks
+    // ~100 of them and would otherwise pay one L2 round trip per partial).
     double t[K];
 #pragma unroll
     for (int k = 0; k < K; k++) {
-        t[k] = 0.0;
-        for (unsigned int b = threadIdx.x; b < nblk; b += NT)
-            t[k] += __ldcg(&rb.partials[k * nblk + b]);
+        const double* pk = rb.partials + (size_t)k * nblk;
+        double acc = 0.0;
+        unsigned int b = threadIdx.x;
+        for (; b + 7u * NT < nblk; b += 8u * NT) {
+            double v[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = __ldcg(pk + b + j * NT);
+#pragma unroll
+            for (int j = 0; j < 8; j++) acc += v[j];
+        }
+        for (; b < nblk; b += NT) acc += __ldcg(pk + b);
+        t[k] = acc;
     }
     block_tree<K, NT>(t, sm);
     if (threadIdx.x == 0) {
