@@ -42,7 +42,7 @@ __device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
 }
 
 template <class T, bool AXPY, bool NORM>
-__global__ void __launch_bounds__(kHopThreads) hop_kernel(Geom g, typename Vec2<T>::type* __restrict__ chi,
+__global__ void __launch_bounds__(kHopThreads, 3) hop_kernel(Geom g, typename Vec2<T>::type* __restrict__ chi,
                                                          const typename Vec2<T>::type* __restrict__ u,
                                                          const typename Vec2<T>::type* __restrict__ psi,
                                                          int subset, T a, T b, ReduceBuf rb) {
