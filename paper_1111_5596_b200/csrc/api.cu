@@ -145,18 +145,21 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     l->geom = Geom::make(dims);
     ENTER(l);
     l->scratch_from_hook = g_alloc != nullptr;
-    // partials: K <= 4 values per block; the fused kernels launch one block per 64..256
-    // sites, the streaming reductions at most kMaxPartialBlocks, qdp_sum 2*36*64 values
+    // partials: K <= 4 values per block (streaming reductions: at most kMaxPartialBlocks) or per
+    // warp of 32 sites plus per group of kWarpGroup warps (fused kernels, reduce.cuh); qdp_sum
+    // 2*36*64 values.  counters: one per group plus one.
+    const size_t nwarp_max = (size_t)l->geom.V / 32 + 64, ngroup_max = nwarp_max / kWarpGroup + 2;
     size_t npart = (size_t)4 * kMaxPartialBlocks;
-    if (npart < (size_t)4 * ((size_t)l->geom.V / 64 + 1)) npart = (size_t)4 * ((size_t)l->geom.V / 64 + 1);
+    if (npart < 4 * (nwarp_max + ngroup_max)) npart = 4 * (nwarp_max + ngroup_max);
     if (npart < (size_t)2 * 36 * 64) npart = (size_t)2 * 36 * 64;
+    const size_t counter_bytes = (ngroup_max + 1) * sizeof(unsigned int);
     int rc;
     void* p = nullptr;
     if ((rc = dev_alloc(npart * sizeof(double), &p)) != QDP_OK) { delete l; return rc; }
     l->partials = (double*)p;
-    if ((rc = dev_alloc(256, &p)) != QDP_OK) { delete l; return rc; }
+    if ((rc = dev_alloc(counter_bytes, &p)) != QDP_OK) { delete l; return rc; }
     l->counter = (unsigned int*)p;
-    CUDA_TRY(cudaMemset(l->counter, 0, 256));
+    CUDA_TRY(cudaMemset(l->counter, 0, counter_bytes));
     CUDA_TRY(cudaHostAlloc((void**)&l->result_host, 72 * sizeof(double), cudaHostAllocMapped));
     CUDA_TRY(cudaHostGetDevicePointer((void**)&l->result_dev, l->result_host, 0));
     l->stage_bytes = (size_t)kStageSites * 36 * 16;

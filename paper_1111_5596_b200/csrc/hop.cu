@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(kHopThreads, 3) hop_kernel(Geom g, typename Ve
             if (NORM) n2[0] += (double)acc.e[c].re * (double)acc.e[c].re + (double)acc.e[c].im * (double)acc.e[c].im;
         }
     }
-    if (NORM) grid_reduce<1, kHopThreads>(n2, rb, nullptr);
+    if (NORM) warp_grid_reduce<1>(n2, rb, nullptr);
 }
 
 template <class T>

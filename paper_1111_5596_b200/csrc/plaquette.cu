@@ -101,7 +101,7 @@ plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u, int subse
         acc[2] += (double)tp;
     }
     acc[0] = acc[1] + acc[2];
-    grid_reduce<3, kPlaqThreads>(acc, rb, sc.s);
+    warp_grid_reduce<3>(acc, rb, sc.s);
 }
 
 #ifndef PLAQ_CTAS_PER_SM
