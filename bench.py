@@ -38,6 +38,14 @@ METRIC = "site-updates/s"
 UNIT = "site-updates/s"
 OPS_PER_STEP = 7          # shift, plaquette, ape, hop(even+odd), inner, axpy_hop+norm2, norm2
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
+# ape_kernel<double> is bound by the plain fp64 pipe, not by HBM.
+# Peak: 64 fp64 FMA lanes per clock per SM x 148 SMs x 1.965 GHz x 2 flop = 37.2 TFLOP/s (unit counts and
+# clocks of the guides; a DFMA-only microbenchmark measured 17.07 T DFMA/s = 34.1 TFLOP/s on this pool).
+FP64_PEAK_TFLOPS = 64 * 148 * 1.965e9 * 2 / 1e12
+# fp64 flops per site of one spatial APE step as implemented: 24 3x3 complex products, the blend and three
+# SU(3) projections = 3327 DFMA + 498 DMUL + 87 DADD per site (SASS of ape_kernel<double,false>,
+# profiles/r1c_ncu_full.md) = 7239 flop.
+APE_FLOPS_PER_SITE_F64 = 3327 * 2 + 498 + 87
 
 
 def algorithmic_bytes(V: int, eb: int) -> dict:
@@ -76,7 +84,7 @@ def ncu_traffic(kernel: str):
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons during the timed region (pynvml)."""
 
-    def __init__(self, index: int, period: float = 0.02):
+    def __init__(self, index: int, period: float = 0.002):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
@@ -119,14 +127,34 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def rank_env() -> tuple[int, int, int]:
+    """(rank, world_size, local_rank) from the torchrun environment; (0, 1, 0) when run directly."""
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")),
+            int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def max_over_ranks(values, dist, device) -> list[float]:
+    """Element-wise MAX over ranks of a list of per-rank times (the job is as slow as its slowest
+    replica); identity when not distributed.  The only cross-rank operation of the bench: the data
+    path itself has no collective ("replicas only")."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def whole_job_value(units_per_rank: int, world: int, ms: float) -> float:
+    """Whole-job throughput: every rank processed units_per_rank units in (max over ranks) ms."""
+    return units_per_rank * world / (ms * 1e-3)
+
+
 def run_ours(args) -> dict | None:
     import torch
     import synth
     import paper_1111_5596_b200 as q
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local)
@@ -225,10 +253,7 @@ def run_ours(args) -> dict | None:
         e2e_s = time.perf_counter() - t0
         barrier()
 
-    times = torch.tensor([total_ms, e2e_s * 1e3], dtype=torch.float64, device=f"cuda:{local}")
-    if dist is not None:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = float(times[0]), float(times[1])
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_s * 1e3], dist, f"cuda:{local}")
 
     out = None
     if rank == 0:
@@ -243,9 +268,22 @@ def run_ours(args) -> dict | None:
         dom = max(per_op_ms, key=per_op_ms.get)
         dom_kernel = {"ape": "ape_kernel", "plaquette": "plaquette_kernel", "axpy_hop_norm2": "hop_kernel",
                       "hop_even": "hop_kernel", "hop_odd": "hop_kernel"}.get(dom, dom + "_kernel")
-        units = OPS_PER_STEP * V * K * world
+        if dom == "ape" and prec == "f64":
+            tf = APE_FLOPS_PER_SITE_F64 * V / per_op_ms[dom] / 1e9
+            roofline = {"bound": "alu", "kernel": dom_kernel, "op": dom, "achieved": round(tf, 2),
+                        "peak": round(FP64_PEAK_TFLOPS, 2), "unit": "TFLOP/s", "frac": round(tf / FP64_PEAK_TFLOPS, 4),
+                        "peak_source": "derived: 64 fp64 FMA lanes/clk/SM x 148 SMs x 1.965 GHz x 2 (DESIGN.md section 4)",
+                        "flops_per_launch": APE_FLOPS_PER_SITE_F64 * V, "traffic": ncu_traffic(dom_kernel),
+                        "hbm": {"achieved": op_report[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                                "frac": op_report[dom]["frac"], "peak_source": peak_src,
+                                "algorithmic_bytes_per_launch": alg[dom]}}
+        else:
+            roofline = {"bound": "hbm", "kernel": dom_kernel, "op": dom,
+                        "achieved": op_report[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                        "frac": op_report[dom]["frac"], "peak_source": peak_src,
+                        "algorithmic_bytes_per_launch": alg[dom], "traffic": ncu_traffic(dom_kernel)}
         out = {
-            "metric": METRIC, "value": units / (total_ms * 1e-3), "unit": UNIT,
+            "metric": METRIC, "value": whole_job_value(OPS_PER_STEP * V * K, world, total_ms), "unit": UNIT,
             "n_gpus": world, "steps": K, "warmup": args.warmup, "ms_per_step": total_ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": prec, "data": "synthetic",
@@ -256,15 +294,12 @@ def run_ours(args) -> dict | None:
                        "l2": "inputs larger than L2 (gauge 1.2 GB, spinor 0.4 GB vs 126 MB)",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "clocks": clocks,
-            "e2e": ({"value": OPS_PER_STEP * V * ke * world / (e2e_ms * 1e-3), "unit": UNIT,
+            "e2e": ({"value": whole_job_value(OPS_PER_STEP * V * ke, world, e2e_ms), "unit": UNIT,
                      "h2d_bytes_per_step": int(hu.nbytes + hp.nbytes),
                      "d2h_bytes_per_step": int(hu.nbytes + hp.nbytes),
                      "steps": ke, "ms_per_step": e2e_ms / ke} if ke else None),
             "gpu_launches": int(launches),
-            "roofline": {"bound": "hbm", "kernel": dom_kernel, "op": dom,
-                         "achieved": op_report[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                         "frac": op_report[dom]["frac"], "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": alg[dom], "traffic": ncu_traffic(dom_kernel)},
+            "roofline": roofline,
             "ops": op_report,
             "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
         }
