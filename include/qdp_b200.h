@@ -91,6 +91,17 @@ int qdp_lattice_destroy(qdp_lattice* lat);
  * NULL = legacy default stream) for every later call on this lattice. */
 int qdp_lattice_set_stream(qdp_lattice* lat, void* cuda_stream);
 
+/* Sweep order of the neighbour-reading kernels (plaquette, APE step, hop): a tuning knob, results
+ * do not depend on it except for the summation order of the fused reductions.  x2_extent = 0:
+ * linear order (x3 slowest over the whole lattice).  x2_extent = c > 0: slabs of c values of x2
+ * (x0, x1 complete) are swept one after the other, x3 slowest inside a slab, so that the links
+ * of x + 3 are still in L2 when the sweep reaches them as own links.
+ * qdp_lattice_create picks the value from the lattice size (slabs of <= 16 MB per x3-slice when a
+ * whole slice of an fp64 gauge field exceeds 24 MB).  Returns QDP_ERR_ARG unless c divides L2
+ * and L0/2 * L1 is a multiple of 32.  The reading of subsets, sites and values is unchanged
+ * (SURVEY.md 8(a) rows a1, a10). */
+int qdp_lattice_set_sweep_slab(qdp_lattice* lat, int x2_extent);
+
 /* Replace the device allocator used by qdp_field_alloc and the library's scratch
  * buffers (default cudaMalloc/cudaFree).  alloc(bytes, ctx) returns a device
  * pointer aligned to >= 256 bytes or NULL; free_(ptr, ctx) releases it.  Lets

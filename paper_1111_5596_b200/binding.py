@@ -14,7 +14,7 @@ __all__ = [
     "QdpError", "Lattice", "Field", "LIB_PATH", "DECLARED_SYMBOLS",
     "QDP_ALL", "QDP_EVEN", "QDP_ODD", "QDP_F32", "QDP_F64",
     "QDP_COLOR_MATRIX", "QDP_GAUGE", "QDP_FERMION",
-    "qdp_lattice_create", "qdp_lattice_destroy", "qdp_lattice_set_stream", "qdp_lattice_volume",
+    "qdp_lattice_create", "qdp_lattice_destroy", "qdp_lattice_set_stream", "qdp_lattice_set_sweep_slab", "qdp_lattice_volume",
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
@@ -47,6 +47,7 @@ DECLARED_SYMBOLS = {
     "qdp_lattice_create": ([_P, _I, _PP], _I),
     "qdp_lattice_destroy": ([_P], _I),
     "qdp_lattice_set_stream": ([_P, _P], _I),
+    "qdp_lattice_set_sweep_slab": ([_P, _I], _I),
     "qdp_set_allocator": ([_P, _P, _P], _I),
     "qdp_lattice_neighbor_table": ([_P, _I, _I, _P], _I),
     "qdp_lattice_parity_mask": ([_P, _P], _I),
@@ -138,6 +139,10 @@ def qdp_lattice_destroy(lat: Lattice) -> None:
 
 def qdp_lattice_set_stream(lat: Lattice, cuda_stream: int | None) -> None:
     _check(_lib.qdp_lattice_set_stream(lat.handle, cuda_stream))
+
+
+def qdp_lattice_set_sweep_slab(lat: Lattice, x2_extent: int) -> None:
+    _check(_lib.qdp_lattice_set_sweep_slab(lat.handle, int(x2_extent)))
 
 
 def qdp_lattice_sync(lat: Lattice) -> None:

@@ -199,6 +199,17 @@ extern "C" int qdp_lattice_set_stream(qdp_lattice* l, void* cuda_stream) {
     return QDP_OK;
 }
 
+extern "C" int qdp_lattice_set_sweep_slab(qdp_lattice* l, int c2) {
+    if (!ok_lat(l)) return fail(QDP_ERR_ARG, "qdp_lattice_set_sweep_slab: not a lattice");
+    Geom& g = l->geom;
+    if (c2 == 0) { g.slab_c2 = 0; g.slab_ipr = 0; return QDP_OK; }
+    if (c2 < 0 || g.L2 % c2 != 0 || (g.s2 & 31) != 0)
+        return fail(QDP_ERR_ARG, "qdp_lattice_set_sweep_slab: extent %d must divide L2 = %d and L0/2*L1 = %d be a multiple of 32",
+                    c2, g.L2, g.s2);
+    g.slab_c2 = c2; g.slab_ipr = g.s2 >> 5;
+    return QDP_OK;
+}
+
 extern "C" int qdp_set_allocator(void* (*alloc)(size_t, void*), void (*free_)(void*, void*), void* ctx) {
     if ((alloc == nullptr) != (free_ == nullptr)) return fail(QDP_ERR_ARG, "qdp_set_allocator: need both alloc and free");
     g_alloc = alloc; g_free = free_; g_alloc_ctx = ctx;

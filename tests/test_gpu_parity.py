@@ -296,3 +296,45 @@ def test_error_codes(qdp, lat_cache):
         assert len(held) == 0
     finally:
         qdp.qdp_set_allocator(None, None)
+
+
+@pytest.mark.parametrize("dims,c2", [((16, 4, 8, 4), 2), ((16, 4, 8, 4), 4), ((8, 8, 6, 4), 3), ((32, 2, 4, 2), 1)])
+def test_sweep_slab_order_gives_the_same_fields(qdp, dims, c2):
+    """qdp_lattice_set_sweep_slab (the L2-aware sweep that qdp_lattice_create switches on for
+    lattices as large as C5) only permutes the order in which sites are visited: fields must come
+    out bit-identical to the linear sweep, sums within the 1e-10 bar, everything within the
+    oracle bars -- here on lattices small enough to compare element by element."""
+    lat, lin = qdp.qdp_lattice_create(dims), qdp.qdp_lattice_create(dims)
+    qdp.qdp_lattice_set_sweep_slab(lat, c2)
+    qdp.qdp_lattice_set_sweep_slab(lin, 0)
+    hu, hp = synth.gauge_hot(dims, _seed(dims) + 21), synth.spinor(dims, _seed(dims) + 22)
+    outs = []
+    for L in (lat, lin):
+        u, psi = qdp.field_from_host(L, 1, hu), qdp.field_from_host(L, 2, hp)
+        u2, chi = qdp.qdp_field_alloc(L, 1, 1), qdp.qdp_field_alloc(L, 2, 1)
+        res = {"plaq": [qdp.qdp_plaquette(u, s) for s in SUBSETS]}
+        for t_dir in (3, -1):
+            qdp.qdp_ape_smear_step(u2, u, 0.5, t_dir)
+            res[f"ape{t_dir}"] = qdp.field_to_host(u2)
+        for s in SUBSETS:
+            chi = qdp.field_from_host(L, 2, hp)
+            res[f"n2_{s}"] = qdp.qdp_axpy_hop(chi, 0.3, -0.7, u, psi, s, want_norm2=True)
+            res[f"hop{s}"] = qdp.field_to_host(chi)
+        outs.append(res)
+    slab, lin_ = outs
+    for k in slab:
+        if k.startswith(("ape", "hop")):
+            assert np.array_equal(slab[k], lin_[k]), k
+    for s in SUBSETS:
+        assert np.abs(slab["plaq"][s] - oracle.plaquette(dims, hu, s)).max() <= 1e-10
+        assert np.abs(slab["plaq"][s] - lin_["plaq"][s]).max() <= 1e-12
+        want = oracle.axpy_hop(dims, 0.3, -0.7, hu, hp, s, chi=hp.copy())
+        assert site_rel_err(slab[f"hop{s}"], want).max() <= TOL_SITE["f64"]
+        assert abs(slab[f"n2_{s}"] - oracle.norm2(dims, want, s)) <= 1e-10 * slab[f"n2_{s}"]
+    assert site_rel_err(links(slab["ape3"]), links(oracle.ape_smear_step(dims, hu, 0.5, 3))).max() <= TOL_SITE["f64"]
+    assert site_rel_err(links(slab["ape-1"]), links(oracle.ape_smear_step(dims, hu, 0.5, -1))).max() <= TOL_SITE["f64"]
+    # argument validation
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_lattice_set_sweep_slab(lat, 5)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_lattice_set_sweep_slab(qdp.qdp_lattice_create((4, 4, 4, 4)), 2)   # L0/2*L1 = 8
