@@ -28,9 +28,12 @@ namespace qdp {
 #define APE_THREADS 128
 #endif
 constexpr int kApeThreads = APE_THREADS;
+#ifndef APE_MIN_BLOCKS_F32
+#define APE_MIN_BLOCKS_F32 3
+#endif
 // fp64: 2 blocks of 128 threads per SM (255 registers, the software pipeline needs them);
-// fp32: 3 blocks (168 registers; the projection runs in fp64 for both)
-template <class T> struct ApeCfg { static constexpr int kMinBlocks = sizeof(T) == 8 ? 2 : 3; };
+// fp32: 3 blocks (168 registers; the projection runs in fp64 for both precisions)
+template <class T> struct ApeCfg { static constexpr int kMinBlocks = sizeof(T) == 8 ? 2 : APE_MIN_BLOCKS_F32; };
 
 __device__ __forceinline__ int sel4(const int (&a)[4], int i) {
     return i == 0 ? a[0] : (i == 1 ? a[1] : (i == 2 ? a[2] : a[3]));

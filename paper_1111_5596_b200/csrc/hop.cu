@@ -12,6 +12,10 @@
 namespace qdp {
 
 constexpr int kHopThreads = 128;
+#ifndef HOP_MIN_BLOCKS_F32
+#define HOP_MIN_BLOCKS_F32 6
+#endif
+template <class T> struct HopCfg { static constexpr int kBlocks = sizeof(T) == 8 ? 3 : HOP_MIN_BLOCKS_F32; };
 
 template <class T, int MU>
 __device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
@@ -42,7 +46,7 @@ __device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
 }
 
 template <class T, bool AXPY, bool NORM>
-__global__ void __launch_bounds__(kHopThreads, 3) hop_kernel(Geom g, typename Vec2<T>::type* __restrict__ chi,
+__global__ void __launch_bounds__(kHopThreads, HopCfg<T>::kBlocks) hop_kernel(Geom g, typename Vec2<T>::type* __restrict__ chi,
                                                          const typename Vec2<T>::type* __restrict__ u,
                                                          const typename Vec2<T>::type* __restrict__ psi,
                                                          int subset, T a, T b, ReduceBuf rb) {

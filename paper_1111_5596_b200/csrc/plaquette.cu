@@ -23,6 +23,11 @@ namespace qdp {
 #ifndef PLAQ_MIN_BLOCKS
 #define PLAQ_MIN_BLOCKS 2
 #endif
+#ifndef PLAQ_MIN_BLOCKS_F32
+#define PLAQ_MIN_BLOCKS_F32 4
+#endif
+// resident blocks per SM = persistent blocks per SM: fp64 2 x 128 threads at 254 registers, fp32 half the registers
+template <class T> struct PlaqCfg { static constexpr int kBlocks = sizeof(T) == 8 ? PLAQ_MIN_BLOCKS : PLAQ_MIN_BLOCKS_F32; };
 constexpr int kPlaqThreads = PLAQ_THREADS;
 #ifndef PLAQ_UNROLL
 #define PLAQ_UNROLL 6
@@ -52,7 +57,7 @@ __device__ __forceinline__ T re_tr_p_adj_ab(const Mat3<T>& P, const Mat3<T>& a, 
 }
 
 template <class T>
-__global__ void __launch_bounds__(kPlaqThreads, PLAQ_MIN_BLOCKS)
+__global__ void __launch_bounds__(kPlaqThreads, PlaqCfg<T>::kBlocks)
 plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u, int subset, ReduceBuf rb, PlaqScale sc) {
     using T2 = typename Vec2<T>::type;
     // Persistent warps: warp w of the grid takes the 32-site work items w, w + W, w + 2W, ...
@@ -104,9 +109,6 @@ plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u, int subse
     warp_grid_reduce<3>(acc, rb, sc.s);
 }
 
-#ifndef PLAQ_CTAS_PER_SM
-#define PLAQ_CTAS_PER_SM PLAQ_MIN_BLOCKS
-#endif
 
 cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb,
                              cudaStream_t st) {
@@ -120,7 +122,8 @@ cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset,
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (sms <= 0) sms = 148;
     }
-    if (grid > sms * PLAQ_CTAS_PER_SM) grid = sms * PLAQ_CTAS_PER_SM;
+    const int per_sm = prec ? PlaqCfg<double>::kBlocks : PlaqCfg<float>::kBlocks;
+    if (grid > sms * per_sm) grid = sms * per_sm;
     PlaqScale sc;
     sc.s[0] = 1.0 / (18.0 * (double)n);
     sc.s[1] = sc.s[2] = 1.0 / (9.0 * (double)n);

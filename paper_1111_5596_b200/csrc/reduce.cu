@@ -93,6 +93,54 @@ __global__ void __launch_bounds__(kReduceThreads) inner_kernel(Geom g, const T2*
     grid_reduce<2>(acc, rb, nullptr);
 }
 
+// fp32 fields without padding lanes: two complex numbers per 128-bit load (a float2 stream would
+// issue twice the load instructions for the same bytes: measured 0.056 ms vs the 0.031 ms floor
+// for norm2 of a C4 spinor).
+__global__ void __launch_bounds__(kReduceThreads) norm2_f32x2_kernel(const float4* __restrict__ p, unsigned n,
+                                                                    ReduceBuf rb) {
+    const unsigned stride = gridDim.x * kReduceThreads;
+    double acc[1] = {0.0};
+    unsigned e = blockIdx.x * kReduceThreads + threadIdx.x;
+    for (; e + (kUnroll - 1) * stride < n; e += kUnroll * stride) {
+        float4 v[kUnroll];
+#pragma unroll
+        for (int k = 0; k < kUnroll; k++) v[k] = __ldg(p + e + k * stride);
+#pragma unroll
+        for (int k = 0; k < kUnroll; k++)
+            acc[0] += ((double)v[k].x * (double)v[k].x + (double)v[k].y * (double)v[k].y) +
+                      ((double)v[k].z * (double)v[k].z + (double)v[k].w * (double)v[k].w);
+    }
+    for (; e < n; e += stride) {
+        float4 v = __ldg(p + e);
+        acc[0] += ((double)v.x * (double)v.x + (double)v.y * (double)v.y) +
+                  ((double)v.z * (double)v.z + (double)v.w * (double)v.w);
+    }
+    grid_reduce<1>(acc, rb, nullptr);
+}
+__global__ void __launch_bounds__(kReduceThreads) inner_f32x2_kernel(const float4* __restrict__ pa,
+                                                                    const float4* __restrict__ pb, unsigned n,
+                                                                    ReduceBuf rb) {
+    const unsigned stride = gridDim.x * kReduceThreads;
+    double acc[2] = {0.0, 0.0};
+    unsigned e = blockIdx.x * kReduceThreads + threadIdx.x;
+    auto add = [&](const float4& a, const float4& b) {   // conj(a) * b for both complex numbers
+        acc[0] += ((double)a.x * (double)b.x + (double)a.y * (double)b.y) + ((double)a.z * (double)b.z + (double)a.w * (double)b.w);
+        acc[1] += ((double)a.x * (double)b.y - (double)a.y * (double)b.x) + ((double)a.z * (double)b.w - (double)a.w * (double)b.z);
+    };
+    for (; e + (kUnroll - 1) * stride < n; e += kUnroll * stride) {
+        float4 va[kUnroll], vb[kUnroll];
+#pragma unroll
+        for (int k = 0; k < kUnroll; k++) {
+            va[k] = __ldg(pa + e + k * stride);
+            vb[k] = __ldg(pb + e + k * stride);
+        }
+#pragma unroll
+        for (int k = 0; k < kUnroll; k++) add(va[k], vb[k]);
+    }
+    for (; e < n; e += stride) add(__ldg(pa + e), __ldg(pb + e));
+    grid_reduce<2>(acc, rb, nullptr);
+}
+
 // sum: blockIdx.y = component; two kernels (partials, then a fixed-order finish)
 constexpr int kSumBlocks = 64;
 template <class T2>
@@ -123,6 +171,11 @@ template <class T2, int NCOMP>
 static void norm2_dispatch(const Geom& g, const void* f, int subset, const ReduceBuf& rb, cudaStream_t st) {
     size_t n = (size_t)g.Vhp * NCOMP * (subset == 0 ? 2 : 1);
     int grid = stream_grid(n);
+    if (sizeof(T2) == 8 && g.Vh == g.Vhp) {
+        const float4* p = (const float4*)((const float2*)f + (subset == 2 ? (size_t)g.Vhp * NCOMP : 0));
+        norm2_f32x2_kernel<<<stream_grid(n / 2), kReduceThreads, 0, st>>>(p, (unsigned)(n / 2), rb);
+        return;
+    }
     if (g.Vh == g.Vhp) norm2_kernel<T2, NCOMP, false><<<grid, kReduceThreads, 0, st>>>(g, (const T2*)f, subset, rb);
     else               norm2_kernel<T2, NCOMP, true><<<grid, kReduceThreads, 0, st>>>(g, (const T2*)f, subset, rb);
 }
@@ -131,6 +184,12 @@ static void inner_dispatch(const Geom& g, const void* a, const void* b, int subs
                            cudaStream_t st) {
     size_t n = (size_t)g.Vhp * NCOMP * (subset == 0 ? 2 : 1);
     int grid = stream_grid(n);
+    if (sizeof(T2) == 8 && g.Vh == g.Vhp) {
+        const size_t off = subset == 2 ? (size_t)g.Vhp * NCOMP : 0;
+        inner_f32x2_kernel<<<stream_grid(n / 2), kReduceThreads, 0, st>>>(
+            (const float4*)((const float2*)a + off), (const float4*)((const float2*)b + off), (unsigned)(n / 2), rb);
+        return;
+    }
     if (g.Vh == g.Vhp)
         inner_kernel<T2, NCOMP, false><<<grid, kReduceThreads, 0, st>>>(g, (const T2*)a, (const T2*)b, subset, rb);
     else
