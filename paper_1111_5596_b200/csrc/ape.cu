@@ -28,6 +28,10 @@ namespace qdp {
 #define APE_THREADS 128
 #endif
 constexpr int kApeThreads = APE_THREADS;
+// A never-taken branch ptxas cannot predicate away: it ends the basic block.  The unrolled
+// directions would otherwise merge into one block of ~5000 instructions in which ptxas hoists
+// the loads of all directions to the top and spills 2-4 KB per thread (measured: 1.96 ms).
+#define BLOCK_BOUNDARY(g) do { if ((g).V < 0) __trap(); } while (0)
 #ifndef APE_MIN_BLOCKS_F32
 #define APE_MIN_BLOCKS_F32 3
 #endif
@@ -116,7 +120,10 @@ ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out, const typename Vec2
             T im = w_link * U.e[c].im + w_staple * S.e[c].im;
             Vd.e[c] = cx<double>((double)re, (double)im);
         }
-        Mat3<double> Pd = proj_su3(Vd);
+        ProjScalars ps[1];
+        proj_stage_a(Vd, ps[0]);
+        proj_stage_b<1>(ps);
+        Mat3<double> Pd = proj_stage_c(Vd, ps[0]);
         T2* o = site_ptr(out, 36, mu * 9, sb);
 #pragma unroll
         for (int c = 0; c < 9; c++) {
@@ -124,6 +131,7 @@ ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out, const typename Vec2
             v.x = (T)Pd.e[c].re; v.y = (T)Pd.e[c].im;
             o[c * kLane] = v;
         }
+        BLOCK_BOUNDARY(g);
     }
 }
 

@@ -96,6 +96,20 @@ __device__ __forceinline__ Spinor<T> ld_spinor(const typename Vec2<T>::type* __r
     return r;
 }
 
+// Read back what this thread stored earlier in the kernel.  An ordinary load would let the
+// compiler forward the stored registers to the use and keep them live in between, which is
+// exactly what parking a value in memory is meant to avoid.
+__device__ __forceinline__ double2 ld_parked(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float2 ld_parked(const float2* p) {
+    float2 v;
+    asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+
 // ---- matrix algebra --------------------------------------------------------
 template <class T> __device__ __forceinline__ Mat3<T> mat_zero() {
     Mat3<T> r;
@@ -179,9 +193,48 @@ template <class T> __device__ __forceinline__ Cx<T> det(const Mat3<T>& a) {
 //   SFU pipes) and polished by three Newton steps in fp64 (quadratic: 3e-4 -> 1e-7 ->
 //   1e-14 -> rounding); the reciprocal of uv - w is carried along by its own Newton step.
 //   The determinant phase exp(-i theta/3) is the principal cube root of conj(d)/|d|:
-//   fp32 seed from atan2f/sincosf, two Newton steps z <- z - (z^3 - c) conj(z^2)/3.
-__device__ __forceinline__ Mat3<double> proj_su3(const Mat3<double>& V) {
-    // H = V^dag V: diagonal real, upper triangle complex
+//   fp32 seed from a polynomial atan2 and __sincosf, two Newton steps z <- z - (z^3 - c) conj(z^2)/3.
+// The projection in three stages: (a) invariants of V and fp32 seeds, (b) the scalar Newton
+// chains, written for N links side by side (iteration loop outside, link loop inside),
+// (c) W = V (f0 + f1 H + f2 H^2) z.  ncu attributes 40 % of the APE kernel's warp time to the
+// projection (31 % of its fp64 instructions) with "wait" (fixed-latency dependency) as the main
+// stall, a third of it in the fp32 seed code; the seeds therefore use branch-free polynomial
+// acos / atan2 and the approximate division and sincos intrinsics.  The IEEE square roots
+// stay: their slow-path branches split the seed code into basic blocks, and every variant
+// without them measured slower (ape.cu: BLOCK_BOUNDARY).
+// Branch-free fp32 approximations for the seeds (absolute error ~1e-4 rad; the fp64 Newton steps
+// that follow converge quadratically from there).  acos: Abramowitz & Stegun 4.4.45 on |x|,
+// reflected for x < 0; atan2: A&S 4.4.49-style odd polynomial on [0, 1] with octant reduction.
+__device__ __forceinline__ float acos_seed(float x) {
+    const float a = fabsf(x);
+    const float p = fmaf(fmaf(fmaf(-0.0187293f, a, 0.0742610f), a, -0.2121144f), a, 1.5707288f);
+    const float r = p * __fsqrt_rn(fmaxf(1.0f - a, 0.0f));
+    return x < 0.0f ? 3.14159265f - r : r;
+}
+__device__ __forceinline__ float atan2_seed(float y, float x) {
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+    const float t = __fdividef(mn, fmaxf(mx, 1e-37f));
+    const float t2 = t * t;
+    // atan(t), t in [0, 1]: max error ~1e-5
+    float r = fmaf(fmaf(fmaf(fmaf(0.0208351f, t2, -0.0851330f), t2, 0.1801410f), t2, -0.3302995f), t2, 0.9998660f) * t;
+    r = ay > ax ? 1.57079633f - r : r;
+    r = x < 0.0f ? 3.14159265f - r : r;
+    return y < 0.0f ? -r : r;
+}
+
+struct ProjScalars {
+    double h00, h11, h22, n01, n02, n12;   // H = V^dag V: diagonal, |off-diagonal|^2
+    Cx<double> h01, h02, h12;
+    double c1, c2, w, rw;                  // invariants, |det V| and its reciprocal
+    Cx<double> cc;                         // conj(det V)/|det V|
+    double u, v, q;                        // Newton state
+    Cx<double> z;                          // cube root state
+    double f0, f1, f2;
+};
+
+// stage A: invariants of V and the fp32 seeds
+__device__ __forceinline__ void proj_stage_a(const Mat3<double>& V, ProjScalars& s) {
     double h00 = 0, h11 = 0, h22 = 0;
     Cx<double> h01 = cx<double>(0, 0), h02 = cx<double>(0, 0), h12 = cx<double>(0, 0);
 #pragma unroll
@@ -194,92 +247,115 @@ __device__ __forceinline__ Mat3<double> proj_su3(const Mat3<double>& V) {
         cmad_conj_a(h02, a, c);
         cmad_conj_a(h12, b, c);
     }
-    const double n01 = h01.re * h01.re + h01.im * h01.im;
-    const double n02 = h02.re * h02.re + h02.im * h02.im;
-    const double n12 = h12.re * h12.re + h12.im * h12.im;
-    const double c2 = h00 + h11 + h22;
-    const double c1 = h00 * h11 + h00 * h22 + h11 * h22 - n01 - n02 - n12;
+    s.h00 = h00; s.h11 = h11; s.h22 = h22; s.h01 = h01; s.h02 = h02; s.h12 = h12;
+    s.n01 = h01.re * h01.re + h01.im * h01.im;
+    s.n02 = h02.re * h02.re + h02.im * h02.im;
+    s.n12 = h12.re * h12.re + h12.im * h12.im;
+    s.c2 = h00 + h11 + h22;
+    s.c1 = h00 * h11 + h00 * h22 + h11 * h22 - s.n01 - s.n02 - s.n12;
     const Cx<double> d = det(V);
     const double w2 = d.re * d.re + d.im * d.im;   // det H
-    const double rw = rsqrt(w2), w = w2 * rw;      // 1/|det V|, |det V|
-    // ---- fp32 seeds ----
-    double u, v, q;
+    // 1/|det V|: fp32 seed, two Newton steps y <- y (1.5 - 0.5 w2 y^2)  (1e-7 -> 1e-14 -> rounding)
+    double y = (double)rsqrtf((float)w2);
+    const double hw2 = 0.5 * w2;
+    y = y * fma(-hw2 * y, y, 1.5);
+    y = y * fma(-hw2 * y, y, 1.5);
+    s.rw = y; s.w = w2 * y;
+    s.cc = cx<double>(d.re * y, -d.im * y);
+    // seeds of (u, v): trigonometric roots of the characteristic cubic, in fp32
     {
-        const float m = (float)c2 * (1.0f / 3.0f), fc1 = (float)c1, fc0 = (float)w2;
+        const float m = (float)s.c2 * (1.0f / 3.0f), fc1 = (float)s.c1, fc0 = (float)w2;
         const float r2 = fmaxf(m * m - fc1 * (1.0f / 3.0f), 0.0f);
-        const float r = sqrtf(r2);
+        const float r = __fsqrt_rn(r2);
         const float qh = m * m * m - 0.5f * m * fc1 + 0.5f * fc0;
-        float c3 = qh / fmaxf(r * r2, 1e-37f);
+        float c3 = __fdividef(qh, fmaxf(r * r2, 1e-37f));
         c3 = fminf(1.0f, fmaxf(-1.0f, c3));
-        const float th = acosf(c3) * (1.0f / 3.0f);
-        float s, c;
-        __sincosf(th, &s, &c);
+        const float th = acos_seed(c3) * (1.0f / 3.0f);
+        float sn, cs;
+        __sincosf(th, &sn, &cs);
         const float rt3 = 1.7320508f;
-        const float g0 = sqrtf(fmaxf(m + 2.0f * r * c, 0.0f));
-        const float g1 = sqrtf(fmaxf(m - r * c - rt3 * r * s, 0.0f));
-        const float g2 = sqrtf(fmaxf(m - r * c + rt3 * r * s, 0.0f));
+        const float g0 = __fsqrt_rn(fmaxf(m + 2.0f * r * cs, 0.0f));
+        const float g1 = __fsqrt_rn(fmaxf(m - r * cs - rt3 * r * sn, 0.0f));
+        const float g2 = __fsqrt_rn(fmaxf(m - r * cs + rt3 * r * sn, 0.0f));
         const float fu = g0 + g1 + g2, fv = g0 * g1 + g0 * g2 + g1 * g2;
-        u = (double)fu;
-        v = (double)fv;
-        q = (double)(1.0f / (fu * fv - (float)w));
+        s.u = (double)fu;
+        s.v = (double)fv;
+        s.q = (double)__fdividef(1.0f, fu * fv - (float)s.w);
     }
-    // ---- Newton on (u, v), q -> 1/(uv - w) ----
+    // seed of the cube root of conj(d)/|d|: principal branch, theta in (-pi, pi]
+    {
+        const float th0 = atan2_seed((float)d.im, (float)d.re) * (1.0f / 3.0f);
+        float sn, cs;
+        __sincosf(th0, &sn, &cs);
+        s.z = cx<double>((double)cs, -(double)sn);
+    }
+}
+
+// stage B: the scalar chains of N links, interleaved
+template <int N>
+__device__ __forceinline__ void proj_stage_b(ProjScalars (&s)[N]) {
 #pragma unroll
     for (int it = 0; it < 3; it++) {
-        const double F1 = fma(u, u, -2.0 * v) - c2;
-        const double F2 = fma(v, v, -2.0 * w * u) - c1;
-        const double hq = 0.5 * q;
-        const double du = fma(v, F1, F2) * hq;
-        const double dv = fma(w, F1, u * F2) * hq;
-        u -= du;
-        v -= dv;
-        const double x = fma(u, v, -w);
-        q = q * fma(-x, q, 2.0);
+#pragma unroll
+        for (int n = 0; n < N; n++) {
+            const double u = s[n].u, v = s[n].v, w = s[n].w, q = s[n].q;
+            const double F1 = fma(u, u, -2.0 * v) - s[n].c2;
+            const double F2 = fma(v, v, -2.0 * w * u) - s[n].c1;
+            const double hq = 0.5 * q;
+            const double un = u - fma(v, F1, F2) * hq;
+            const double vn = v - fma(w, F1, u * F2) * hq;
+            const double x = fma(un, vn, -w);
+            s[n].u = un; s[n].v = vn;
+            s[n].q = q * fma(-x, q, 2.0);
+        }
     }
-    const double den = q * rw;
-    const double f0 = (u * v * v - w * (u * u + v)) * den;
-    const double f1 = (2 * u * v - w - u * u * u) * den;
-    const double f2 = u * den;
-    // H^2 (Hermitian): diagonal and upper triangle
-    const double q00 = h00 * h00 + n01 + n02;
-    const double q11 = h11 * h11 + n01 + n12;
-    const double q22 = h22 * h22 + n02 + n12;
+#pragma unroll
+    for (int it = 0; it < 2; it++) {
+#pragma unroll
+        for (int n = 0; n < N; n++) {
+            const Cx<double> z = s[n].z, z2 = z * z;
+            const Cx<double> e = z2 * z - s[n].cc;
+            const Cx<double> t = e * conj(z2);
+            s[n].z = cx<double>(fma(t.re, -1.0 / 3.0, z.re), fma(t.im, -1.0 / 3.0, z.im));
+        }
+    }
+#pragma unroll
+    for (int n = 0; n < N; n++) {
+        const double u = s[n].u, v = s[n].v, w = s[n].w;
+        const double den = s[n].q * s[n].rw;
+        s[n].f0 = (u * v * v - w * (u * u + v)) * den;
+        s[n].f1 = (2 * u * v - w - u * u * u) * den;
+        s[n].f2 = u * den;
+    }
+}
+
+// stage C: W = V (f0 + f1 H + f2 H^2) z
+__device__ __forceinline__ Mat3<double> proj_stage_c(const Mat3<double>& V, const ProjScalars& s) {
+    const double h00 = s.h00, h11 = s.h11, h22 = s.h22, f0 = s.f0, f1 = s.f1, f2 = s.f2;
+    const Cx<double> h01 = s.h01, h02 = s.h02, h12 = s.h12;
+    const double q00 = h00 * h00 + s.n01 + s.n02;
+    const double q11 = h11 * h11 + s.n01 + s.n12;
+    const double q22 = h22 * h22 + s.n02 + s.n12;
     Cx<double> q01 = cx<double>((h00 + h11) * h01.re, (h00 + h11) * h01.im);
     cmad_conj_b(q01, h02, h12);          // + h02 conj(h12)
     Cx<double> q02 = cx<double>((h00 + h22) * h02.re, (h00 + h22) * h02.im);
     cmad(q02, h01, h12);                 // + h01 h12
     Cx<double> q12 = cx<double>((h11 + h22) * h12.re, (h11 + h22) * h12.im);
     cmad_conj_a(q12, h01, h02);          // + conj(h01) h02
-    // R = f0 + f1 H + f2 H^2 (Hermitian)
+    // R z with R = f0 + f1 H + f2 H^2 Hermitian: fold the phase into R (nine complex entries)
+    const Cx<double> z = s.z;
+    const double r00 = f0 + f1 * h00 + f2 * q00, r11 = f0 + f1 * h11 + f2 * q11, r22 = f0 + f1 * h22 + f2 * q22;
+    const Cx<double> r01 = cx<double>(f1 * h01.re + f2 * q01.re, f1 * h01.im + f2 * q01.im);
+    const Cx<double> r02 = cx<double>(f1 * h02.re + f2 * q02.re, f1 * h02.im + f2 * q02.im);
+    const Cx<double> r12 = cx<double>(f1 * h12.re + f2 * q12.re, f1 * h12.im + f2 * q12.im);
     Mat3<double> R;
-    R.e[0] = cx<double>(f0 + f1 * h00 + f2 * q00, 0);
-    R.e[4] = cx<double>(f0 + f1 * h11 + f2 * q11, 0);
-    R.e[8] = cx<double>(f0 + f1 * h22 + f2 * q22, 0);
-    R.e[1] = cx<double>(f1 * h01.re + f2 * q01.re, f1 * h01.im + f2 * q01.im);
-    R.e[2] = cx<double>(f1 * h02.re + f2 * q02.re, f1 * h02.im + f2 * q02.im);
-    R.e[5] = cx<double>(f1 * h12.re + f2 * q12.re, f1 * h12.im + f2 * q12.im);
-    R.e[3] = conj(R.e[1]); R.e[6] = conj(R.e[2]); R.e[7] = conj(R.e[5]);
-    Mat3<double> W = mul(V, R);
-    // ---- determinant phase: z = principal cube root of conj(d)/|d| (arg det W = arg det V since R > 0) ----
-    Cx<double> z;
-    {
-        const float th0 = atan2f((float)d.im, (float)d.re) * (1.0f / 3.0f);
-        float s, c;
-        sincosf(th0, &s, &c);
-        z = cx<double>((double)c, -(double)s);
-    }
-    const Cx<double> cc = cx<double>(d.re * rw, -d.im * rw);
-#pragma unroll
-    for (int it = 0; it < 2; it++) {
-        const Cx<double> z2 = z * z;
-        const Cx<double> e = z2 * z - cc;
-        const Cx<double> t = e * conj(z2);
-        z.re = fma(t.re, -1.0 / 3.0, z.re);
-        z.im = fma(t.im, -1.0 / 3.0, z.im);
-    }
-#pragma unroll
-    for (int i = 0; i < 9; i++) W.e[i] = W.e[i] * z;
-    return W;
+    R.e[0] = cx<double>(r00 * z.re, r00 * z.im);
+    R.e[4] = cx<double>(r11 * z.re, r11 * z.im);
+    R.e[8] = cx<double>(r22 * z.re, r22 * z.im);
+    R.e[1] = r01 * z; R.e[3] = conj(r01) * z;
+    R.e[2] = r02 * z; R.e[6] = conj(r02) * z;
+    R.e[5] = r12 * z; R.e[7] = conj(r12) * z;
+    return mul(V, R);
 }
 
 }  // namespace qdp
