@@ -43,9 +43,9 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
 # clocks of the guides; a DFMA-only microbenchmark measured 17.07 T DFMA/s = 34.1 TFLOP/s on this pool).
 FP64_PEAK_TFLOPS = 64 * 148 * 1.965e9 * 2 / 1e12
 # fp64 flops per site of one spatial APE step as implemented: 24 3x3 complex products, the blend and three
-# SU(3) projections = 3327 DFMA + 498 DMUL + 87 DADD per site (SASS of ape_kernel<double,false>,
-# profiles/r1c_ncu_full.md) = 7239 flop.
-APE_FLOPS_PER_SITE_F64 = 3327 * 2 + 498 + 87
+# SU(3) projections = 3300 DFMA + 491 DMUL + 92 DADD per site (SASS of ape_kernel<double,false>: straight-line
+# code, every instruction executes once per site; profiles/r1d_ncu_full.md) = 7183 flop.
+APE_FLOPS_PER_SITE_F64 = 3300 * 2 + 491 + 92
 
 
 def algorithmic_bytes(V: int, eb: int) -> dict:

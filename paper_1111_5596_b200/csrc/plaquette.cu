@@ -101,6 +101,10 @@ plaquette_kernel(Geom g, const typename Vec2<T>::type* __restrict__ u, int subse
             }
             const T v = re_tr_p_adj_ab(P, A2, B2);
             if (pl < 3) sp += v; else tp += v;
+            // A never-taken branch ptxas cannot predicate away ends the basic block between the
+            // spatial and the temporal planes: measured 0.347 -> 0.332 ms (one block of 1900
+            // instructions schedules worse than two; boundaries elsewhere gain nothing).
+            if (pl == 2 && g.V < 0) __trap();
         }
         acc[1] += (double)sp;
         acc[2] += (double)tp;
