@@ -57,6 +57,8 @@ def _get():
             "orc_hop_site": ([P, P, P, Z, P], None),
             "orc_hop": ([P, P, P, P, I], None),
             "orc_axpy_hop": ([P, D, D, P, P, P, I], None),
+            "orc_hop_site_dirs": ([P, P, P, Z, I, P], None),
+            "orc_smear_hop": ([P, D, D, P, P, P, I, I], None),
             "orc_norm2": ([P, I, P, I], D),
             "orc_inner": ([P, I, P, P, I, P], None),
             "orc_sum": ([P, I, P, I, P], None),
@@ -190,6 +192,21 @@ def axpy_hop(dims, a, b, u, psi, subset=ALL, chi=None):
     u, psi = _c128(u), _c128(psi)
     out = np.zeros_like(psi) if chi is None else _c128(chi).copy()
     _get().orc_axpy_hop(_dims(dims), a, b, u.ctypes.data, psi.ctypes.data, out.ctypes.data, subset)
+    return out
+
+
+def smear_hop(dims, a, b, u, psi, t_dir=3, subset=ALL, chi=None):
+    """chi = a psi + b sum_{mu != t_dir} [U_mu(x) psi(x+mu) + U_mu(x-mu)^dag psi(x-mu)] (row f2)."""
+    u, psi = _c128(u), _c128(psi)
+    out = np.zeros_like(psi) if chi is None else _c128(chi).copy()
+    _get().orc_smear_hop(_dims(dims), a, b, u.ctypes.data, psi.ctypes.data, out.ctypes.data, t_dir, subset)
+    return out
+
+
+def hop_site_dirs(dims, u, psi, lex, t_dir=3):
+    u, psi = _c128(u), _c128(psi)
+    out = np.empty((4, 3), dtype=np.complex128)
+    _get().orc_hop_site_dirs(_dims(dims), u.ctypes.data, psi.ctypes.data, lex, t_dir, out.ctypes.data)
     return out
 
 

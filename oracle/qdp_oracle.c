@@ -369,11 +369,14 @@ void orc_ape_smear_step(const int *L, const double *u_in, double *u_out, double 
 /* ---- hop (definition 5) ---------------------------------------------------
  * chi(x)_{s a} = sum_mu sum_b [ U_mu(x)_{ab} psi(x+mu)_{sb}
  *                             + conj(U_mu(x-mu)_{ba}) psi(x-mu)_{sb} ]      */
-void orc_hop_site(const int *L, const double *u, const double *psi, size_t lex, double *out24) {
+/* hop restricted to the directions mu != t_dir (t_dir = -1: all four) */
+void orc_hop_site_dirs(const int *L, const double *u, const double *psi, size_t lex, int t_dir,
+                       double *out24) {
     int x[4]; coords_of(L, lex, x);
     cplx chi[12];
     memset(chi, 0, sizeof chi);
     for (int mu = 0; mu < 4; mu++) {
+        if (mu == t_dir) continue;
         size_t lf = hop_lex(L, x, mu, +1), lb = hop_lex(L, x, mu, -1);
         const cplx *Uf = link_at(u, lex, mu), *Ub = link_at(u, lb, mu);
         const cplx *pf = (const cplx *)(psi + lf * 24), *pb = (const cplx *)(psi + lb * 24);
@@ -385,6 +388,9 @@ void orc_hop_site(const int *L, const double *u, const double *psi, size_t lex, 
                 }
     }
     memcpy(out24, chi, sizeof chi);
+}
+void orc_hop_site(const int *L, const double *u, const double *psi, size_t lex, double *out24) {
+    orc_hop_site_dirs(L, u, psi, lex, -1, out24);
 }
 
 void orc_hop_range(const int *L, const double *u, const double *psi, double *chi, int subset,
@@ -413,6 +419,25 @@ void orc_axpy_hop_range(const int *L, double a, double b, const double *u, const
 void orc_axpy_hop(const int *L, double a, double b, const double *u, const double *psi,
                   double *chi, int subset) {
     orc_axpy_hop_range(L, a, b, u, psi, chi, subset, 0, volume(L));
+}
+
+/* ---- quark smearing step (the SRC/SNK smearing stage of PAPER.md:82, 106) --
+ * chi(x) = a psi(x) + b sum_{mu != t_dir} [ U_mu(x) psi(x+mu) + U_mu(x-mu)^dag psi(x-mu) ]
+ * on the subset: one step of gauge-covariant Wuppertal / Gaussian smearing for t_dir = 3
+ * (spatial hops only); t_dir = -1 is definition 6 (axpy_hop). */
+void orc_smear_hop_range(const int *L, double a, double b, const double *u, const double *psi,
+                         double *chi, int t_dir, int subset, size_t lex_begin, size_t lex_end) {
+    for (size_t s = lex_begin; s < lex_end; s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        double h[24];
+        orc_hop_site_dirs(L, u, psi, s, t_dir, h);
+        for (int i = 0; i < 24; i++) chi[s * 24 + i] = a * psi[s * 24 + i] + b * h[i];
+    }
+}
+void orc_smear_hop(const int *L, double a, double b, const double *u, const double *psi,
+                   double *chi, int t_dir, int subset) {
+    orc_smear_hop_range(L, a, b, u, psi, chi, t_dir, subset, 0, volume(L));
 }
 
 /* ---- global reductions (definition 6) -------------------------------------
