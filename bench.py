@@ -224,6 +224,19 @@ def run_ours(args) -> dict | None:
     per_op_ms = {name: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)]))
                  for i, (name, _) in enumerate(ops)}
 
+    # ---- rows widened beyond the step: timed separately, not part of `value` -------
+    extra_ms = {}
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for name, fn in (("smear_hop", lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3)),):
+        for _ in range(3):
+            fn()
+        ev0.record(stream)
+        for _ in range(K):
+            fn()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        extra_ms[name] = ev0.elapsed_time(ev1) / K
+
     # ---- end to end through the C ABI from pinned host buffers ----------------------
     ke = max(1, min(args.e2e_steps, K))
     if args.no_e2e:
@@ -301,6 +314,11 @@ def run_ours(args) -> dict | None:
             "gpu_launches": int(launches),
             "roofline": roofline,
             "ops": op_report,
+            "extra_ops": {"smear_hop": {"ms": round(extra_ms["smear_hop"], 5),
+                                        "gbs": round(V * 51 * eb / extra_ms["smear_hop"] / 1e6, 1),
+                                        "frac": round(V * 51 * eb / extra_ms["smear_hop"] / 1e6 / peak, 4),
+                                        "note": "qdp_smear_hop, t_dir = 3 (row f2): u 27 + psi 12 + chi 12 complex per site; "
+                                                "not part of the step"}},
             "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
         }
         if world == 1 and not args.no_cpu_baseline:

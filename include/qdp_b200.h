@@ -184,6 +184,15 @@ int qdp_hop(qdp_field* chi, const qdp_field* u, const qdp_field* psi, qdp_subset
 int qdp_axpy_hop(qdp_field* chi, double a, double b, const qdp_field* u, const qdp_field* psi,
                  qdp_subset subset, double* norm2_out);
 
+/* one step of gauge-covariant quark smearing (Wuppertal / Gaussian:
+ * the source and sink smearing stages SRC, SNK of the paper's Fig. 4):
+ *   chi(x) = a psi(x) + b sum_{mu != t_dir} [ U_mu(x) psi(x+mu) + U_mu(x-mu)^dag psi(x-mu) ]
+ * for x in subset.  t_dir = 3: spatial hops only (time-slices never mix); t_dir = -1: all four
+ * directions, identical to qdp_axpy_hop; anything else is QDP_ERR_ARG.  Same fields, aliasing
+ * rule, norm2_out behaviour and casts as qdp_axpy_hop. */
+int qdp_smear_hop(qdp_field* chi, double a, double b, const qdp_field* u, const qdp_field* psi,
+                  int t_dir, qdp_subset subset, double* norm2_out);
+
 /* def. 6: global reductions over the subset, any kind; accumulated and returned
  * in fp64 for both precisions; fixed-shape tree.  Synchronous.
  *   qdp_norm2: out[0]   = sum_x sum_c |f_c(x)|^2

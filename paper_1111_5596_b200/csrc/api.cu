@@ -419,7 +419,7 @@ extern "C" int qdp_ape_smear_step(qdp_field* u_out, const qdp_field* u_in, doubl
 }
 
 static int hop_common(const char* who, qdp_field* chi, const qdp_field* u, const qdp_field* psi, qdp_subset subset,
-                      bool axpy, double a, double b, double* norm2_out) {
+                      bool axpy, double a, double b, double* norm2_out, int ndir = 4) {
     if (!ok_field(chi) || !ok_field(u) || !ok_field(psi) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "%s: bad argument", who);
     if (chi->kind != QDP_FERMION || psi->kind != QDP_FERMION || u->kind != QDP_GAUGE)
         return fail(QDP_ERR_KIND, "%s: need (fermion, gauge, fermion)", who);
@@ -430,7 +430,7 @@ static int hop_common(const char* who, qdp_field* chi, const qdp_field* u, const
     qdp_lattice* l = chi->lat;
     ENTER(l);
     CUDA_TRY(launch_hop(chi->prec, l->geom, chi->data, u->data, psi->data, subset, axpy, a, b, norm2_out != nullptr,
-                        reduce_buf(l), l->stream));
+                        reduce_buf(l), l->stream, ndir));
     if (norm2_out) return fetch_result(l, 1, norm2_out);
     return QDP_OK;
 }
@@ -441,6 +441,11 @@ extern "C" int qdp_hop(qdp_field* chi, const qdp_field* u, const qdp_field* psi,
 extern "C" int qdp_axpy_hop(qdp_field* chi, double a, double b, const qdp_field* u, const qdp_field* psi,
                             qdp_subset subset, double* norm2_out) {
     return hop_common("qdp_axpy_hop", chi, u, psi, subset, true, a, b, norm2_out);
+}
+extern "C" int qdp_smear_hop(qdp_field* chi, double a, double b, const qdp_field* u, const qdp_field* psi,
+                             int t_dir, qdp_subset subset, double* norm2_out) {
+    if (t_dir != 3 && t_dir != -1) return fail(QDP_ERR_ARG, "qdp_smear_hop: t_dir must be 3 or -1");
+    return hop_common("qdp_smear_hop", chi, u, psi, subset, true, a, b, norm2_out, t_dir == 3 ? 3 : 4);
 }
 
 extern "C" int qdp_norm2(const qdp_field* f, qdp_subset subset, double* out) {

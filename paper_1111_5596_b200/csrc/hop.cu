@@ -1,5 +1,6 @@
 // hop.cu -- chi(x) = sum_mu [ U_mu(x) psi(x+mu) + U_mu(x-mu)^dag psi(x-mu) ]   (def. 5)
-// and the fused chi = a psi + b hop(psi) with optional fused norm2 (def. 6).
+// and the fused chi = a psi + b hop(psi) with optional fused norm2 (def. 6); with NDIR = 3 the
+// time direction is left out: one step of Wuppertal / Gaussian quark smearing (qdp_smear_hop).
 // (SURVEY.md 8(a) rows a7, a8.)  One kernel per expression, no lattice-sized
 // temporaries -- the point of the paper's expression fusion.
 //
@@ -45,7 +46,7 @@ __device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
     }
 }
 
-template <class T, bool AXPY, bool NORM>
+template <class T, bool AXPY, bool NORM, int NDIR>
 __global__ void __launch_bounds__(kHopThreads, HopCfg<T>::kBlocks) hop_kernel(Geom g, typename Vec2<T>::type* __restrict__ chi,
                                                          const typename Vec2<T>::type* __restrict__ u,
                                                          const typename Vec2<T>::type* __restrict__ psi,
@@ -63,7 +64,7 @@ __global__ void __launch_bounds__(kHopThreads, HopCfg<T>::kBlocks) hop_kernel(Ge
         hop_dir<T, 0>(g, x, s, u, psi, acc);
         hop_dir<T, 1>(g, x, s, u, psi, acc);
         hop_dir<T, 2>(g, x, s, u, psi, acc);
-        hop_dir<T, 3>(g, x, s, u, psi, acc);
+        if (NDIR == 4) hop_dir<T, 3>(g, x, s, u, psi, acc);
         if (AXPY) {
             Spinor<T> p = ld_spinor<T>(psi, s);
 #pragma unroll
@@ -88,22 +89,27 @@ __global__ void __launch_bounds__(kHopThreads, HopCfg<T>::kBlocks) hop_kernel(Ge
 template <class T>
 static cudaError_t launch_hop_t(const Geom& g, void* chi, const void* u, const void* psi, int subset,
                                 bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb,
-                                cudaStream_t st) {
+                                cudaStream_t st, int ndir) {
     using T2 = typename Vec2<T>::type;
     int n = subset == 0 ? 2 * g.Vhp : g.Vh;
     int grid = (n + kHopThreads - 1) / kHopThreads;
     T2* c = (T2*)chi; const T2* uu = (const T2*)u; const T2* p = (const T2*)psi;
-    if (!axpy)            hop_kernel<T, false, false><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
-    else if (!want_norm2) hop_kernel<T, true, false><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
-    else                  hop_kernel<T, true, true><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
+    if (ndir == 3) {   // the smearing step is always the axpy form
+        if (!want_norm2) hop_kernel<T, true, false, 3><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
+        else             hop_kernel<T, true, true, 3><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
+    }
+    else if (!axpy)       hop_kernel<T, false, false, 4><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
+    else if (!want_norm2) hop_kernel<T, true, false, 4><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
+    else                  hop_kernel<T, true, true, 4><<<grid, kHopThreads, 0, st>>>(g, c, uu, p, subset, (T)a, (T)b, rb);
     g_launch_count++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_hop(int prec, const Geom& g, void* chi, const void* u, const void* psi, int subset,
-                       bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb, cudaStream_t st) {
-    return prec ? launch_hop_t<double>(g, chi, u, psi, subset, axpy, a, b, want_norm2, rb, st)
-                : launch_hop_t<float>(g, chi, u, psi, subset, axpy, a, b, want_norm2, rb, st);
+                       bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb, cudaStream_t st,
+                       int ndir) {
+    return prec ? launch_hop_t<double>(g, chi, u, psi, subset, axpy, a, b, want_norm2, rb, st, ndir)
+                : launch_hop_t<float>(g, chi, u, psi, subset, axpy, a, b, want_norm2, rb, st, ndir);
 }
 
 }  // namespace qdp

@@ -36,9 +36,10 @@ cudaError_t launch_sum(int prec, const Geom& g, int ncomp, const void* f, int su
                        double* partials, double* out_dev, cudaStream_t st);
 
 // hop.cu
+// ndir = 4: all directions; 3: mu = 0, 1, 2 only (qdp_smear_hop with t_dir = 3)
 cudaError_t launch_hop(int prec, const Geom& g, void* chi, const void* u, const void* psi, int subset,
                        bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb,
-                       cudaStream_t st);
+                       cudaStream_t st, int ndir = 4);
 
 // plaquette.cu
 cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb,

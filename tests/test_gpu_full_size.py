@@ -120,6 +120,13 @@ def _check_step(qdp, dims, prec, seed, n_ape_steps=1, warm=False):
     ne, no_ = qdp.qdp_norm2(chi, 1), qdp.qdp_norm2(chi, 2)
     assert abs(ne + no_ - sep) <= 1e-12 * sep
 
+    # ---- quark-smearing step (row f2): spatial hops only, sampled sites vs the oracle
+    n2 = qdp.qdp_smear_hop(chi, a, b, u, psi, 3, 0, want_norm2=True)
+    out = qdp.field_to_host(chi)
+    want = a * p64[sites] + b * np.stack([oracle.hop_site_dirs(dims, u64, p64, int(s), 3) for s in sites])
+    assert site_rel_err(_as64(out[sites]), want).max() <= TOL_SITE[prec]
+    assert abs(n2 - oracle.norm2(dims, _as64(out))) <= 1e-10 * n2
+
     # ---- shift: bit-exact on the whole lattice (one direction per axis, both signs on axis 3)
     sh = qdp.qdp_field_alloc(lat, 2, _prec_id(prec))
     for mu, sign in ((0, 1), (1, -1), (2, 1), (3, 1), (3, -1)):

@@ -338,3 +338,44 @@ def test_sweep_slab_order_gives_the_same_fields(qdp, dims, c2):
         qdp.qdp_lattice_set_sweep_slab(lat, 5)
     with pytest.raises(qdp.QdpError):
         qdp.qdp_lattice_set_sweep_slab(qdp.qdp_lattice_create((4, 4, 4, 4)), 2)   # L0/2*L1 = 8
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_smear_hop(qdp, lat_cache, dims, prec):
+    """qdp_smear_hop (row f2): spatial and four-direction steps on every subset vs the oracle."""
+    lat = lat_cache(dims)
+    hu = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 31), prec)
+    hp = synth.round_to(synth.spinor(dims, _seed(dims) + 32), prec)
+    sentinel = synth.round_to(synth.spinor(dims, _seed(dims) + 33, 1), prec)
+    u, psi = qdp.field_from_host(lat, 1, hu), qdp.field_from_host(lat, 2, hp)
+    a, b = synth.scalars_ab(_seed(dims) + 3)
+    if prec == "f32":
+        a, b = float(np.float32(a)), float(np.float32(b))
+    for t_dir in (3, -1):
+        for sub in SUBSETS:
+            chi = qdp.field_from_host(lat, 2, sentinel)
+            n2 = qdp.qdp_smear_hop(chi, a, b, u, psi, t_dir, sub, want_norm2=True)
+            got = qdp.field_to_host(chi)
+            want = oracle.smear_hop(dims, a, b, _as64(hu), _as64(hp), t_dir, sub, chi=_as64(sentinel))
+            assert site_rel_err(got, want).max() <= TOL_SITE[prec], (t_dir, sub)
+            assert abs(n2 - oracle.norm2(dims, want, sub)) <= TOL_SUM[prec] * n2
+            chi2 = qdp.field_from_host(lat, 2, sentinel)
+            qdp.qdp_smear_hop(chi2, a, b, u, psi, t_dir, sub)
+            assert np.array_equal(qdp.field_to_host(chi2), got)          # with and without the fused norm2
+            if t_dir == -1:                                               # identical to qdp_axpy_hop
+                chi3 = qdp.field_from_host(lat, 2, sentinel)
+                qdp.qdp_axpy_hop(chi3, a, b, u, psi, sub)
+                assert np.array_equal(qdp.field_to_host(chi3), got)
+    # a source on one time-slice stays there under the spatial step (exact zeros elsewhere)
+    on = (np.arange(synth.volume(dims)) // (dims[0] * dims[1] * dims[2])) == dims[3] // 2
+    src = hp.copy()
+    src[~on] = 0
+    bufs = [qdp.field_from_host(lat, 2, src), qdp.field_from_host(lat, 2, np.zeros_like(src))]
+    for _ in range(3):
+        qdp.qdp_smear_hop(bufs[1], 1.0, 0.25, u, bufs[0], 3)
+        bufs.reverse()
+    out = qdp.field_to_host(bufs[0])
+    assert np.all(out[~on] == 0) and np.abs(out[on]).max() > 0
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_smear_hop(bufs[1], 1.0, 0.25, u, bufs[0], 2)
