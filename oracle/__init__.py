@@ -62,6 +62,7 @@ def _get():
             "orc_norm2": ([P, I, P, I], D),
             "orc_inner": ([P, I, P, P, I, P], None),
             "orc_sum": ([P, I, P, I, P], None),
+            "orc_inner_timeslices": ([P, I, P, P, I, P], None),
             # the same loops over lex sites [begin, end): bounded samples for bench.py
             "orc_shift_bytes_range": ([P, Z, P, P, I, I, I, Z, Z], None),
             "orc_plaquette_range": ([P, P, I, Z, Z, P], None),
@@ -225,6 +226,15 @@ def inner(dims, a, b, subset=ALL):
     _get().orc_inner(_dims(dims), _reals(dims, a), a.ctypes.data, b.ctypes.data, subset,
                      out.ctypes.data)
     return complex(out[0], out[1])
+
+
+def inner_timeslices(dims, a, b, subset=ALL):
+    """out[t] = sum over the sites of time-slice x3 = t of conj(a) . b  (row f3), complex [L3]."""
+    a, b = _c128(a), _c128(b)
+    out = np.empty(2 * int(dims[3]))
+    _get().orc_inner_timeslices(_dims(dims), _reals(dims, a), a.ctypes.data, b.ctypes.data, subset,
+                                out.ctypes.data)
+    return out[0::2] + 1j * out[1::2]
 
 
 def sum_field(dims, f, subset=ALL):

@@ -477,6 +477,29 @@ void orc_inner(const int *L, int reals, const double *a, const double *b, int su
     orc_inner_range(L, reals, a, b, subset, 0, volume(L), out2);
 }
 
+/* time-slice sums, the reduction under every hadron two-point function
+ * (HAD stage):
+ *   out[t] = sum_{x in subset, x3 = t} sum_c conj(a_c(x)) b_c(x),   t = 0 .. L3-1   (re, im pairs).
+ * With a = b a quark propagator column this is the pion correlator of that column. */
+void orc_inner_timeslices(const int *L, int reals, const double *a, const double *b, int subset,
+                          double *out) {
+    for (int t = 0; t < L[3]; t++) {
+        ksum kr = { 0, 0 }, ki = { 0, 0 };
+        for (size_t s = 0; s < volume(L); s++) {
+            int x[4]; coords_of(L, s, x);
+            if (x[3] != t || !in_subset(x, subset)) continue;
+            for (int c = 0; c < reals / 2; c++) {
+                cplx p = c_mul(c_conj(((const cplx *)a)[s * (reals / 2) + c]),
+                               ((const cplx *)b)[s * (reals / 2) + c]);
+                k_add(&kr, p.re);
+                k_add(&ki, p.im);
+            }
+        }
+        out[2 * t] = k_val(&kr);
+        out[2 * t + 1] = k_val(&ki);
+    }
+}
+
 /* out[c] = sum_x f_c(x), per real component (re, im interleaved like f). */
 void orc_sum(const int *L, int reals, const double *f, int subset, double *out) {
     size_t V = volume(L);
