@@ -227,7 +227,8 @@ def run_ours(args) -> dict | None:
     # ---- rows widened beyond the step: timed separately, not part of `value` -------
     extra_ms = {}
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    for name, fn in (("smear_hop", lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3)),):
+    for name, fn in (("smear_hop", lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3)),
+                     ("inner_timeslices", lambda: q.qdp_inner_timeslices(psi, chi))):
         for _ in range(3):
             fn()
         ev0.record(stream)
@@ -318,7 +319,12 @@ def run_ours(args) -> dict | None:
                                         "gbs": round(V * 51 * eb / extra_ms["smear_hop"] / 1e6, 1),
                                         "frac": round(V * 51 * eb / extra_ms["smear_hop"] / 1e6 / peak, 4),
                                         "note": "qdp_smear_hop, t_dir = 3 (row f2): u 27 + psi 12 + chi 12 complex per site; "
-                                                "not part of the step"}},
+                                                "not part of the step"},
+                          "inner_timeslices": {"ms": round(extra_ms["inner_timeslices"], 5),
+                                               "gbs": round(V * 24 * eb / extra_ms["inner_timeslices"] / 1e6, 1),
+                                               "frac": round(V * 24 * eb / extra_ms["inner_timeslices"] / 1e6 / peak, 4),
+                                               "note": "qdp_inner_timeslices (row f3): 2 x 12 complex per site, includes the "
+                                                       "host round trip; not part of the step"}},
             "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
         }
         if world == 1 and not args.no_cpu_baseline:

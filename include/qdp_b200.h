@@ -202,6 +202,14 @@ int qdp_norm2(const qdp_field* f, qdp_subset subset, double* out);
 int qdp_inner(const qdp_field* a, const qdp_field* b, qdp_subset subset, double out[2]);
 int qdp_sum(const qdp_field* f, qdp_subset subset, double* out);
 
+/* time-slice sums, the reduction under every hadron two-point function
+ * (the HAD stage of the paper's Fig. 4):
+ *   out[2t], out[2t+1] = (re, im) of sum_{x in subset, x3 = t} sum_c conj(a_c(x)) b_c(x),  t < L3.
+ * out: host, 2*L3 doubles.  a == b gives the per-slice norm (the pion correlator of a propagator
+ * column).  Same kinds/precisions rule as qdp_inner; fp64 accumulation, fixed summation order.
+ * Synchronous. */
+int qdp_inner_timeslices(const qdp_field* a, const qdp_field* b, qdp_subset subset, double* out);
+
 /* Block the host until every call enqueued on the lattice's stream has finished. */
 int qdp_lattice_sync(qdp_lattice* lat);
 

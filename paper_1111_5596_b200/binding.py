@@ -18,7 +18,7 @@ __all__ = [
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
-    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop",
+    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
 ]
@@ -65,6 +65,7 @@ DECLARED_SYMBOLS = {
     "qdp_hop": ([_P, _P, _P, _I], _I),
     "qdp_axpy_hop": ([_P, _D, _D, _P, _P, _I, _P], _I),
     "qdp_smear_hop": ([_P, _D, _D, _P, _P, _I, _I, _P], _I),
+    "qdp_inner_timeslices": ([_P, _P, _I, _P], _I),
     "qdp_norm2": ([_P, _I, _P], _I),
     "qdp_inner": ([_P, _P, _I, _P], _I),
     "qdp_sum": ([_P, _I, _P], _I),
@@ -292,6 +293,13 @@ def qdp_inner(a: Field, b: Field, subset: int = QDP_ALL) -> complex:
     out = np.empty(2)
     _check(_lib.qdp_inner(a.handle, b.handle, subset, out.ctypes.data))
     return complex(out[0], out[1])
+
+
+def qdp_inner_timeslices(a: Field, b: Field, subset: int = QDP_ALL) -> np.ndarray:
+    """complex [L3]: sum over the sites of each time-slice x3 = t of conj(a) . b"""
+    out = np.empty(2 * int(a.lat.dims[3]), dtype=np.float64)
+    _check(_lib.qdp_inner_timeslices(a.handle, b.handle, subset, out.ctypes.data))
+    return out[0::2] + 1j * out[1::2]
 
 
 def qdp_sum(f: Field, subset: int = QDP_ALL) -> np.ndarray:

@@ -152,6 +152,7 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     size_t npart = (size_t)4 * kMaxPartialBlocks;
     if (npart < 4 * (nwarp_max + ngroup_max)) npart = 4 * (nwarp_max + ngroup_max);
     if (npart < (size_t)2 * 36 * 64) npart = (size_t)2 * 36 * 64;
+    if (npart < (size_t)34 * dims[3]) npart = (size_t)34 * dims[3];   // qdp_inner_timeslices: 2*16*L3 partials + 2*L3 results
     const size_t counter_bytes = (ngroup_max + 1) * sizeof(unsigned int);
     int rc;
     void* p = nullptr;
@@ -465,6 +466,23 @@ extern "C" int qdp_inner(const qdp_field* a, const qdp_field* b, qdp_subset subs
     ENTER(l);
     CUDA_TRY(launch_inner(a->prec, l->geom, a->ncomp, a->data, b->data, subset, reduce_buf(l), l->stream));
     return fetch_result(l, 2, out);
+}
+
+extern "C" int qdp_inner_timeslices(const qdp_field* a, const qdp_field* b, qdp_subset subset, double* out) {
+    if (!ok_field(a) || !ok_field(b) || !out || !ok_subset(subset))
+        return fail(QDP_ERR_ARG, "qdp_inner_timeslices: bad argument");
+    int rc = check_pair("qdp_inner_timeslices", a, b);
+    if (rc != QDP_OK) return rc;
+    if (a->kind != b->kind) return fail(QDP_ERR_KIND, "qdp_inner_timeslices: kinds differ");
+    qdp_lattice* l = a->lat;
+    ENTER(l);
+    const int L3 = l->geom.L3;
+    double* out_dev = l->partials + (size_t)2 * 16 * L3;   // behind the per-block partials
+    CUDA_TRY(launch_inner_timeslices(a->prec, l->geom, a->ncomp, a->data, b->data, subset, l->partials, out_dev,
+                                     l->stream));
+    CUDA_TRY(cudaMemcpyAsync(out, out_dev, (size_t)2 * L3 * sizeof(double), cudaMemcpyDeviceToHost, l->stream));
+    CUDA_TRY(cudaStreamSynchronize(l->stream));
+    return QDP_OK;
 }
 
 extern "C" int qdp_sum(const qdp_field* f, qdp_subset subset, double* out) {

@@ -35,6 +35,10 @@ cudaError_t launch_inner(int prec, const Geom& g, int ncomp, const void* a, cons
 cudaError_t launch_sum(int prec, const Geom& g, int ncomp, const void* f, int subset,
                        double* partials, double* out_dev, cudaStream_t st);
 
+// partials: scratch of 2*16*L3 doubles; out_dev: 2*L3 doubles on the device
+cudaError_t launch_inner_timeslices(int prec, const Geom& g, int ncomp, const void* a, const void* b, int subset,
+                                    double* partials, double* out_dev, cudaStream_t st);
+
 // hop.cu
 // ndir = 4: all directions; 3: mu = 0, 1, 2 only (qdp_smear_hop with t_dir = 3)
 cudaError_t launch_hop(int prec, const Geom& g, void* chi, const void* u, const void* psi, int subset,

@@ -167,6 +167,74 @@ __global__ void sum_finish_kernel(int nblk, const double* __restrict__ partials,
     out[c * 2 + k] = t;
 }
 
+// ---- time-slice inner products -----------------------------------
+// out[t] = sum over the sites with x3 = t of conj(a) . b.  In the blocked layout the half-indices of
+// a time-slice are one run [t*s3, (t+1)*s3) per parity half, so when s3 is a multiple of 32 a slice
+// is two contiguous element ranges and the kernel streams them (blockIdx.y = t, kTsBlocks blocks
+// per slice); otherwise (tiny or ragged lattices) every block scans its half and keeps the
+// elements whose site has x3 = t.  One partial per block, summed in block order by the finish
+// kernel: deterministic, fp64.
+constexpr int kTsBlocks = 16;
+template <class T2, bool FAST>
+__global__ void __launch_bounds__(kReduceThreads) inner_ts_kernel(Geom g, int ncomp, const T2* __restrict__ a,
+                                                                 const T2* __restrict__ b, int subset,
+                                                                 double* __restrict__ partials) {
+    __shared__ double sm[2][kReduceThreads / 32];
+    const int t = blockIdx.y;
+    const unsigned stride = gridDim.x * kReduceThreads;
+    double acc[2] = {0.0, 0.0};
+    for (int p = (subset == 2 ? 1 : 0); p <= (subset == 1 ? 0 : 1); p++) {
+        if (FAST) {
+            const size_t begin = ((size_t)p * g.Vhp + (size_t)t * g.s3) * ncomp;
+            const unsigned n = (unsigned)g.s3 * ncomp;
+            const T2 *pa = a + begin, *pb = b + begin;
+#pragma unroll 4
+            for (unsigned e = blockIdx.x * kReduceThreads + threadIdx.x; e < n; e += stride) {
+                const T2 va = __ldg(pa + e), vb = __ldg(pb + e);
+                acc[0] += (double)va.x * (double)vb.x + (double)va.y * (double)vb.y;
+                acc[1] += (double)va.x * (double)vb.y - (double)va.y * (double)vb.x;
+            }
+        } else {
+            const size_t begin = (size_t)p * g.Vhp * ncomp;
+            const unsigned n = (unsigned)g.Vhp * ncomp;
+            for (unsigned e = blockIdx.x * kReduceThreads + threadIdx.x; e < n; e += stride) {
+                const int h = (int)(e / (ncomp * 32u)) * 32 + (int)(e & 31u);
+                if (h >= g.Vh || h / g.s3 != t) continue;
+                const T2 va = __ldg(a + begin + e), vb = __ldg(b + begin + e);
+                acc[0] += (double)va.x * (double)vb.x + (double)va.y * (double)vb.y;
+                acc[1] += (double)va.x * (double)vb.y - (double)va.y * (double)vb.x;
+            }
+        }
+    }
+    block_tree<2, kReduceThreads>(acc, sm);
+    if (threadIdx.x == 0) {
+        partials[((size_t)t * gridDim.x + blockIdx.x) * 2 + 0] = acc[0];
+        partials[((size_t)t * gridDim.x + blockIdx.x) * 2 + 1] = acc[1];
+    }
+}
+__global__ void inner_ts_finish_kernel(int nblk, const double* __restrict__ partials, double* __restrict__ out) {
+    const int t = blockIdx.x, k = threadIdx.x;   // 2 threads: re, im
+    double s = 0.0;
+    for (int b = 0; b < nblk; b++) s += partials[((size_t)t * nblk + b) * 2 + k];
+    out[t * 2 + k] = s;
+}
+
+cudaError_t launch_inner_timeslices(int prec, const Geom& g, int ncomp, const void* a, const void* b, int subset,
+                                    double* partials, double* out_dev, cudaStream_t st) {
+    dim3 grid(kTsBlocks, g.L3);
+    const bool fast = (g.s3 & 31) == 0;
+    if (prec) {
+        if (fast) inner_ts_kernel<double2, true><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const double2*)a, (const double2*)b, subset, partials);
+        else      inner_ts_kernel<double2, false><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const double2*)a, (const double2*)b, subset, partials);
+    } else {
+        if (fast) inner_ts_kernel<float2, true><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const float2*)a, (const float2*)b, subset, partials);
+        else      inner_ts_kernel<float2, false><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const float2*)a, (const float2*)b, subset, partials);
+    }
+    inner_ts_finish_kernel<<<g.L3, 2, 0, st>>>(kTsBlocks, partials, out_dev);
+    g_launch_count += 2;
+    return cudaGetLastError();
+}
+
 template <class T2, int NCOMP>
 static void norm2_dispatch(const Geom& g, const void* f, int subset, const ReduceBuf& rb, cudaStream_t st) {
     size_t n = (size_t)g.Vhp * NCOMP * (subset == 0 ? 2 : 1);

@@ -127,6 +127,12 @@ def _check_step(qdp, dims, prec, seed, n_ape_steps=1, warm=False):
     assert site_rel_err(_as64(out[sites]), want).max() <= TOL_SITE[prec]
     assert abs(n2 - oracle.norm2(dims, _as64(out))) <= 1e-10 * n2
 
+    # ---- time-slice inner products (row f3): whole-lattice oracle on the downloaded fields
+    ts = qdp.qdp_inner_timeslices(psi, chi)
+    want_ts = oracle.inner_timeslices(dims, p64, _as64(out))
+    assert np.abs(ts - want_ts).max() <= (1e-10 if prec == "f64" else 1e-6) * 8 * n2p
+    assert abs(ts.sum() - qdp.qdp_inner(psi, chi)) <= 1e-12 * 8 * n2p
+
     # ---- shift: bit-exact on the whole lattice (one direction per axis, both signs on axis 3)
     sh = qdp.qdp_field_alloc(lat, 2, _prec_id(prec))
     for mu, sign in ((0, 1), (1, -1), (2, 1), (3, 1), (3, -1)):

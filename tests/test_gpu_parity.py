@@ -379,3 +379,29 @@ def test_smear_hop(qdp, lat_cache, dims, prec):
     assert np.all(out[~on] == 0) and np.abs(out[on]).max() > 0
     with pytest.raises(qdp.QdpError):
         qdp.qdp_smear_hop(bufs[1], 1.0, 0.25, u, bufs[0], 2)
+
+
+@pytest.mark.parametrize("dims", SMALL + [(2, 2, 2, 40), C2])
+@pytest.mark.parametrize("prec", PRECS)
+@pytest.mark.parametrize("kind", ["fermion", "matrix"])
+def test_inner_timeslices(qdp, lat_cache, dims, prec, kind):
+    """qdp_inner_timeslices (row f3) on every subset vs the oracle; both the streaming path
+    (s3 a multiple of 32) and the scanning path (ragged lattices)."""
+    lat = lat_cache(dims)
+    ha = synth.round_to(_field(dims, kind, _seed(dims) + 41), prec)
+    hb = synth.round_to(_field(dims, kind, _seed(dims) + 42) if kind == "matrix" else synth.spinor(dims, _seed(dims) + 42, 1), prec)
+    a, b = qdp.field_from_host(lat, KINDS[kind], ha), qdp.field_from_host(lat, KINDS[kind], hb)
+    scale = oracle.norm2(dims, _as64(ha)) + oracle.norm2(dims, _as64(hb))
+    for sub in SUBSETS:
+        got = qdp.qdp_inner_timeslices(a, b, sub)
+        want = oracle.inner_timeslices(dims, _as64(ha), _as64(hb), sub)
+        assert got.shape == (dims[3],)
+        assert np.abs(got - want).max() <= TOL_SUM[prec] * scale / dims[3], sub
+        assert np.array_equal(got, qdp.qdp_inner_timeslices(a, b, sub))          # deterministic
+        assert abs(got.sum() - qdp.qdp_inner(a, b, sub)) <= 1e-12 * scale
+    n = qdp.qdp_inner_timeslices(a, a)
+    # (the imaginary part is a sum of x*y - y*x terms: zero up to the rounding of the fused multiply-add)
+    assert np.abs(n.imag).max() <= 1e-14 * scale and abs(n.real.sum() - qdp.qdp_norm2(a)) <= 1e-12 * scale
+    if kind == "fermion":
+        with pytest.raises(qdp.QdpError):
+            qdp.qdp_inner_timeslices(a, qdp.qdp_field_alloc(lat, 0, 1 if prec == "f64" else 0))
