@@ -405,3 +405,40 @@ def test_inner_timeslices(qdp, lat_cache, dims, prec, kind):
     if kind == "fermion":
         with pytest.raises(qdp.QdpError):
             qdp.qdp_inner_timeslices(a, qdp.qdp_field_alloc(lat, 0, 1 if prec == "f64" else 0))
+
+
+def test_streams_copy_and_wrapped_memory(qdp):
+    """Plumbing entry points: qdp_lattice_set_stream / qdp_lattice_sync with a torch stream,
+    qdp_field_copy, qdp_field_wrap on torch-owned memory (size check included)."""
+    import torch
+    dims = (8, 4, 4, 6)
+    lat = qdp.qdp_lattice_create(dims)
+    hu, hp = synth.gauge_hot(dims, 51), synth.spinor(dims, 52)
+    stream = torch.cuda.Stream()
+    qdp.qdp_lattice_set_stream(lat, stream.cuda_stream)
+    u, psi = qdp.field_from_host(lat, 1, hu), qdp.field_from_host(lat, 2, hp)
+    chi, cpy = qdp.qdp_field_alloc(lat, 2, 1), qdp.qdp_field_alloc(lat, 2, 1)
+    for _ in range(4):                       # a chain of asynchronous calls on the user's stream
+        qdp.qdp_hop(chi, u, psi, 0)
+        qdp.qdp_field_copy(cpy, chi)
+        qdp.qdp_smear_hop(chi, 0.5, 0.1, u, cpy, 3)
+    qdp.qdp_lattice_sync(lat)
+    assert stream.query()                    # nothing left in flight after the sync
+    want = oracle.smear_hop(dims, 0.5, 0.1, hu, oracle.hop(dims, hu, hp), 3)
+    assert site_rel_err(qdp.field_to_host(chi), want).max() <= TOL_SITE["f64"]
+    assert np.array_equal(qdp.field_to_host(cpy), qdp.field_to_host(cpy))
+    assert site_rel_err(qdp.field_to_host(cpy), oracle.hop(dims, hu, hp)).max() <= TOL_SITE["f64"]
+    qdp.qdp_lattice_set_stream(lat, None)    # back to the default stream
+    assert abs(qdp.qdp_norm2(psi) - oracle.norm2(dims, hp)) <= 1e-10 * oracle.norm2(dims, hp)
+    # wrapped torch memory: the field lives in the tensor
+    nbytes = qdp.qdp_field_bytes(lat, 2, 1)
+    buf = torch.zeros(nbytes, dtype=torch.uint8, device="cuda:0")
+    w = qdp.qdp_field_wrap(lat, 2, 1, buf.data_ptr(), nbytes, storage=buf)
+    qdp.qdp_field_copy(w, psi)
+    qdp.qdp_lattice_sync(lat)
+    assert int(buf.count_nonzero()) > nbytes // 2
+    assert qdp.qdp_norm2(w) == qdp.qdp_norm2(psi)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_field_wrap(lat, 2, 1, buf.data_ptr(), nbytes - 16)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_field_copy(w, u)              # kinds differ
