@@ -50,6 +50,8 @@ def _get():
             "orc_polar_unitary": ([P, P], None),
             "orc_proj_su3": ([P, P], None),
             "orc_min_eig_vdv": ([P], D),
+            "orc_gram_schmidt_su3": ([P, P], None),
+            "orc_reunitarize": ([P, I, P, P, I, I], None),
             "orc_staple_site": ([P, P, Z, I, I, P], I),
             "orc_ape_blend_site": ([P, P, Z, I, D, I, P], None),
             "orc_ape_site": ([P, P, Z, I, D, I, P], None),
@@ -140,6 +142,25 @@ def proj_su3(V):
     out = np.empty((3, 3), dtype=np.complex128)
     _get().orc_proj_su3(V.ctypes.data, out.ctypes.data)
     return out
+
+
+def gram_schmidt_su3(V):
+    V = _c128(V)
+    out = np.empty((3, 3), dtype=np.complex128)
+    _get().orc_gram_schmidt_su3(V.ctypes.data, out.ctypes.data)
+    return out
+
+
+POLAR, GRAM_SCHMIDT = 0, 1
+
+
+def reunitarize(dims, f, method=POLAR, subset=ALL, out=None):
+    """Every 3x3 matrix of the field ([V,4,3,3] or [V,3,3]) projected to SU(3) (row f2)."""
+    f = _c128(f)
+    res = np.zeros_like(f) if out is None else _c128(out).copy()
+    nmat = f.size // (volume(dims) * 9)
+    _get().orc_reunitarize(_dims(dims), nmat, f.ctypes.data, res.ctypes.data, method, subset)
+    return res
 
 
 def min_eig_vdv(V):

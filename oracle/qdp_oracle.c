@@ -285,6 +285,52 @@ void orc_proj_su3(const double *Vin, double *out) {
     for (int i = 0; i < 9; i++) o[i] = c_mul(W[i], ph);
 }
 
+/* ---- reunitarisation of whole fields (alternative projections) ----------
+ * Gram-Schmidt: row0 = v0/|v0|; row1 = v1 - (row0 . v1) row0, normalised, with (a . b) = sum_j conj(a_j) b_j;
+ * row2 = conj(row0 x row1).  The result is in SU(3) by construction; unlike Proj it is not gauge
+ * covariant (reading A8), which is why the APE step does not use it. */
+void orc_gram_schmidt_su3(const double *Vin, double *out) {
+    const cplx *v = (const cplx *)Vin;
+    cplx r[9];
+    double n0 = 0;
+    for (int j = 0; j < 3; j++) n0 += v[j].re * v[j].re + v[j].im * v[j].im;
+    n0 = sqrt(n0);
+    for (int j = 0; j < 3; j++) r[j] = c_scale(1.0 / n0, v[j]);
+    cplx dot = { 0, 0 };
+    for (int j = 0; j < 3; j++) dot = c_add(dot, c_mul(c_conj(r[j]), v[3 + j]));
+    double n1 = 0;
+    for (int j = 0; j < 3; j++) {
+        cplx t = c_mul(dot, r[j]);
+        r[3 + j].re = v[3 + j].re - t.re;
+        r[3 + j].im = v[3 + j].im - t.im;
+        n1 += r[3 + j].re * r[3 + j].re + r[3 + j].im * r[3 + j].im;
+    }
+    n1 = sqrt(n1);
+    for (int j = 0; j < 3; j++) r[3 + j] = c_scale(1.0 / n1, r[3 + j]);
+    for (int j = 0; j < 3; j++) {
+        int a = (j + 1) % 3, b = (j + 2) % 3;
+        cplx x = c_mul(r[a], r[3 + b]), y = c_mul(r[b], r[3 + a]);
+        cplx c = { x.re - y.re, x.im - y.im };
+        r[6 + j] = c_conj(c);
+    }
+    memcpy(out, r, sizeof r);
+}
+
+/* out(x) = method(in(x)) for every 3x3 matrix of the sites in the subset; method 0 = Proj
+ * (definition 4), 1 = Gram-Schmidt.  nmat = matrices per site (4 for a gauge field, 1 for a colour
+ * matrix).  Sites outside the subset keep what `out` held. */
+void orc_reunitarize(const int *L, int nmat, const double *in, double *out, int method, int subset) {
+    for (size_t s = 0; s < volume(L); s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        for (int m = 0; m < nmat; m++) {
+            const double *vi = in + (s * nmat + m) * 18;
+            double *vo = out + (s * nmat + m) * 18;
+            if (method == 0) orc_proj_su3(vi, vo); else orc_gram_schmidt_su3(vi, vo);
+        }
+    }
+}
+
 /* smallest singular value^2 of V (lambda_min of V^dag V), for reading A10 */
 double orc_min_eig_vdv(const double *Vin) {
     const cplx *V = (const cplx *)Vin;
