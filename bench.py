@@ -229,7 +229,8 @@ def run_ours(args) -> dict | None:
     extra_ms = {}
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for name, fn in (("smear_hop", lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3)),
-                     ("inner_timeslices", lambda: q.qdp_inner_timeslices(psi, chi))):
+                     ("inner_timeslices", lambda: q.qdp_inner_timeslices(psi, chi)),
+                     ("reunitarize_gs", lambda: q.qdp_reunitarize(u2, u, q.QDP_REUNIT_GRAM_SCHMIDT))):
         for _ in range(3):
             fn()
         ev0.record(stream)
@@ -364,7 +365,12 @@ def run_ours(args) -> dict | None:
                                                "gbs": round(V * 24 * eb / extra_ms["inner_timeslices"] / 1e6, 1),
                                                "frac": round(V * 24 * eb / extra_ms["inner_timeslices"] / 1e6 / peak, 4),
                                                "note": "qdp_inner_timeslices (row f3): 2 x 12 complex per site, includes the "
-                                                       "host round trip; not part of the step"}},
+                                                       "host round trip; not part of the step"},
+                          "reunitarize_gs": {"ms": round(extra_ms["reunitarize_gs"], 5),
+                                             "gbs": round(V * 60 * eb / extra_ms["reunitarize_gs"] / 1e6, 1),
+                                             "frac": round(V * 60 * eb / extra_ms["reunitarize_gs"] / 1e6 / peak, 4),
+                                             "note": "qdp_reunitarize, Gram-Schmidt (row f2): 24 complex read (rows 0, 1 of four "
+                                                     "links; row 2 is not an input) + 36 written per site; not part of the step"}},
             "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
         }
         if world == 1 and not args.no_cpu_baseline:

@@ -171,6 +171,17 @@ int qdp_plaquette(const qdp_field* u, qdp_subset subset, double out[3]);
 int qdp_ape_smear_step(qdp_field* u_out, const qdp_field* u_in, double alpha, int t_dir,
                        qdp_subset subset);
 
+/* SURVEY.md 8(f) row f2 (alternative projections) -- every 3x3 matrix of the sites in the subset
+ * projected to SU(3):
+ *   method QDP_REUNIT_POLAR (0):        Proj of def. 4 (unitary polar factor, determinant phase
+ *                                       removed; gauge covariant; what the APE step applies);
+ *   method QDP_REUNIT_GRAM_SCHMIDT (1): row0 normalised, row1 orthogonalised against it and
+ *                                       normalised, row2 = conj(row0 x row1) (cheaper, not covariant).
+ * u_out, u_in: QDP_GAUGE or QDP_COLOR_MATRIX of the same kind and precision; site-local, so
+ * u_out == u_in is allowed.  Arithmetic in fp64 for both precisions.  Asynchronous. */
+enum { QDP_REUNIT_POLAR = 0, QDP_REUNIT_GRAM_SCHMIDT = 1 };
+int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset);
+
 /* def. 5: chi(x)_{s a} = sum_mu sum_b [ U_mu(x)_{ab} psi(x+mu)_{s b}
  *                                      + conj(U_mu(x-mu)_{ba}) psi(x-mu)_{s b} ]
  * for x in subset (no gamma matrices, no kappa, periodic in all directions).

@@ -419,6 +419,22 @@ extern "C" int qdp_ape_smear_step(qdp_field* u_out, const qdp_field* u_in, doubl
     return QDP_OK;
 }
 
+extern "C" int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset) {
+    if (!ok_field(u_out) || !ok_field(u_in) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_reunitarize: bad argument");
+    if (method != QDP_REUNIT_POLAR && method != QDP_REUNIT_GRAM_SCHMIDT)
+        return fail(QDP_ERR_ARG, "qdp_reunitarize: unknown method %d", method);
+    if (u_in->kind == QDP_FERMION || u_out->kind != u_in->kind)
+        return fail(QDP_ERR_KIND, "qdp_reunitarize: need two gauge fields or two colour matrices");
+    int rc = check_pair("qdp_reunitarize", u_out, u_in);
+    if (rc != QDP_OK) return rc;
+    if (u_out != u_in && u_out->data != u_in->data && overlaps(u_out, u_in))
+        return fail(QDP_ERR_ALIAS, "qdp_reunitarize: u_out partially overlaps u_in");
+    qdp_lattice* l = u_out->lat;
+    ENTER(l);
+    CUDA_TRY(launch_reunit(u_out->prec, l->geom, u_out->ncomp, u_out->data, u_in->data, method, subset, l->stream));
+    return QDP_OK;
+}
+
 static int hop_common(const char* who, qdp_field* chi, const qdp_field* u, const qdp_field* psi, qdp_subset subset,
                       bool axpy, double a, double b, double* norm2_out, int ndir = 4) {
     if (!ok_field(chi) || !ok_field(u) || !ok_field(psi) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "%s: bad argument", who);

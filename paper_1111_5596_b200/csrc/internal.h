@@ -49,6 +49,10 @@ cudaError_t launch_hop(int prec, const Geom& g, void* chi, const void* u, const 
 cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb,
                              cudaStream_t st);
 
+// reunit.cu: method 0 = Proj (polar factor, determinant phase removed), 1 = Gram-Schmidt; in place allowed
+cudaError_t launch_reunit(int prec, const Geom& g, int ncomp, void* out, const void* in, int method, int subset,
+                          cudaStream_t st);
+
 // ape.cu
 cudaError_t launch_ape(int prec, const Geom& g, void* u_out, const void* u_in, double alpha, int t_dir,
                        int subset, cudaStream_t st);

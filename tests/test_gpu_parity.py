@@ -442,3 +442,41 @@ def test_streams_copy_and_wrapped_memory(qdp):
         qdp.qdp_field_wrap(lat, 2, 1, buf.data_ptr(), nbytes - 16)
     with pytest.raises(qdp.QdpError):
         qdp.qdp_field_copy(w, u)              # kinds differ
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_reunitarize(qdp, lat_cache, dims, prec):
+    """qdp_reunitarize (row f2): Proj and Gram-Schmidt on gauge fields and colour matrices,
+    every subset, out of place and in place."""
+    lat = lat_cache(dims)
+    P = 1 if prec == "f64" else 0
+    # links pushed off the group (general matrices, well conditioned); colour matrices fully general
+    hg = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 61) + 0.2 * synth.gauge_hot(dims, _seed(dims) + 62), prec)
+    hm = synth.round_to(synth.color_matrix(dims, _seed(dims) + 63), prec)
+    unit_bar = 1e-12 if prec == "f64" else 1e-5
+    for kind, host in ((1, hg), (0, hm)):
+        src = qdp.field_from_host(lat, kind, host)
+        for method in (qdp.QDP_REUNIT_POLAR, qdp.QDP_REUNIT_GRAM_SCHMIDT):
+            if kind == 0 and method == qdp.QDP_REUNIT_POLAR and prec == "f32":
+                continue      # Gaussian 3x3 matrices can be arbitrarily ill conditioned: no fp32 bar for Proj
+            for sub in SUBSETS:
+                sentinel = np.full_like(host, 3.0 - 2.0j)
+                dst = qdp.field_from_host(lat, kind, sentinel)
+                qdp.qdp_reunitarize(dst, src, method, sub)
+                got = qdp.field_to_host(dst)
+                want = oracle.reunitarize(dims, _as64(host), method, sub, out=_as64(sentinel))
+                fixed, n_centre = z3_fix(links(_as64(got)), links(want))
+                tol = TOL_SITE[prec] * (1 if kind == 1 else 50)     # general matrices: cond up to ~50
+                assert site_rel_err(fixed, links(want)).max() <= tol, (kind, method, sub)
+                assert n_centre == 0 or method == qdp.QDP_REUNIT_POLAR
+            work = qdp.field_from_host(lat, kind, host)            # in place, whole lattice
+            qdp.qdp_reunitarize(work, work, method)
+            g = links(_as64(qdp.field_to_host(work)))
+            assert np.abs(g @ np.conj(np.swapaxes(g, 1, 2)) - np.eye(3)).max() <= unit_bar * (1 if kind == 1 else 50)
+            assert np.abs(np.linalg.det(g) - 1).max() <= unit_bar * (1 if kind == 1 else 50)
+    psi = qdp.qdp_field_alloc(lat, 2, P)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_reunitarize(psi, psi, 0)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_reunitarize(qdp.field_from_host(lat, 1, hg), qdp.field_from_host(lat, 1, hg), 2)
