@@ -51,6 +51,7 @@ def _get():
             "orc_proj_su3": ([P, P], None),
             "orc_min_eig_vdv": ([P], D),
             "orc_gram_schmidt_su3": ([P, P], None),
+            "orc_matmul": ([P, P, I, I, P, I, I, I, P, I, I, I, I, I, I], None),
             "orc_reunitarize": ([P, I, P, P, I, I], None),
             "orc_staple_site": ([P, P, Z, I, I, P], I),
             "orc_ape_blend_site": ([P, P, Z, I, D, I, P], None),
@@ -141,6 +142,16 @@ def proj_su3(V):
     V = _c128(V)
     out = np.empty((3, 3), dtype=np.complex128)
     _get().orc_proj_su3(V.ctypes.data, out.ctypes.data)
+    return out
+
+
+def matmul(dims, dst, id_, a, ia, adj_a, b, ib, adj_b, mu=-1, sign=1, subset=ALL):
+    """dst[:, id_] = op(a[:, ia])(x) @ op(b[:, ib])(x + sign*mu) on the subset (row f1); fields are
+    [V,3,3] (index 0) or [V,4,3,3]; returns the updated copy of dst."""
+    a, b, out = _c128(a), _c128(b), _c128(dst).copy()
+    V = volume(dims)
+    _get().orc_matmul(_dims(dims), out.ctypes.data, out.size // (9 * V), id_, a.ctypes.data, a.size // (9 * V), ia,
+                      int(adj_a), b.ctypes.data, b.size // (9 * V), ib, int(adj_b), mu, sign, subset)
     return out
 
 

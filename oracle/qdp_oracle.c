@@ -285,6 +285,26 @@ void orc_proj_su3(const double *Vin, double *out) {
     for (int i = 0; i < 9; i++) o[i] = c_mul(W[i], ph);
 }
 
+/* ---- one binary colour-matrix expression (first step) -------------------
+ *   dst(x) = opA(A(x)) * opB(B(x + sign*mu)),   op = identity (0) or adjoint (1),   x in subset;
+ * mu = -1: no shift.  A, B, dst are arrays of `na`, `nb`, `nd` matrices per site of which matrix
+ * `ia`, `ib`, `id` takes part (a colour-matrix field has 1, a gauge field 4: "U_mu" is matrix mu).
+ * This is the building block of QDP++ expressions such as  m = u[mu] * shift(u[nu], FORWARD, mu). */
+void orc_matmul(const int *L, double *dst, int nd, int id, const double *A, int na, int ia, int adj_a,
+                const double *B, int nb, int ib, int adj_b, int mu, int sign, int subset) {
+    for (size_t s = 0; s < volume(L); s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        size_t sbn = mu < 0 ? s : hop_lex(L, x, mu, sign);
+        const cplx *a = (const cplx *)A + (s * na + ia) * 9, *b = (const cplx *)B + (sbn * nb + ib) * 9;
+        cplx ta[9], tb[9], r[9];
+        if (adj_a) m_adj(a, ta); else memcpy(ta, a, sizeof ta);
+        if (adj_b) m_adj(b, tb); else memcpy(tb, b, sizeof tb);
+        m_mul(ta, tb, r);
+        memcpy((cplx *)dst + (s * nd + id) * 9, r, sizeof r);
+    }
+}
+
 /* ---- reunitarisation of whole fields (alternative projections) ----------
  * Gram-Schmidt: row0 = v0/|v0|; row1 = v1 - (row0 . v1) row0, normalised, with (a . b) = sum_j conj(a_j) b_j;
  * row2 = conj(row0 x row1).  The result is in SU(3) by construction; unlike Proj it is not gauge
