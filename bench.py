@@ -230,7 +230,8 @@ def run_ours(args) -> dict | None:
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for name, fn in (("smear_hop", lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3)),
                      ("inner_timeslices", lambda: q.qdp_inner_timeslices(psi, chi)),
-                     ("reunitarize_gs", lambda: q.qdp_reunitarize(u2, u, q.QDP_REUNIT_GRAM_SCHMIDT))):
+                     ("reunitarize_gs", lambda: q.qdp_reunitarize(u2, u, q.QDP_REUNIT_GRAM_SCHMIDT)),
+                     ("matmul", lambda: q.qdp_matmul(u2, 0, u, 0, 0, u, 1, 1, 0, 1))):
         for _ in range(3):
             fn()
         ev0.record(stream)
@@ -370,7 +371,12 @@ def run_ours(args) -> dict | None:
                                              "gbs": round(V * 60 * eb / extra_ms["reunitarize_gs"] / 1e6, 1),
                                              "frac": round(V * 60 * eb / extra_ms["reunitarize_gs"] / 1e6 / peak, 4),
                                              "note": "qdp_reunitarize, Gram-Schmidt (row f2): 24 complex read (rows 0, 1 of four "
-                                                     "links; row 2 is not an input) + 36 written per site; not part of the step"}},
+                                                     "links; row 2 is not an input) + 36 written per site; not part of the step"},
+                          "matmul": {"ms": round(extra_ms["matmul"], 5),
+                                     "gbs": round(V * 27 * eb / extra_ms["matmul"] / 1e6, 1),
+                                     "frac": round(V * 27 * eb / extra_ms["matmul"] / 1e6 / peak, 4),
+                                     "note": "qdp_matmul u2[0] = u[0] * adj(u[1])(x+0) (row f1): 2 x 9 complex read + 9 written "
+                                             "per site; not part of the step"}},
             "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
         }
         if world == 1 and not args.no_cpu_baseline:

@@ -171,6 +171,18 @@ int qdp_plaquette(const qdp_field* u, qdp_subset subset, double out[3]);
 int qdp_ape_smear_step(qdp_field* u_out, const qdp_field* u_in, double alpha, int t_dir,
                        qdp_subset subset);
 
+/* SURVEY.md 8(f) row f1, first step -- one fused binary colour-matrix expression, the building
+ * block of QDP++ expressions such as  m = u[mu] * shift(adj(u[nu]), FORWARD, mu):
+ *   dst[slot_d](x) = opA(a[slot_a](x)) * opB(b[slot_b](x + sign*mu)),   x in subset,
+ * op = adjoint if adj_a / adj_b is non-zero, else identity.  mu = 0..3 with sign = +1 | -1
+ * shifts the second operand (def. 1); mu = -1: no shift.  A slot is one 3x3 matrix of a field:
+ * 0 for QDP_COLOR_MATRIX, the link index 0..3 for QDP_GAUGE (QDP_ERR_ARG otherwise; QDP_FERMION
+ * fields are QDP_ERR_KIND).  dst may share a field with an operand, but if mu >= 0 the slot
+ * written must not be the shifted operand's slot of the same field (QDP_ERR_ALIAS).
+ * Asynchronous. */
+int qdp_matmul(qdp_field* dst, int slot_d, const qdp_field* a, int slot_a, int adj_a,
+               const qdp_field* b, int slot_b, int adj_b, int mu, int sign, qdp_subset subset);
+
 /* SURVEY.md 8(f) row f2 (alternative projections) -- every 3x3 matrix of the sites in the subset
  * projected to SU(3):
  *   method QDP_REUNIT_POLAR (0):        Proj of def. 4 (unitary polar factor, determinant phase

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqdp_b200.so")
-SOURCES = ["api.cu", "layout.cu", "shift.cu", "reduce.cu", "hop.cu", "plaquette.cu", "ape.cu", "reunit.cu"]
+SOURCES = ["api.cu", "layout.cu", "shift.cu", "reduce.cu", "hop.cu", "plaquette.cu", "ape.cu", "reunit.cu", "matmul.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xptxas", "-v",

@@ -419,6 +419,29 @@ extern "C" int qdp_ape_smear_step(qdp_field* u_out, const qdp_field* u_in, doubl
     return QDP_OK;
 }
 
+extern "C" int qdp_matmul(qdp_field* dst, int slot_d, const qdp_field* a, int slot_a, int adj_a,
+                          const qdp_field* b, int slot_b, int adj_b, int mu, int sign, qdp_subset subset) {
+    if (!ok_field(dst) || !ok_field(a) || !ok_field(b) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_matmul: bad argument");
+    if (dst->kind == QDP_FERMION || a->kind == QDP_FERMION || b->kind == QDP_FERMION)
+        return fail(QDP_ERR_KIND, "qdp_matmul: operands are colour matrices or links of gauge fields");
+    auto slots = [](const qdp_field* f) { return f->ncomp / 9; };
+    if (slot_d < 0 || slot_d >= slots(dst) || slot_a < 0 || slot_a >= slots(a) || slot_b < 0 || slot_b >= slots(b))
+        return fail(QDP_ERR_ARG, "qdp_matmul: slot out of range");
+    if (mu < -1 || mu > 3 || (mu >= 0 && sign != 1 && sign != -1)) return fail(QDP_ERR_ARG, "qdp_matmul: bad mu / sign");
+    int rc = check_pair("qdp_matmul", dst, a);
+    if (rc == QDP_OK) rc = check_pair("qdp_matmul", dst, b);
+    if (rc != QDP_OK) return rc;
+    if (mu >= 0 && overlaps(dst, b) && (dst->data != b->data || slot_d == slot_b))
+        return fail(QDP_ERR_ALIAS, "qdp_matmul: dst slot aliases the shifted operand");
+    if ((overlaps(dst, a) && dst->data != a->data) || (overlaps(dst, b) && dst->data != b->data))
+        return fail(QDP_ERR_ALIAS, "qdp_matmul: dst partially overlaps an operand");
+    qdp_lattice* l = dst->lat;
+    ENTER(l);
+    CUDA_TRY(launch_matmul(dst->prec, l->geom, dst->data, dst->ncomp, slot_d, a->data, a->ncomp, slot_a, adj_a != 0,
+                           b->data, b->ncomp, slot_b, adj_b != 0, mu, sign, subset, l->stream));
+    return QDP_OK;
+}
+
 extern "C" int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset) {
     if (!ok_field(u_out) || !ok_field(u_in) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_reunitarize: bad argument");
     if (method != QDP_REUNIT_POLAR && method != QDP_REUNIT_GRAM_SCHMIDT)

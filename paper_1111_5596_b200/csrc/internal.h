@@ -49,6 +49,10 @@ cudaError_t launch_hop(int prec, const Geom& g, void* chi, const void* u, const 
 cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb,
                              cudaStream_t st);
 
+// matmul.cu: dst slot id = op(a slot ia)(x) * op(b slot ib)(x + sign*mu); mu < 0: no shift; n* = components per site
+cudaError_t launch_matmul(int prec, const Geom& g, void* dst, int nd, int id, const void* a, int na, int ia, bool adj_a,
+                          const void* b, int nb, int ib, bool adj_b, int mu, int sign, int subset, cudaStream_t st);
+
 // reunit.cu: method 0 = Proj (polar factor, determinant phase removed), 1 = Gram-Schmidt; in place allowed
 cudaError_t launch_reunit(int prec, const Geom& g, int ncomp, void* out, const void* in, int method, int subset,
                           cudaStream_t st);

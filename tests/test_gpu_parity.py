@@ -480,3 +480,53 @@ def test_reunitarize(qdp, lat_cache, dims, prec):
         qdp.qdp_reunitarize(psi, psi, 0)
     with pytest.raises(qdp.QdpError):
         qdp.qdp_reunitarize(qdp.field_from_host(lat, 1, hg), qdp.field_from_host(lat, 1, hg), 2)
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_matmul(qdp, lat_cache, dims, prec):
+    """qdp_matmul (row f1, first step): every operand form vs the oracle, subsets, gauge-field slots,
+    the allowed in-place forms, and the plaquette composed from three products."""
+    lat = lat_cache(dims)
+    P = 1 if prec == "f64" else 0
+    hu = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 71), prec)
+    hm = synth.round_to(synth.color_matrix(dims, _seed(dims) + 72), prec)
+    u, m = qdp.field_from_host(lat, 1, hu), qdp.field_from_host(lat, 0, hm)
+    u64, m64 = _as64(hu), _as64(hm)
+    sentinel = np.full_like(hm, 2.0 + 1.0j)
+    tol = TOL_SITE[prec]
+    for adj_a in (0, 1):
+        for adj_b in (0, 1):
+            for mu, sign in ((-1, 1), (0, 1), (1, -1), (2, 1), (3, -1)):
+                sub = (adj_a + 2 * adj_b + mu) % 3
+                dst = qdp.field_from_host(lat, 0, sentinel)
+                qdp.qdp_matmul(dst, 0, u, 2, adj_a, m, 0, adj_b, mu, sign, sub)
+                want = oracle.matmul(dims, _as64(sentinel), 0, u64, 2, adj_a, m64, 0, adj_b, mu, sign, sub)
+                assert site_rel_err(qdp.field_to_host(dst), want).max() <= tol, (adj_a, adj_b, mu, sign, sub)
+    # into a slot of a gauge field; operands from the same field; unshifted in place
+    g = qdp.field_from_host(lat, 1, hu)
+    qdp.qdp_matmul(g, 3, g, 0, 0, g, 1, 1, 2, 1)                      # u3 = u0 * adj(u1)(x+2)
+    want = oracle.matmul(dims, u64, 3, u64, 0, 0, u64, 1, 1, 2, 1)
+    assert site_rel_err(links(qdp.field_to_host(g)), links(want)).max() <= tol
+    mm = qdp.field_from_host(lat, 0, hm)
+    qdp.qdp_matmul(mm, 0, mm, 0, 1, mm, 0, 0)                          # m = adj(m) * m in place (site-local)
+    want = np.conj(np.swapaxes(m64, 1, 2)) @ m64
+    assert site_rel_err(qdp.field_to_host(mm), want).max() <= tol
+    # plaquette from three generic products + qdp_sum == qdp_plaquette
+    a, b, p = (qdp.qdp_field_alloc(lat, 0, P) for _ in range(3))
+    total = 0.0
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            qdp.qdp_matmul(a, 0, u, mu, 0, u, nu, 0, mu, 1)
+            qdp.qdp_matmul(b, 0, u, nu, 0, u, mu, 0, nu, 1)
+            qdp.qdp_matmul(p, 0, a, 0, 0, b, 0, 1)
+            s = qdp.qdp_sum(p).reshape(3, 3)
+            total += (s[0, 0] + s[1, 1] + s[2, 2]).real
+    assert abs(total / (18 * synth.volume(dims)) - qdp.qdp_plaquette(u)[0]) <= (1e-10 if prec == "f64" else 1e-5)
+    # errors
+    psi = qdp.qdp_field_alloc(lat, 2, P)
+    for args, code in (((a, 1, u, 0, 0, u, 1, 0), -1), ((a, 0, u, 4, 0, u, 1, 0), -1), ((a, 0, psi, 0, 0, u, 1, 0), -3),
+                       ((a, 0, u, 0, 0, a, 0, 0, 1, 1), -6), ((a, 0, u, 0, 0, u, 1, 0, 4, 1), -1)):
+        with pytest.raises(qdp.QdpError) as e:
+            qdp.qdp_matmul(*args)
+        assert e.value.code == code, args
