@@ -66,6 +66,7 @@ def _get():
             "orc_inner": ([P, I, P, P, I, P], None),
             "orc_sum": ([P, I, P, I, P], None),
             "orc_inner_timeslices": ([P, I, P, P, I, P], None),
+            "orc_axpby": ([P, I, D, P, D, P, P, I], None),
             # the same loops over lex sites [begin, end): bounded samples for bench.py
             "orc_shift_bytes_range": ([P, Z, P, P, I, I, I, Z, Z], None),
             "orc_plaquette_range": ([P, P, I, Z, Z, P], None),
@@ -258,6 +259,14 @@ def inner(dims, a, b, subset=ALL):
     _get().orc_inner(_dims(dims), _reals(dims, a), a.ctypes.data, b.ctypes.data, subset,
                      out.ctypes.data)
     return complex(out[0], out[1])
+
+
+def axpby(dims, a, x, b, y, subset=ALL, dst=None):
+    """dst = a x + b y on the subset (real a, b; any kind)."""
+    x, y = _c128(x), _c128(y)
+    out = np.zeros_like(x) if dst is None else _c128(dst).copy()
+    _get().orc_axpby(_dims(dims), _reals(dims, x), a, x.ctypes.data, b, y.ctypes.data, out.ctypes.data, subset)
+    return out
 
 
 def inner_timeslices(dims, a, b, subset=ALL):

@@ -543,6 +543,18 @@ void orc_inner(const int *L, int reals, const double *a, const double *b, int su
     orc_inner_range(L, reals, a, b, subset, 0, volume(L), out2);
 }
 
+/* dst = a x + b y on the subset, real a, b, any field kind (reals = 2 * complex components per
+ * site): the "residual calculation and solution reconstruction" expressions of PAPER.md:96
+ * (r = b - A x, x += alpha p ...).  Two roundings per term, like a*psi + b*hop in definition 6. */
+void orc_axpby(const int *L, int reals, double a, const double *x, double b, const double *y,
+               double *dst, int subset) {
+    for (size_t s = 0; s < volume(L); s++) {
+        int c[4]; coords_of(L, s, c);
+        if (!in_subset(c, subset)) continue;
+        for (int i = 0; i < reals; i++) dst[s * reals + i] = a * x[s * reals + i] + b * y[s * reals + i];
+    }
+}
+
 /* time-slice sums, the reduction under every hadron two-point function
  * (HAD stage):
  *   out[t] = sum_{x in subset, x3 = t} sum_c conj(a_c(x)) b_c(x),   t = 0 .. L3-1   (re, im pairs).
