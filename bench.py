@@ -231,7 +231,8 @@ def run_ours(args) -> dict | None:
     for name, fn in (("smear_hop", lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3)),
                      ("inner_timeslices", lambda: q.qdp_inner_timeslices(psi, chi)),
                      ("reunitarize_gs", lambda: q.qdp_reunitarize(u2, u, q.QDP_REUNIT_GRAM_SCHMIDT)),
-                     ("matmul", lambda: q.qdp_matmul(u2, 0, u, 0, 0, u, 1, 1, 0, 1))):
+                     ("matmul", lambda: q.qdp_matmul(u2, 0, u, 0, 0, u, 1, 1, 0, 1)),
+                     ("axpby", lambda: q.qdp_axpby(sh, a, psi, b, chi))):
         for _ in range(3):
             fn()
         ev0.record(stream)
@@ -376,7 +377,12 @@ def run_ours(args) -> dict | None:
                                      "gbs": round(V * 27 * eb / extra_ms["matmul"] / 1e6, 1),
                                      "frac": round(V * 27 * eb / extra_ms["matmul"] / 1e6 / peak, 4),
                                      "note": "qdp_matmul u2[0] = u[0] * adj(u[1])(x+0) (row f1): 2 x 9 complex read + 9 written "
-                                             "per site; not part of the step"}},
+                                             "per site; not part of the step"},
+                          "axpby": {"ms": round(extra_ms["axpby"], 5),
+                                    "gbs": round(V * 36 * eb / extra_ms["axpby"] / 1e6, 1),
+                                    "frac": round(V * 36 * eb / extra_ms["axpby"] / 1e6 / peak, 4),
+                                    "note": "qdp_axpby on spinors (PAPER.md:96): 2 x 12 complex read + 12 written per site; "
+                                            "not part of the step"}},
             "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
         }
         if world == 1 and not args.no_cpu_baseline:

@@ -225,6 +225,14 @@ int qdp_norm2(const qdp_field* f, qdp_subset subset, double* out);
 int qdp_inner(const qdp_field* a, const qdp_field* b, qdp_subset subset, double out[2]);
 int qdp_sum(const qdp_field* f, qdp_subset subset, double* out);
 
+/* dst = a*x + b*y on the subset, real a, b cast to the field precision, any kind (all three
+ * fields of the same kind and precision): the residual and solution-reconstruction expressions
+ * around the solver (r = b - A x, x += alpha p).  Element-wise, so dst may be x or y.
+ * If norm2_out is not NULL it receives sum_{x in subset} |dst(x)|^2 accumulated in the same pass
+ * (fp64) and the call is synchronous; otherwise asynchronous. */
+int qdp_axpby(qdp_field* dst, double a, const qdp_field* x, double b, const qdp_field* y,
+              qdp_subset subset, double* norm2_out);
+
 /* time-slice sums, the reduction under every hadron two-point function
  * (the HAD stage of the paper's Fig. 4):
  *   out[2t], out[2t+1] = (re, im) of sum_{x in subset, x3 = t} sum_c conj(a_c(x)) b_c(x),  t < L3.

@@ -18,7 +18,7 @@ __all__ = [
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
-    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_reunitarize", "qdp_matmul", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
+    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_reunitarize", "qdp_matmul", "qdp_axpby", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
 ]
@@ -67,6 +67,7 @@ DECLARED_SYMBOLS = {
     "qdp_smear_hop": ([_P, _D, _D, _P, _P, _I, _I, _P], _I),
     "qdp_inner_timeslices": ([_P, _P, _I, _P], _I),
     "qdp_reunitarize": ([_P, _P, _I, _I], _I),
+    "qdp_axpby": ([_P, _D, _P, _D, _P, _I, _P], _I),
     "qdp_matmul": ([_P, _I, _P, _I, _I, _P, _I, _I, _I, _I, _I], _I),
     "qdp_norm2": ([_P, _I, _P], _I),
     "qdp_inner": ([_P, _P, _I, _P], _I),
@@ -296,6 +297,13 @@ def qdp_smear_hop(chi: Field, a: float, b: float, u: Field, psi: Field, t_dir: i
     out = ctypes.c_double()
     _check(_lib.qdp_smear_hop(chi.handle, float(a), float(b), u.handle, psi.handle, int(t_dir), subset,
                               ctypes.addressof(out) if want_norm2 else None))
+    return out.value if want_norm2 else None
+
+
+def qdp_axpby(dst: Field, a: float, x: Field, b: float, y: Field, subset: int = QDP_ALL, want_norm2: bool = False):
+    out = ctypes.c_double()
+    _check(_lib.qdp_axpby(dst.handle, float(a), x.handle, float(b), y.handle, subset,
+                          ctypes.addressof(out) if want_norm2 else None))
     return out.value if want_norm2 else None
 
 

@@ -507,6 +507,23 @@ extern "C" int qdp_inner(const qdp_field* a, const qdp_field* b, qdp_subset subs
     return fetch_result(l, 2, out);
 }
 
+extern "C" int qdp_axpby(qdp_field* dst, double a, const qdp_field* x, double b, const qdp_field* y,
+                         qdp_subset subset, double* norm2_out) {
+    if (!ok_field(dst) || !ok_field(x) || !ok_field(y) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_axpby: bad argument");
+    int rc = check_pair("qdp_axpby", dst, x);
+    if (rc == QDP_OK) rc = check_pair("qdp_axpby", dst, y);
+    if (rc != QDP_OK) return rc;
+    if (dst->kind != x->kind || dst->kind != y->kind) return fail(QDP_ERR_KIND, "qdp_axpby: kinds differ");
+    if ((overlaps(dst, x) && dst->data != x->data) || (overlaps(dst, y) && dst->data != y->data))
+        return fail(QDP_ERR_ALIAS, "qdp_axpby: dst partially overlaps an operand");
+    qdp_lattice* l = dst->lat;
+    ENTER(l);
+    CUDA_TRY(launch_axpby(dst->prec, l->geom, dst->ncomp, dst->data, x->data, y->data, a, b, subset,
+                          norm2_out != nullptr, reduce_buf(l), l->stream));
+    if (norm2_out) return fetch_result(l, 1, norm2_out);
+    return QDP_OK;
+}
+
 extern "C" int qdp_inner_timeslices(const qdp_field* a, const qdp_field* b, qdp_subset subset, double* out) {
     if (!ok_field(a) || !ok_field(b) || !out || !ok_subset(subset))
         return fail(QDP_ERR_ARG, "qdp_inner_timeslices: bad argument");

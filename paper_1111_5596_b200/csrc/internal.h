@@ -35,6 +35,9 @@ cudaError_t launch_inner(int prec, const Geom& g, int ncomp, const void* a, cons
 cudaError_t launch_sum(int prec, const Geom& g, int ncomp, const void* f, int subset,
                        double* partials, double* out_dev, cudaStream_t st);
 
+// dst = a x + b y on the subset (dst may be x or y); want_norm2: norm2(dst) through rb
+cudaError_t launch_axpby(int prec, const Geom& g, int ncomp, void* dst, const void* x, const void* y, double a,
+                         double b, int subset, bool want_norm2, const ReduceBuf& rb, cudaStream_t st);
 // partials: scratch of 2*16*L3 doubles; out_dev: 2*L3 doubles on the device
 cudaError_t launch_inner_timeslices(int prec, const Geom& g, int ncomp, const void* a, const void* b, int subset,
                                     double* partials, double* out_dev, cudaStream_t st);

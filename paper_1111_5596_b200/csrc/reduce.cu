@@ -167,6 +167,59 @@ __global__ void sum_finish_kernel(int nblk, const double* __restrict__ partials,
     out[c * 2 + k] = t;
 }
 
+// ---- dst = a x + b y (+ fused norm2 of dst) -------------------------------------------------
+// The residual / solution-reconstruction expressions of PAPER.md:96.  Element-wise on the
+// contiguous range of the subset; dst may be x or y.  Padding lanes of a ragged lattice are
+// written too (nothing reads them as sites) but masked out of the norm.
+// a*x + b*y with the three roundings of the definition (no contraction into an fma), so that fp64
+// results equal the oracle's bit for bit
+__device__ __forceinline__ double axpby1(double a, double x, double b, double y) { return __dadd_rn(__dmul_rn(a, x), __dmul_rn(b, y)); }
+__device__ __forceinline__ float axpby1(float a, float x, float b, float y) { return __fadd_rn(__fmul_rn(a, x), __fmul_rn(b, y)); }
+
+template <class T2, bool NORM>
+__global__ void __launch_bounds__(kReduceThreads) axpby_kernel(Geom g, int ncomp, T2* dst, const T2* x, const T2* y,
+                                                              double a, double b, int subset, ReduceBuf rb) {
+    using R = decltype(T2::x);
+    const unsigned half = (unsigned)g.Vhp * ncomp;
+    const unsigned begin = subset == 2 ? half : 0u, n = subset == 0 ? 2u * half : half;
+    const bool ragged = g.Vh != g.Vhp;
+    const R ra = (R)a, rb_ = (R)b;
+    const unsigned stride = gridDim.x * kReduceThreads;
+    double acc[1] = {0.0};
+#pragma unroll 4
+    for (unsigned e = blockIdx.x * kReduceThreads + threadIdx.x; e < n; e += stride) {
+        const T2 vx = x[begin + e], vy = y[begin + e];
+        T2 r;
+        r.x = axpby1(ra, vx.x, rb_, vy.x);
+        r.y = axpby1(ra, vx.y, rb_, vy.y);
+        dst[begin + e] = r;
+        if (NORM) {
+            bool real = true;
+            if (ragged) {
+                const unsigned eh = begin + e >= half ? begin + e - half : begin + e;
+                real = (eh / (ncomp * 32u)) * 32u + (eh & 31u) < (unsigned)g.Vh;
+            }
+            if (real) acc[0] += (double)r.x * (double)r.x + (double)r.y * (double)r.y;
+        }
+    }
+    if (NORM) grid_reduce<1>(acc, rb, nullptr);
+}
+
+cudaError_t launch_axpby(int prec, const Geom& g, int ncomp, void* dst, const void* x, const void* y, double a,
+                         double b, int subset, bool want_norm2, const ReduceBuf& rb, cudaStream_t st) {
+    const size_t n = (size_t)g.Vhp * ncomp * (subset == 0 ? 2 : 1);
+    const int grid = stream_grid(n);
+    if (prec) {
+        if (want_norm2) axpby_kernel<double2, true><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (double2*)dst, (const double2*)x, (const double2*)y, a, b, subset, rb);
+        else            axpby_kernel<double2, false><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (double2*)dst, (const double2*)x, (const double2*)y, a, b, subset, rb);
+    } else {
+        if (want_norm2) axpby_kernel<float2, true><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (float2*)dst, (const float2*)x, (const float2*)y, a, b, subset, rb);
+        else            axpby_kernel<float2, false><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (float2*)dst, (const float2*)x, (const float2*)y, a, b, subset, rb);
+    }
+    g_launch_count++;
+    return cudaGetLastError();
+}
+
 // ---- time-slice inner products -----------------------------------
 // out[t] = sum over the sites with x3 = t of conj(a) . b.  In the blocked layout the half-indices of
 // a time-slice are one run [t*s3, (t+1)*s3) per parity half, so when s3 is a multiple of 32 a slice

@@ -530,3 +530,38 @@ def test_matmul(qdp, lat_cache, dims, prec):
         with pytest.raises(qdp.QdpError) as e:
             qdp.qdp_matmul(*args)
         assert e.value.code == code, args
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+@pytest.mark.parametrize("kind", ["fermion", "gauge"])
+def test_axpby(qdp, lat_cache, dims, prec, kind):
+    """qdp_axpby: dst = a x + b y on every subset, with and without the fused norm2, in place."""
+    lat = lat_cache(dims)
+    hx = synth.round_to(_field(dims, kind, _seed(dims) + 81), prec)
+    hy = synth.round_to(_field(dims, kind, _seed(dims) + 82) if kind != "fermion" else synth.spinor(dims, _seed(dims) + 82, 1), prec)
+    x, y = qdp.field_from_host(lat, KINDS[kind], hx), qdp.field_from_host(lat, KINDS[kind], hy)
+    a, b = synth.scalars_ab(_seed(dims) + 8)
+    if prec == "f32":
+        a, b = float(np.float32(a)), float(np.float32(b))
+    sentinel = np.full_like(hx, 1.5 - 0.5j)
+    for sub in SUBSETS:
+        dst = qdp.field_from_host(lat, KINDS[kind], sentinel)
+        n2 = qdp.qdp_axpby(dst, a, x, b, y, sub, want_norm2=True)
+        got = qdp.field_to_host(dst)
+        want = oracle.axpby(dims, a, _as64(hx), b, _as64(hy), sub, dst=_as64(sentinel))
+        if prec == "f64":
+            assert np.array_equal(got, want), sub            # same two roundings per term
+        else:
+            assert site_rel_err(got, want).max() <= TOL_SITE[prec], sub
+        assert abs(n2 - oracle.norm2(dims, want if prec == "f64" else _as64(got), sub)) <= 1e-10 * n2
+        dst2 = qdp.field_from_host(lat, KINDS[kind], sentinel)
+        qdp.qdp_axpby(dst2, a, x, b, y, sub)
+        assert np.array_equal(qdp.field_to_host(dst2), got)
+    work = qdp.field_from_host(lat, KINDS[kind], hx)                 # x <- a x + b y in place
+    qdp.qdp_axpby(work, a, work, b, y)
+    full = qdp.field_from_host(lat, KINDS[kind], sentinel)
+    qdp.qdp_axpby(full, a, x, b, y)
+    assert np.array_equal(qdp.field_to_host(work), qdp.field_to_host(full))
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_axpby(work, a, x, b, qdp.qdp_field_alloc(lat, 0, 1 if prec == "f64" else 0))
