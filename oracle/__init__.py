@@ -51,6 +51,7 @@ def _get():
             "orc_proj_su3": ([P, P], None),
             "orc_min_eig_vdv": ([P], D),
             "orc_gram_schmidt_su3": ([P, P], None),
+            "orc_matvec": ([P, P, P, I, I, I, P, I, I, I], None),
             "orc_matmul": ([P, P, I, I, P, I, I, I, P, I, I, I, I, I, I], None),
             "orc_reunitarize": ([P, I, P, P, I, I], None),
             "orc_staple_site": ([P, P, Z, I, I, P], I),
@@ -153,6 +154,15 @@ def matmul(dims, dst, id_, a, ia, adj_a, b, ib, adj_b, mu=-1, sign=1, subset=ALL
     V = volume(dims)
     _get().orc_matmul(_dims(dims), out.ctypes.data, out.size // (9 * V), id_, a.ctypes.data, a.size // (9 * V), ia,
                       int(adj_a), b.ctypes.data, b.size // (9 * V), ib, int(adj_b), mu, sign, subset)
+    return out
+
+
+def matvec(dims, a, ia, adj_a, psi, mu=-1, sign=1, subset=ALL, chi=None):
+    """chi(x) = op(a[:, ia])(x) psi(x + sign*mu) on the subset (row f1); a is [V,3,3] or [V,4,3,3]."""
+    a, psi = _c128(a), _c128(psi)
+    out = np.zeros_like(psi) if chi is None else _c128(chi).copy()
+    _get().orc_matvec(_dims(dims), out.ctypes.data, a.ctypes.data, a.size // (9 * volume(dims)), ia, int(adj_a),
+                      psi.ctypes.data, mu, sign, subset)
     return out
 
 

@@ -305,6 +305,28 @@ void orc_matmul(const int *L, double *dst, int nd, int id, const double *A, int 
     }
 }
 
+/* chi(x) = opA(A(x)) psi(x + sign*mu) on the subset: colour matrix (slot ia of na per site) times
+ * the colour index of every spin component of a fermion; op = identity or adjoint; mu = -1: no shift.
+ * ("colour-matrix x fermion on arbitrary fields, shift of leaves".) */
+void orc_matvec(const int *L, double *chi, const double *A, int na, int ia, int adj_a, const double *psi,
+                int mu, int sign, int subset) {
+    for (size_t s = 0; s < volume(L); s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        size_t sn = mu < 0 ? s : hop_lex(L, x, mu, sign);
+        const cplx *a = (const cplx *)A + (s * na + ia) * 9, *p = (const cplx *)psi + sn * 12;
+        cplx ta[9], r[12];
+        if (adj_a) m_adj(a, ta); else memcpy(ta, a, sizeof ta);
+        for (int sp = 0; sp < 4; sp++)
+            for (int i = 0; i < 3; i++) {
+                cplx acc = { 0, 0 };
+                for (int j = 0; j < 3; j++) acc = c_add(acc, c_mul(ta[i * 3 + j], p[sp * 3 + j]));
+                r[sp * 3 + i] = acc;
+            }
+        memcpy((cplx *)chi + s * 12, r, sizeof r);
+    }
+}
+
 /* ---- reunitarisation of whole fields (alternative projections) ----------
  * Gram-Schmidt: row0 = v0/|v0|; row1 = v1 - (row0 . v1) row0, normalised, with (a . b) = sum_j conj(a_j) b_j;
  * row2 = conj(row0 x row1).  The result is in SU(3) by construction; unlike Proj it is not gauge

@@ -56,3 +56,26 @@ def test_unitarity_adjoint_rule_subsets_and_gauge_slots():
     out = oracle.matmul(dims, sentinel, 3, m, 0, 0, n, 0, 0, -1, 1, 2)       # into link 3 of a gauge field, odd sites
     assert np.all(out[:, :3] == 5.0) and np.all(out[~odd, 3] == 5.0)
     assert np.abs(out[odd, 3] - (m @ n)[odd]).max() < 1e-13
+
+
+def test_matvec_brute_force_and_hop_composed_from_it():
+    """matvec against numpy einsum for every operand form, and the hop term (def. 5) rebuilt from
+    eight matvecs: chi = sum_mu [U_mu(x) psi(x+mu) + shift(adj(U_mu) psi, -mu)]."""
+    dims = (4, 2, 6, 4)
+    u, m, psi = synth.gauge_hot(dims, 511), synth.color_matrix(dims, 512), synth.spinor(dims, 513)
+    for adj_a in (0, 1):
+        for mu, sign in ((-1, 1), (0, 1), (2, -1), (3, 1)):
+            A = dag(m) if adj_a else m
+            p = psi if mu < 0 else sh(dims, psi, mu, sign)
+            want = np.einsum("xab,xsb->xsa", A, p)
+            assert np.abs(oracle.matvec(dims, m, 0, adj_a, psi, mu, sign) - want).max() < 1e-13
+    chi = np.zeros_like(psi)
+    for mu in range(4):
+        chi += oracle.matvec(dims, u, mu, 0, psi, mu, +1)
+        back = oracle.matvec(dims, u, mu, 1, psi)                       # U_mu(y)^dag psi(y) at y
+        chi += oracle.shift(dims, back, mu, -1)
+    assert np.abs(chi - oracle.hop(dims, u, psi)).max() < 1e-13
+    odd = parity(dims) == 1
+    sentinel = np.full_like(psi, 4.0)
+    out = oracle.matvec(dims, u, 1, 0, psi, 1, 1, 1, chi=sentinel)
+    assert np.all(out[odd] == 4.0) and np.abs(out[~odd] - np.einsum("xab,xsb->xsa", u[:, 1], sh(dims, psi, 1, 1))[~odd]).max() < 1e-13
