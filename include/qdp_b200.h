@@ -183,6 +183,13 @@ int qdp_ape_smear_step(qdp_field* u_out, const qdp_field* u_in, double alpha, in
 int qdp_matmul(qdp_field* dst, int slot_d, const qdp_field* a, int slot_a, int adj_a,
                const qdp_field* b, int slot_b, int adj_b, int mu, int sign, qdp_subset subset);
 
+/* Row f1, colour matrix times fermion:  chi(x) = opA(a[slot_a](x)) psi(x + sign*mu),  x in subset;
+ * the matrix acts on the colour index of each spin component.  Slots, adj_a, mu, sign as in
+ * qdp_matmul.  chi, psi: QDP_FERMION; chi == psi is allowed only without a shift (mu = -1),
+ * otherwise QDP_ERR_ALIAS.  Asynchronous. */
+int qdp_matvec(qdp_field* chi, const qdp_field* a, int slot_a, int adj_a, const qdp_field* psi,
+               int mu, int sign, qdp_subset subset);
+
 /* SURVEY.md 8(f) row f2 (alternative projections) -- every 3x3 matrix of the sites in the subset
  * projected to SU(3):
  *   method QDP_REUNIT_POLAR (0):        Proj of def. 4 (unitary polar factor, determinant phase

@@ -18,7 +18,7 @@ __all__ = [
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
-    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_reunitarize", "qdp_matmul", "qdp_axpby", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
+    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_reunitarize", "qdp_matmul", "qdp_matvec", "qdp_axpby", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
 ]
@@ -68,6 +68,7 @@ DECLARED_SYMBOLS = {
     "qdp_inner_timeslices": ([_P, _P, _I, _P], _I),
     "qdp_reunitarize": ([_P, _P, _I, _I], _I),
     "qdp_axpby": ([_P, _D, _P, _D, _P, _I, _P], _I),
+    "qdp_matvec": ([_P, _P, _I, _I, _P, _I, _I, _I], _I),
     "qdp_matmul": ([_P, _I, _P, _I, _I, _P, _I, _I, _I, _I, _I], _I),
     "qdp_norm2": ([_P, _I, _P], _I),
     "qdp_inner": ([_P, _P, _I, _P], _I),
@@ -265,6 +266,12 @@ def qdp_ape_smear_step(u_out: Field, u_in: Field, alpha: float, t_dir: int = 3, 
 
 
 QDP_REUNIT_POLAR, QDP_REUNIT_GRAM_SCHMIDT = 0, 1
+
+
+def qdp_matvec(chi: Field, a: Field, slot_a: int, adj_a: bool, psi: Field, mu: int = -1, sign: int = 1,
+               subset: int = QDP_ALL) -> None:
+    """chi(x) = op(a[slot_a])(x) psi(x + sign*mu); mu = -1: no shift."""
+    _check(_lib.qdp_matvec(chi.handle, a.handle, slot_a, int(bool(adj_a)), psi.handle, mu, sign, subset))
 
 
 def qdp_matmul(dst: Field, slot_d: int, a: Field, slot_a: int, adj_a: bool, b: Field, slot_b: int, adj_b: bool,

@@ -442,6 +442,25 @@ extern "C" int qdp_matmul(qdp_field* dst, int slot_d, const qdp_field* a, int sl
     return QDP_OK;
 }
 
+extern "C" int qdp_matvec(qdp_field* chi, const qdp_field* a, int slot_a, int adj_a, const qdp_field* psi,
+                          int mu, int sign, qdp_subset subset) {
+    if (!ok_field(chi) || !ok_field(a) || !ok_field(psi) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_matvec: bad argument");
+    if (chi->kind != QDP_FERMION || psi->kind != QDP_FERMION || a->kind == QDP_FERMION)
+        return fail(QDP_ERR_KIND, "qdp_matvec: need (fermion, colour matrix or gauge, fermion)");
+    if (slot_a < 0 || slot_a >= a->ncomp / 9) return fail(QDP_ERR_ARG, "qdp_matvec: slot out of range");
+    if (mu < -1 || mu > 3 || (mu >= 0 && sign != 1 && sign != -1)) return fail(QDP_ERR_ARG, "qdp_matvec: bad mu / sign");
+    int rc = check_pair("qdp_matvec", chi, psi);
+    if (rc == QDP_OK) rc = check_pair("qdp_matvec", chi, a);
+    if (rc != QDP_OK) return rc;
+    if (overlaps(chi, psi) && (mu >= 0 || chi->data != psi->data))
+        return fail(QDP_ERR_ALIAS, "qdp_matvec: chi aliases the shifted psi");
+    qdp_lattice* l = chi->lat;
+    ENTER(l);
+    CUDA_TRY(launch_matvec(chi->prec, l->geom, chi->data, a->data, a->ncomp, slot_a, adj_a != 0, psi->data, mu, sign,
+                           subset, l->stream));
+    return QDP_OK;
+}
+
 extern "C" int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset) {
     if (!ok_field(u_out) || !ok_field(u_in) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_reunitarize: bad argument");
     if (method != QDP_REUNIT_POLAR && method != QDP_REUNIT_GRAM_SCHMIDT)

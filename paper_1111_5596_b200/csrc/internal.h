@@ -56,6 +56,10 @@ cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset,
 cudaError_t launch_matmul(int prec, const Geom& g, void* dst, int nd, int id, const void* a, int na, int ia, bool adj_a,
                           const void* b, int nb, int ib, bool adj_b, int mu, int sign, int subset, cudaStream_t st);
 
+// chi(x) = op(a slot ia)(x) psi(x + sign*mu); mu < 0: no shift
+cudaError_t launch_matvec(int prec, const Geom& g, void* chi, const void* a, int na, int ia, bool adj_a, const void* psi,
+                          int mu, int sign, int subset, cudaStream_t st);
+
 // reunit.cu: method 0 = Proj (polar factor, determinant phase removed), 1 = Gram-Schmidt; in place allowed
 cudaError_t launch_reunit(int prec, const Geom& g, int ncomp, void* out, const void* in, int method, int subset,
                           cudaStream_t st);

@@ -47,6 +47,55 @@ __global__ void __launch_bounds__(256) matmul_kernel(Geom g, typename Vec2<T>::t
     st_mat_at<T>(site_ptr(dst, nd, id * 9, s), R);
 }
 
+// chi(x) = opA(A(x)) psi(x + sign*mu): the colour matrix acts on the colour index of each of the four
+// spin components.  chi must not be psi when mu >= 0 (checked by the caller).
+template <class T, bool ADJ_A>
+__global__ void __launch_bounds__(256) matvec_kernel(Geom g, typename Vec2<T>::type* chi,
+                                                    const typename Vec2<T>::type* a, int na, int ia,
+                                                    const typename Vec2<T>::type* psi, int mu, int sign, int subset) {
+    using T2 = typename Vec2<T>::type;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= subset_count(g, subset)) return;
+    const Site x = subset_site(g, subset, i);
+    const int s = x.index(g);
+    const int sn = mu < 0 ? s : site_step_rt(g, x, mu, sign).index(g);
+    const T2* pa = site_ptr(a, na, ia * 9, s);
+    const T2* pp = site_ptr(psi, 12, 0, sn);
+    Mat3<T> A;
+    Spinor<T> p, r;
+#pragma unroll
+    for (int c = 0; c < 9; c++) { const T2 v = pa[c * kLane]; A.e[c] = cx<T>(v.x, v.y); }
+#pragma unroll
+    for (int c = 0; c < 12; c++) { const T2 v = pp[c * kLane]; p.e[c] = cx<T>(v.x, v.y); }
+#pragma unroll
+    for (int sp = 0; sp < 4; sp++)
+#pragma unroll
+        for (int r_ = 0; r_ < 3; r_++) {
+            Cx<T> acc = cx<T>(0, 0);
+#pragma unroll
+            for (int k = 0; k < 3; k++) cmad(acc, ADJ_A ? conj(A.e[k * 3 + r_]) : A.e[r_ * 3 + k], p.e[sp * 3 + k]);
+            r.e[sp * 3 + r_] = acc;
+        }
+    T2* o = site_ptr(chi, 12, 0, s);
+#pragma unroll
+    for (int c = 0; c < 12; c++) { T2 v; v.x = r.e[c].re; v.y = r.e[c].im; o[c * kLane] = v; }
+}
+
+cudaError_t launch_matvec(int prec, const Geom& g, void* chi, const void* a, int na, int ia, bool adj_a, const void* psi,
+                          int mu, int sign, int subset, cudaStream_t st) {
+    const int n = subset == 0 ? g.V : g.Vh;
+    const int grid = (n + 255) / 256;
+    if (prec) {
+        if (adj_a) matvec_kernel<double, true><<<grid, 256, 0, st>>>(g, (double2*)chi, (const double2*)a, na, ia, (const double2*)psi, mu, sign, subset);
+        else       matvec_kernel<double, false><<<grid, 256, 0, st>>>(g, (double2*)chi, (const double2*)a, na, ia, (const double2*)psi, mu, sign, subset);
+    } else {
+        if (adj_a) matvec_kernel<float, true><<<grid, 256, 0, st>>>(g, (float2*)chi, (const float2*)a, na, ia, (const float2*)psi, mu, sign, subset);
+        else       matvec_kernel<float, false><<<grid, 256, 0, st>>>(g, (float2*)chi, (const float2*)a, na, ia, (const float2*)psi, mu, sign, subset);
+    }
+    g_launch_count++;
+    return cudaGetLastError();
+}
+
 template <class T>
 static void matmul_dispatch(const Geom& g, void* dst, int nd, int id, const void* a, int na, int ia, bool adj_a,
                             const void* b, int nb, int ib, bool adj_b, int mu, int sign, int subset, cudaStream_t st) {

@@ -565,3 +565,40 @@ def test_axpby(qdp, lat_cache, dims, prec, kind):
     assert np.array_equal(qdp.field_to_host(work), qdp.field_to_host(full))
     with pytest.raises(qdp.QdpError):
         qdp.qdp_axpby(work, a, x, b, qdp.qdp_field_alloc(lat, 0, 1 if prec == "f64" else 0))
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_matvec_and_hop_composed_from_generic_ops(qdp, lat_cache, dims, prec):
+    """qdp_matvec vs the oracle in every operand form, and the hop term rebuilt from generic calls
+    (8 matvecs, 4 shifts, 8 axpbys) against the fused qdp_hop."""
+    lat = lat_cache(dims)
+    P = 1 if prec == "f64" else 0
+    hu = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 91), prec)
+    hm = synth.round_to(synth.color_matrix(dims, _seed(dims) + 92), prec)
+    hp = synth.round_to(synth.spinor(dims, _seed(dims) + 93), prec)
+    u, m, psi = qdp.field_from_host(lat, 1, hu), qdp.field_from_host(lat, 0, hm), qdp.field_from_host(lat, 2, hp)
+    sentinel = np.full_like(hp, -1.0 + 2.0j)
+    for adj_a in (0, 1):
+        for mu, sign in ((-1, 1), (0, -1), (1, 1), (2, -1), (3, 1)):
+            sub = (adj_a + mu + 1) % 3
+            chi = qdp.field_from_host(lat, 2, sentinel)
+            qdp.qdp_matvec(chi, m, 0, adj_a, psi, mu, sign, sub)
+            want = oracle.matvec(dims, _as64(hm), 0, adj_a, _as64(hp), mu, sign, sub, chi=_as64(sentinel))
+            assert site_rel_err(qdp.field_to_host(chi), want).max() <= TOL_SITE[prec], (adj_a, mu, sign, sub)
+    acc, t, t2 = (qdp.field_from_host(lat, 2, np.zeros_like(hp)) for _ in range(3))
+    for mu in range(4):
+        qdp.qdp_matvec(t, u, mu, 0, psi, mu, 1)                    # U_mu(x) psi(x+mu)
+        qdp.qdp_axpby(acc, 1.0, acc, 1.0, t)
+        qdp.qdp_matvec(t, u, mu, 1, psi)                           # U_mu(y)^dag psi(y)
+        qdp.qdp_shift(t2, t, mu, -1)                               # ... moved to y + mu
+        qdp.qdp_axpby(acc, 1.0, acc, 1.0, t2)
+    fused = qdp.qdp_field_alloc(lat, 2, P)
+    qdp.qdp_hop(fused, u, psi)
+    assert site_rel_err(qdp.field_to_host(acc), _as64(qdp.field_to_host(fused))).max() <= 8 * TOL_SITE[prec]
+    inplace = qdp.field_from_host(lat, 2, hp)
+    qdp.qdp_matvec(inplace, u, 2, 1, inplace)                      # site-local: in place allowed
+    assert site_rel_err(qdp.field_to_host(inplace), oracle.matvec(dims, _as64(hu), 2, 1, _as64(hp))).max() <= TOL_SITE[prec]
+    with pytest.raises(qdp.QdpError) as e:
+        qdp.qdp_matvec(inplace, u, 2, 1, inplace, 0, 1)
+    assert e.value.code == -6
