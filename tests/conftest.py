@@ -15,5 +15,8 @@ def pytest_configure(config):
 @pytest.fixture(scope="session")
 def qdp():
     """The CUDA path's Python binding; only -m gpu tests and the symbol test use it."""
+    from paper_1111_5596_b200.build import LIB, build
+    if not os.path.exists(LIB):      # fresh checkout: the .so is a build artefact, not in the history
+        build()
     import paper_1111_5596_b200 as q
     return q
