@@ -153,6 +153,9 @@ def whole_job_value(units_per_rank: int, world: int, ms: float) -> float:
 def run_ours(args) -> dict | None:
     import torch
     import synth
+    from paper_1111_5596_b200.build import LIB, build as build_cuda
+    if not os.path.exists(LIB) and int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        build_cuda()                 # fresh checkout: compile the library (no fallback: without it nothing runs)
     import paper_1111_5596_b200 as q
 
     rank, world, local = rank_env()
