@@ -124,6 +124,21 @@ struct DeviceGuard {
     if (!guard_.ok) return fail(QDP_ERR_CUDA, "cannot select CUDA device %d", (lat)->device)
 
 // ---- lattice -------------------------------------------------------------------
+// frees whatever a (possibly half-constructed) lattice owns, then the handle itself
+static void release_lattice(qdp_lattice* l) {
+    dev_free(l->partials, l->scratch_from_hook);
+    dev_free(l->counter, l->scratch_from_hook);
+    if (l->result_host) cudaFreeHost(l->result_host);
+    for (int i = 0; i < 2; i++) {
+        dev_free(l->stage[i], l->scratch_from_hook);
+        if (l->ev_copied[i]) cudaEventDestroy(l->ev_copied[i]);
+        if (l->ev_done[i]) cudaEventDestroy(l->ev_done[i]);
+    }
+    if (l->copy_stream) cudaStreamDestroy(l->copy_stream);
+    l->magic = 0;
+    delete l;
+}
+
 extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** out) {
     if (!dims || !out) return fail(QDP_ERR_ARG, "qdp_lattice_create: null argument");
     long long V = 1;
@@ -143,7 +158,8 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     l->device = device;
     memcpy(l->dims, dims, sizeof l->dims);
     l->geom = Geom::make(dims);
-    ENTER(l);
+    DeviceGuard guard_(device);
+    if (!guard_.ok) { delete l; return fail(QDP_ERR_CUDA, "cannot select CUDA device %d", device); }
     l->scratch_from_hook = g_alloc != nullptr;
     // partials: K <= 4 values per block (streaming reductions: at most kMaxPartialBlocks) or per
     // warp of 32 sites plus per group of kWarpGroup warps (fused kernels, reduce.cuh); qdp_sum
@@ -154,22 +170,28 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     if (npart < (size_t)2 * 36 * 64) npart = (size_t)2 * 36 * 64;
     if (npart < (size_t)34 * dims[3]) npart = (size_t)34 * dims[3];   // qdp_inner_timeslices: 2*16*L3 partials + 2*L3 results
     const size_t counter_bytes = (ngroup_max + 1) * sizeof(unsigned int);
-    int rc;
-    void* p = nullptr;
-    if ((rc = dev_alloc(npart * sizeof(double), &p)) != QDP_OK) { delete l; return rc; }
-    l->partials = (double*)p;
-    if ((rc = dev_alloc(counter_bytes, &p)) != QDP_OK) { delete l; return rc; }
-    l->counter = (unsigned int*)p;
-    CUDA_TRY(cudaMemset(l->counter, 0, counter_bytes));
-    CUDA_TRY(cudaHostAlloc((void**)&l->result_host, 72 * sizeof(double), cudaHostAllocMapped));
-    CUDA_TRY(cudaHostGetDevicePointer((void**)&l->result_dev, l->result_host, 0));
-    l->stage_bytes = (size_t)kStageSites * 36 * 16;
-    for (int i = 0; i < 2; i++) {
-        if ((rc = dev_alloc(l->stage_bytes, &l->stage[i])) != QDP_OK) { delete l; return rc; }
-        CUDA_TRY(cudaEventCreateWithFlags(&l->ev_copied[i], cudaEventDisableTiming));
-        CUDA_TRY(cudaEventCreateWithFlags(&l->ev_done[i], cudaEventDisableTiming));
-    }
-    CUDA_TRY(cudaStreamCreateWithFlags(&l->copy_stream, cudaStreamNonBlocking));
+    // everything below is released by release_lattice() on any failure
+    auto attempt = [&]() -> int {
+        int rc;
+        void* p = nullptr;
+        if ((rc = dev_alloc(npart * sizeof(double), &p)) != QDP_OK) return rc;
+        l->partials = (double*)p;
+        if ((rc = dev_alloc(counter_bytes, &p)) != QDP_OK) return rc;
+        l->counter = (unsigned int*)p;
+        CUDA_TRY(cudaMemset(l->counter, 0, counter_bytes));
+        CUDA_TRY(cudaHostAlloc((void**)&l->result_host, 72 * sizeof(double), cudaHostAllocMapped));
+        CUDA_TRY(cudaHostGetDevicePointer((void**)&l->result_dev, l->result_host, 0));
+        l->stage_bytes = (size_t)kStageSites * 36 * 16;
+        for (int i = 0; i < 2; i++) {
+            if ((rc = dev_alloc(l->stage_bytes, &l->stage[i])) != QDP_OK) return rc;
+            CUDA_TRY(cudaEventCreateWithFlags(&l->ev_copied[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&l->ev_done[i], cudaEventDisableTiming));
+        }
+        CUDA_TRY(cudaStreamCreateWithFlags(&l->copy_stream, cudaStreamNonBlocking));
+        return QDP_OK;
+    };
+    const int rc = attempt();
+    if (rc != QDP_OK) { release_lattice(l); return rc; }
     *out = l;
     return QDP_OK;
 }
@@ -179,18 +201,8 @@ extern "C" int qdp_lattice_destroy(qdp_lattice* l) {
     if (l->live_fields) return fail(QDP_ERR_ARG, "qdp_lattice_destroy: %d fields still alive", l->live_fields);
     ENTER(l);
     cudaStreamSynchronize(l->stream);
-    cudaStreamSynchronize(l->copy_stream);
-    dev_free(l->partials, l->scratch_from_hook);
-    dev_free(l->counter, l->scratch_from_hook);
-    cudaFreeHost(l->result_host);
-    for (int i = 0; i < 2; i++) {
-        dev_free(l->stage[i], l->scratch_from_hook);
-        cudaEventDestroy(l->ev_copied[i]);
-        cudaEventDestroy(l->ev_done[i]);
-    }
-    cudaStreamDestroy(l->copy_stream);
-    l->magic = 0;
-    delete l;
+    if (l->copy_stream) cudaStreamSynchronize(l->copy_stream);
+    release_lattice(l);
     return QDP_OK;
 }
 
