@@ -36,7 +36,7 @@ constexpr int kApeThreads = APE_THREADS;
 #define APE_MIN_BLOCKS_F32 3
 #endif
 // fp64: 2 blocks of 128 threads per SM (255 registers, the software pipeline needs them);
-// fp32: 3 blocks (168 registers; the projection runs in fp64 for both precisions)
+// fp32: 3 blocks (168 registers; 4 blocks x 128 registers measured the same, 5 x 96 slower)
 template <class T> struct ApeCfg { static constexpr int kMinBlocks = sizeof(T) == 8 ? 2 : APE_MIN_BLOCKS_F32; };
 
 __device__ __forceinline__ int sel4(const int (&a)[4], int i) {
@@ -110,30 +110,37 @@ ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out, const typename Vec2
             A = ld_mat_at<T>(ptrA(mu + 1, 0));
             B = ld_mat_at<T>(ptrB(mu + 1, 0));
         }
-        // (1-alpha) U + (alpha/n) S, then the projection, always in fp64: for fp32 fields the
-        // closed form on an ill-conditioned V^dag V (hot links: cond ~ 100) would lose ~2e-5 in
-        // fp32, the whole fp32 error budget.
-        Mat3<double> Vd;
-#pragma unroll
-        for (int c = 0; c < 9; c++) {
-            T re = w_link * U.e[c].re + w_staple * S.e[c].re;
-            T im = w_link * U.e[c].im + w_staple * S.e[c].im;
-            Vd.e[c] = cx<double>((double)re, (double)im);
-        }
-        ProjScalars ps[1];
-        proj_stage_a(Vd, ps[0]);
-        // The block ends here, after the seeds: the scalar Newton chains and the final product of
-        // this link then share a basic block with the staples of the next direction, and ptxas
-        // fills the chains' dependency stalls with independent matrix work (0.757 -> 0.732 ms;
-        // a boundary after the store instead keeps them apart).
-        BLOCK_BOUNDARY(g);
-        proj_stage_b<1>(ps);
-        Mat3<double> Pd = proj_stage_c(Vd, ps[0]);
+        // (1-alpha) U + (alpha/n) S, then the projection: fp64 fields in fp64 (su3.cuh: staged closed
+        // form), fp32 fields entirely in fp32 (closed form + one Newton-Schulz step, su3.cuh:
+        // proj_su3_f32), so the fp32 kernel never touches the fp64 pipe.
         T2* o = site_ptr(out, 36, mu * 9, sb);
+        Mat3<T> W;
+        if constexpr (sizeof(T) == 8) {
+            Mat3<double> Vd;
+#pragma unroll
+            for (int c = 0; c < 9; c++)
+                Vd.e[c] = cx<double>(w_link * U.e[c].re + w_staple * S.e[c].re, w_link * U.e[c].im + w_staple * S.e[c].im);
+            ProjScalars ps[1];
+            proj_stage_a(Vd, ps[0]);
+            // The block ends here, after the seeds: the scalar Newton chains and the final product of
+            // this link then share a basic block with the staples of the next direction, and ptxas
+            // fills the chains' dependency stalls with independent matrix work (0.757 -> 0.732 ms;
+            // a boundary after the store instead keeps them apart).
+            BLOCK_BOUNDARY(g);
+            proj_stage_b<1>(ps);
+            W = proj_stage_c(Vd, ps[0]);
+        } else {
+            Mat3<float> Vf;
+#pragma unroll
+            for (int c = 0; c < 9; c++)
+                Vf.e[c] = cx<float>(w_link * U.e[c].re + w_staple * S.e[c].re, w_link * U.e[c].im + w_staple * S.e[c].im);
+            W = proj_su3_f32(Vf);
+            BLOCK_BOUNDARY(g);
+        }
 #pragma unroll
         for (int c = 0; c < 9; c++) {
             T2 v;
-            v.x = (T)Pd.e[c].re; v.y = (T)Pd.e[c].im;
+            v.x = W.e[c].re; v.y = W.e[c].im;
             o[c * kLane] = v;
         }
     }
