@@ -282,15 +282,19 @@ def run_ours(args) -> dict | None:
     # Two lattices driven by two host threads: PCIe is full duplex, so the upload of one step
     # overlaps the download of the other (a single synchronous step uses one direction at a time).
     # Every step still moves its own inputs and results; `value` = steps of both pipes / wall time.
-    e2e_s, n_pipes = 0.0, 2
+    e2e_s, n_pipes = 0.0, args.e2e_pipes
     if ke:
         pipes = [make_pipe(lat, u, psi, u2, chi, sh)]
-        lat_b = q.qdp_lattice_create(dims, local)
-        stream_b = torch.cuda.Stream()
-        q.qdp_lattice_set_stream(lat_b, stream_b.cuda_stream)
-        pipes.append(make_pipe(lat_b, q.qdp_field_alloc(lat_b, q.QDP_GAUGE, P), q.qdp_field_alloc(lat_b, q.QDP_FERMION, P),
-                               q.qdp_field_alloc(lat_b, q.QDP_GAUGE, P), q.qdp_field_alloc(lat_b, q.QDP_FERMION, P),
-                               q.qdp_field_alloc(lat_b, q.QDP_FERMION, P)))
+        extra = []      # keep the extra lattices, streams and fields alive
+        for _ in range(n_pipes - 1):
+            lat_b = q.qdp_lattice_create(dims, local)
+            stream_b = torch.cuda.Stream()
+            q.qdp_lattice_set_stream(lat_b, stream_b.cuda_stream)
+            fields_b = (q.qdp_field_alloc(lat_b, q.QDP_GAUGE, P), q.qdp_field_alloc(lat_b, q.QDP_FERMION, P),
+                        q.qdp_field_alloc(lat_b, q.QDP_GAUGE, P), q.qdp_field_alloc(lat_b, q.QDP_FERMION, P),
+                        q.qdp_field_alloc(lat_b, q.QDP_FERMION, P))
+            extra.append((lat_b, stream_b, fields_b))
+            pipes.append(make_pipe(lat_b, *fields_b))
         for one in pipes:
             one(0)
         barrier()
@@ -360,7 +364,7 @@ def run_ours(args) -> dict | None:
                      "h2d_bytes_per_step": int(hu.nbytes + hp.nbytes),
                      "d2h_bytes_per_step": int(hu.nbytes + hp.nbytes),
                      "steps": ke * n_pipes, "ms_per_step": e2e_ms / (ke * n_pipes),
-                     "pipelining": "2 lattices x 2 host threads, one transfer per PCIe direction at a time (the upload of one "
+                     "pipelining": f"{n_pipes} lattices x {n_pipes} host threads, one transfer per PCIe direction at a time (the upload of one "
                                    "step overlaps the download of the other); each step moves its own inputs and results"}
                     if ke else None),
             "gpu_launches": int(launches),
@@ -472,6 +476,7 @@ def main():
     ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-pipes", type=int, default=2, help="lattices (host threads) pipelined in the e2e leg")
     ap.add_argument("--cpu-fraction", type=int, default=1, help="cpu_baseline runs on V/fraction sites (1: one whole pass, ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
