@@ -602,3 +602,35 @@ def test_matvec_and_hop_composed_from_generic_ops(qdp, lat_cache, dims, prec):
     with pytest.raises(qdp.QdpError) as e:
         qdp.qdp_matvec(inplace, u, 2, 1, inplace, 0, 1)
     assert e.value.code == -6
+
+
+@pytest.mark.parametrize("dims", [(2, 4, 2, 6), (12, 2, 2, 2), (2, 2, 2, 34), (14, 2, 6, 2), (64, 2, 2, 2), (2, 18, 2, 4)])
+def test_unusual_shapes_one_pass(qdp, dims):
+    """Extents of 2 in every position, rows longer and shorter than a warp, half-volumes that are
+    not multiples of 32: one fp64 pass of every neighbour-reading op against the oracle."""
+    lat = qdp.qdp_lattice_create(dims)
+    hu, hp = synth.gauge_hot(dims, _seed(dims) + 101), synth.spinor(dims, _seed(dims) + 102)
+    u, psi = qdp.field_from_host(lat, 1, hu), qdp.field_from_host(lat, 2, hp)
+    u2, chi = qdp.qdp_field_alloc(lat, 1, 1), qdp.qdp_field_alloc(lat, 2, 1)
+    for mu in range(4):
+        for sign in (1, -1):
+            qdp.qdp_shift(chi, psi, mu, sign)
+            assert np.array_equal(qdp.field_to_host(chi), oracle.shift(dims, hp, mu, sign)), (mu, sign)
+    assert np.abs(qdp.qdp_plaquette(u) - oracle.plaquette(dims, hu)).max() <= 1e-10
+    for t_dir in (3, -1):
+        qdp.qdp_ape_smear_step(u2, u, 0.5, t_dir)
+        want = oracle.ape_smear_step(dims, hu, 0.5, t_dir)
+        fixed, _ = z3_fix(links(qdp.field_to_host(u2)), links(want))
+        assert site_rel_err(fixed, links(want)).max() <= TOL_SITE["f64"], t_dir
+    for sub in SUBSETS:
+        chi = qdp.field_from_host(lat, 2, hp)
+        n2 = qdp.qdp_axpy_hop(chi, 0.7, -0.4, u, psi, sub, want_norm2=True)
+        want = oracle.axpy_hop(dims, 0.7, -0.4, hu, hp, sub, chi=hp)
+        assert site_rel_err(qdp.field_to_host(chi), want).max() <= TOL_SITE["f64"], sub
+        assert abs(n2 - oracle.norm2(dims, want, sub)) <= 1e-10 * n2
+    ts = qdp.qdp_inner_timeslices(psi, chi)
+    assert np.abs(ts - oracle.inner_timeslices(dims, hp, qdp.field_to_host(chi))).max() <= 1e-10 * 8 * oracle.norm2(dims, hp)
+    m = qdp.qdp_field_alloc(lat, 0, 1)
+    qdp.qdp_matmul(m, 0, u, 1, 0, u, 0, 1, 1, -1)
+    want = oracle.matmul(dims, np.zeros((synth.volume(dims), 3, 3), dtype=np.complex128), 0, hu, 1, 0, hu, 0, 1, 1, -1)
+    assert site_rel_err(qdp.field_to_host(m), want).max() <= TOL_SITE["f64"]
