@@ -68,6 +68,8 @@ def _get():
             "orc_sum": ([P, I, P, I, P], None),
             "orc_inner_timeslices": ([P, I, P, P, I, P], None),
             "orc_axpby": ([P, I, D, P, D, P, P, I], None),
+            "orc_gamma_matrix": ([I, P], None),
+            "orc_inner_timeslices_gamma": ([P, P, P, I, I, P], None),
             # the same loops over lex sites [begin, end): bounded samples for bench.py
             "orc_shift_bytes_range": ([P, Z, P, P, I, I, I, Z, Z], None),
             "orc_plaquette_range": ([P, P, I, Z, Z, P], None),
@@ -269,6 +271,21 @@ def inner(dims, a, b, subset=ALL):
     _get().orc_inner(_dims(dims), _reals(dims, a), a.ctypes.data, b.ctypes.data, subset,
                      out.ctypes.data)
     return complex(out[0], out[1])
+
+
+def gamma_matrix(n):
+    """Gamma(n) = g0^n0 g1^n1 g2^n2 g3^n3 (DeGrand-Rossi basis), complex [4,4]."""
+    out = np.empty((4, 4), dtype=np.complex128)
+    _get().orc_gamma_matrix(int(n), out.ctypes.data)
+    return out
+
+
+def inner_timeslices_gamma(dims, a, b, n, subset=ALL):
+    """out[t] = sum over x3 = t of a^dag Gamma(n) b (spin matrix on the spin index), complex [L3]."""
+    a, b = _c128(a), _c128(b)
+    out = np.empty(2 * int(dims[3]))
+    _get().orc_inner_timeslices_gamma(_dims(dims), a.ctypes.data, b.ctypes.data, int(n), subset, out.ctypes.data)
+    return out[0::2] + 1j * out[1::2]
 
 
 def axpby(dims, a, x, b, y, subset=ALL, dst=None):

@@ -600,6 +600,61 @@ void orc_inner_timeslices(const int *L, int reals, const double *a, const double
     }
 }
 
+/* ---- spin matrices (meson contractions) -----------------------------------
+ * Euclidean gamma matrices in the DeGrand-Rossi basis (the convention of QDP++/Chroma):
+ *   g0 = [[0,0,0,i],[0,0,i,0],[0,-i,0,0],[-i,0,0,0]]    g1 = [[0,0,0,-1],[0,0,1,0],[0,1,0,0],[-1,0,0,0]]
+ *   g2 = [[0,0,i,0],[0,0,0,-i],[-i,0,0,0],[0,i,0,0]]    g3 = [[0,0,1,0],[0,0,0,1],[1,0,0,0],[0,1,0,0]]
+ * Gamma(n) = g0^n0 g1^n1 g2^n2 g3^n3 with n = n0 + 2 n1 + 4 n2 + 8 n3 (Gamma(15) = gamma_5). */
+static void gamma_base(int mu, cplx g[16]) {
+    static const int pos[4][4] = { {3, 2, 1, 0}, {3, 2, 1, 0}, {2, 3, 0, 1}, {2, 3, 0, 1} };
+    static const double re[4][4] = { {0, 0, 0, 0}, {-1, 1, 1, -1}, {0, 0, 0, 0}, {1, 1, 1, 1} };
+    static const double im[4][4] = { {1, 1, -1, -1}, {0, 0, 0, 0}, {1, -1, -1, 1}, {0, 0, 0, 0} };
+    memset(g, 0, 16 * sizeof(cplx));
+    for (int r = 0; r < 4; r++) { g[r * 4 + pos[mu][r]].re = re[mu][r]; g[r * 4 + pos[mu][r]].im = im[mu][r]; }
+}
+void orc_gamma_matrix(int n, double *out32) {
+    cplx acc[16], tmp[16], g[16];
+    memset(acc, 0, sizeof acc);
+    for (int i = 0; i < 4; i++) acc[i * 5].re = 1.0;
+    for (int mu = 0; mu < 4; mu++) {
+        if (!((n >> mu) & 1)) continue;
+        gamma_base(mu, g);
+        for (int i = 0; i < 4; i++)
+            for (int j = 0; j < 4; j++) {
+                cplx t = { 0, 0 };
+                for (int k = 0; k < 4; k++) t = c_add(t, c_mul(acc[i * 4 + k], g[k * 4 + j]));
+                tmp[i * 4 + j] = t;
+            }
+        memcpy(acc, tmp, sizeof acc);
+    }
+    memcpy(out32, acc, sizeof acc);
+}
+/* out[t] = sum_{x in subset, x3 = t} sum_{s' s c} conj(a_{s' c}(x)) Gamma(n)_{s' s} b_{s c}(x):
+ * with a, b columns of a quark propagator, the building block of meson two-point functions. */
+void orc_inner_timeslices_gamma(const int *L, const double *a, const double *b, int n, int subset,
+                                double *out) {
+    cplx G[16];
+    orc_gamma_matrix(n, (double *)G);
+    for (int t = 0; t < L[3]; t++) {
+        ksum kr = { 0, 0 }, ki = { 0, 0 };
+        for (size_t s = 0; s < volume(L); s++) {
+            int x[4]; coords_of(L, s, x);
+            if (x[3] != t || !in_subset(x, subset)) continue;
+            const cplx *pa = (const cplx *)a + s * 12, *pb = (const cplx *)b + s * 12;
+            for (int sp = 0; sp < 4; sp++)
+                for (int c = 0; c < 3; c++) {
+                    cplx gb = { 0, 0 };
+                    for (int s2 = 0; s2 < 4; s2++) gb = c_add(gb, c_mul(G[sp * 4 + s2], pb[s2 * 3 + c]));
+                    cplx p = c_mul(c_conj(pa[sp * 3 + c]), gb);
+                    k_add(&kr, p.re);
+                    k_add(&ki, p.im);
+                }
+        }
+        out[2 * t] = k_val(&kr);
+        out[2 * t + 1] = k_val(&ki);
+    }
+}
+
 /* out[c] = sum_x f_c(x), per real component (re, im interleaved like f). */
 void orc_sum(const int *L, int reals, const double *f, int subset, double *out) {
     size_t V = volume(L);

@@ -1,0 +1,55 @@
+"""Pins for the oracle's spin matrices and the gamma-inserted time-slice contraction (row f3)."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from npref import view4
+
+
+def test_clifford_algebra_hermiticity_and_gamma5():
+    g = [oracle.gamma_matrix(1 << mu) for mu in range(4)]
+    eye = np.eye(4)
+    for mu in range(4):
+        assert np.array_equal(g[mu], np.conj(g[mu].T))                       # Hermitian
+        for nu in range(4):
+            assert np.array_equal(g[mu] @ g[nu] + g[nu] @ g[mu], 2 * eye * (mu == nu))
+    g5 = oracle.gamma_matrix(15)
+    assert np.array_equal(g5, g[0] @ g[1] @ g[2] @ g[3])
+    assert np.array_equal(g5 @ g5, eye) and np.trace(g5) == 0 and np.array_equal(g5, np.conj(g5.T))
+    for mu in range(4):
+        assert np.array_equal(g5 @ g[mu] + g[mu] @ g5, np.zeros((4, 4)))
+    assert np.array_equal(oracle.gamma_matrix(0), eye)
+    # every Gamma(n) is a signed/phased permutation (one entry of modulus 1 per row and column): the
+    # 16 of them are linearly independent (a basis of the 4x4 matrices)
+    basis = np.stack([oracle.gamma_matrix(n).ravel() for n in range(16)])
+    assert np.linalg.matrix_rank(basis) == 16
+    for n in range(16):
+        G = oracle.gamma_matrix(n)
+        assert np.array_equal((np.abs(G) == 1).sum(axis=0), np.ones(4)) and np.abs(G).sum() == 4
+        assert n == sum(((n >> mu) & 1) << mu for mu in range(4))
+        want = eye.astype(complex)
+        for mu in range(4):
+            if (n >> mu) & 1:
+                want = want @ g[mu]
+        assert np.array_equal(G, want)
+
+
+@pytest.mark.parametrize("dims", [(2, 2, 2, 4), (4, 2, 6, 4)])
+def test_contraction_brute_force_and_identities(dims):
+    a, b = synth.spinor(dims, 701), synth.spinor(dims, 702, 1)
+    scale = oracle.norm2(dims, a) + oracle.norm2(dims, b)
+    for n in (0, 1, 6, 8, 15, 11):
+        G = oracle.gamma_matrix(n)
+        gb = np.einsum("ts,xsc->xtc", G, b)
+        want = view4(dims, np.conj(a) * gb).reshape(dims[3], -1).sum(axis=1)
+        got = oracle.inner_timeslices_gamma(dims, a, b, n)
+        assert np.abs(got - want).max() < 1e-13 * scale
+        # <a, G b> = conj(<b, G^dag a>), G^dag = +-G
+        sign = 1.0 if np.array_equal(G, np.conj(G.T)) else -1.0
+        assert np.array_equal(np.conj(G.T), sign * G)
+        back = oracle.inner_timeslices_gamma(dims, b, a, n)
+        assert np.abs(got - sign * np.conj(back)).max() < 1e-13 * scale
+    assert np.abs(oracle.inner_timeslices_gamma(dims, a, b, 0) - oracle.inner_timeslices(dims, a, b)).max() < 1e-13 * scale
+    e, o = oracle.inner_timeslices_gamma(dims, a, b, 15, 1), oracle.inner_timeslices_gamma(dims, a, b, 15, 2)
+    assert np.abs(e + o - oracle.inner_timeslices_gamma(dims, a, b, 15)).max() < 1e-13 * scale
