@@ -248,6 +248,16 @@ int qdp_axpby(qdp_field* dst, double a, const qdp_field* x, double b, const qdp_
  * Synchronous. */
 int qdp_inner_timeslices(const qdp_field* a, const qdp_field* b, qdp_subset subset, double* out);
 
+/* Row f3, meson contractions: the same sums with a spin matrix inserted,
+ *   out[2t], out[2t+1] = sum_{x in subset, x3 = t} sum_{s' s c} conj(a_{s' c}(x)) Gamma(n)_{s' s} b_{s c}(x),
+ * a, b: QDP_FERMION.  Gamma(n) = g0^n0 g1^n1 g2^n2 g3^n3, n = n0 + 2 n1 + 4 n2 + 8 n3 in 0..15 (Gamma(15) = gamma_5),
+ * Euclidean Hermitian gamma matrices in the DeGrand-Rossi basis (the QDP++ convention):
+ *   g0 = [[0,0,0,i],[0,0,i,0],[0,-i,0,0],[-i,0,0,0]]    g1 = [[0,0,0,-1],[0,0,1,0],[0,1,0,0],[-1,0,0,0]]
+ *   g2 = [[0,0,i,0],[0,0,0,-i],[-i,0,0,0],[0,i,0,0]]    g3 = [[0,0,1,0],[0,0,0,1],[1,0,0,0],[0,1,0,0]]
+ * With a, b columns of quark propagators this is the building block of meson two-point functions
+ * (HAD stage).  n = 0 equals qdp_inner_timeslices.  Synchronous. */
+int qdp_inner_timeslices_gamma(const qdp_field* a, const qdp_field* b, int n, qdp_subset subset, double* out);
+
 /* Block the host until every call enqueued on the lattice's stream has finished. */
 int qdp_lattice_sync(qdp_lattice* lat);
 

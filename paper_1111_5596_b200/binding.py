@@ -18,7 +18,7 @@ __all__ = [
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
-    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_reunitarize", "qdp_matmul", "qdp_matvec", "qdp_axpby", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
+    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_matmul", "qdp_matvec", "qdp_axpby", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
 ]
@@ -66,6 +66,7 @@ DECLARED_SYMBOLS = {
     "qdp_axpy_hop": ([_P, _D, _D, _P, _P, _I, _P], _I),
     "qdp_smear_hop": ([_P, _D, _D, _P, _P, _I, _I, _P], _I),
     "qdp_inner_timeslices": ([_P, _P, _I, _P], _I),
+    "qdp_inner_timeslices_gamma": ([_P, _P, _I, _I, _P], _I),
     "qdp_reunitarize": ([_P, _P, _I, _I], _I),
     "qdp_axpby": ([_P, _D, _P, _D, _P, _I, _P], _I),
     "qdp_matvec": ([_P, _P, _I, _I, _P, _I, _I, _I], _I),
@@ -330,6 +331,13 @@ def qdp_inner_timeslices(a: Field, b: Field, subset: int = QDP_ALL) -> np.ndarra
     """complex [L3]: sum over the sites of each time-slice x3 = t of conj(a) . b"""
     out = np.empty(2 * int(a.lat.dims[3]), dtype=np.float64)
     _check(_lib.qdp_inner_timeslices(a.handle, b.handle, subset, out.ctypes.data))
+    return out[0::2] + 1j * out[1::2]
+
+
+def qdp_inner_timeslices_gamma(a: Field, b: Field, n: int, subset: int = QDP_ALL) -> np.ndarray:
+    """complex [L3]: sum over the sites of each time-slice of a^dag Gamma(n) b (Gamma(15) = gamma_5)"""
+    out = np.empty(2 * int(a.lat.dims[3]), dtype=np.float64)
+    _check(_lib.qdp_inner_timeslices_gamma(a.handle, b.handle, int(n), subset, out.ctypes.data))
     return out[0::2] + 1j * out[1::2]
 
 

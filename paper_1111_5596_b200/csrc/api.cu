@@ -555,18 +555,51 @@ extern "C" int qdp_axpby(qdp_field* dst, double a, const qdp_field* x, double b,
     return QDP_OK;
 }
 
+// Gamma(n) as a phased permutation, built from the four base matrices of the header:
+// (A B) has perm[r] = pB[pA[r]] and phase phA[r] + phB[pA[r]] (phases count powers of i).
+static SpinMatrix spin_matrix(int n) {
+    static const int bperm[4][4] = { {3, 2, 1, 0}, {3, 2, 1, 0}, {2, 3, 0, 1}, {2, 3, 0, 1} };
+    static const int bph[4][4] = { {1, 1, 3, 3}, {2, 0, 0, 2}, {1, 3, 3, 1}, {0, 0, 0, 0} };
+    SpinMatrix m = {{0, 1, 2, 3}, {0, 0, 0, 0}};
+    for (int mu = 0; mu < 4; mu++) {
+        if (!((n >> mu) & 1)) continue;
+        SpinMatrix r;
+        for (int row = 0; row < 4; row++) {
+            r.perm[row] = bperm[mu][m.perm[row]];
+            r.ph[row] = (m.ph[row] + bph[mu][m.perm[row]]) & 3;
+        }
+        m = r;
+    }
+    return m;
+}
+
+static int inner_timeslices_common(const char* who, const qdp_field* a, const qdp_field* b, qdp_subset subset, double* out,
+                                   const SpinMatrix* gamma);
+
 extern "C" int qdp_inner_timeslices(const qdp_field* a, const qdp_field* b, qdp_subset subset, double* out) {
+    return inner_timeslices_common("qdp_inner_timeslices", a, b, subset, out, nullptr);
+}
+extern "C" int qdp_inner_timeslices_gamma(const qdp_field* a, const qdp_field* b, int n, qdp_subset subset, double* out) {
+    if (n < 0 || n > 15) return fail(QDP_ERR_ARG, "qdp_inner_timeslices_gamma: n must be 0..15");
+    if (ok_field(a) && ok_field(b) && (a->kind != QDP_FERMION || b->kind != QDP_FERMION))
+        return fail(QDP_ERR_KIND, "qdp_inner_timeslices_gamma: fermion fields needed");
+    const SpinMatrix m = spin_matrix(n);
+    return inner_timeslices_common("qdp_inner_timeslices_gamma", a, b, subset, out, &m);
+}
+
+static int inner_timeslices_common(const char* who, const qdp_field* a, const qdp_field* b, qdp_subset subset, double* out,
+                                   const SpinMatrix* gamma) {
     if (!ok_field(a) || !ok_field(b) || !out || !ok_subset(subset))
-        return fail(QDP_ERR_ARG, "qdp_inner_timeslices: bad argument");
-    int rc = check_pair("qdp_inner_timeslices", a, b);
+        return fail(QDP_ERR_ARG, "%s: bad argument", who);
+    int rc = check_pair(who, a, b);
     if (rc != QDP_OK) return rc;
-    if (a->kind != b->kind) return fail(QDP_ERR_KIND, "qdp_inner_timeslices: kinds differ");
+    if (a->kind != b->kind) return fail(QDP_ERR_KIND, "%s: kinds differ", who);
     qdp_lattice* l = a->lat;
     ENTER(l);
     const int L3 = l->geom.L3;
     double* out_dev = l->partials + (size_t)2 * 16 * L3;   // behind the per-block partials
     CUDA_TRY(launch_inner_timeslices(a->prec, l->geom, a->ncomp, a->data, b->data, subset, l->partials, out_dev,
-                                     l->stream));
+                                     l->stream, gamma));
     CUDA_TRY(cudaMemcpyAsync(out, out_dev, (size_t)2 * L3 * sizeof(double), cudaMemcpyDeviceToHost, l->stream));
     CUDA_TRY(cudaStreamSynchronize(l->stream));
     return QDP_OK;

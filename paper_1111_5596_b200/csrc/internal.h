@@ -38,9 +38,12 @@ cudaError_t launch_sum(int prec, const Geom& g, int ncomp, const void* f, int su
 // dst = a x + b y on the subset (dst may be x or y); want_norm2: norm2(dst) through rb
 cudaError_t launch_axpby(int prec, const Geom& g, int ncomp, void* dst, const void* x, const void* y, double a,
                          double b, int subset, bool want_norm2, const ReduceBuf& rb, cudaStream_t st);
-// partials: scratch of 2*16*L3 doubles; out_dev: 2*L3 doubles on the device
+// A spin matrix that is a phased permutation: (Gamma psi)_s = i^ph[s] psi_perm[s] (every product of gamma matrices is one)
+struct SpinMatrix { int perm[4]; int ph[4]; };
+// partials: scratch of 2*16*L3 doubles; out_dev: 2*L3 doubles on the device; gamma != nullptr (fermions only):
+// a is paired with Gamma b
 cudaError_t launch_inner_timeslices(int prec, const Geom& g, int ncomp, const void* a, const void* b, int subset,
-                                    double* partials, double* out_dev, cudaStream_t st);
+                                    double* partials, double* out_dev, cudaStream_t st, const SpinMatrix* gamma = nullptr);
 
 // hop.cu
 // ndir = 4: all directions; 3: mu = 0, 1, 2 only (qdp_smear_hop with t_dir = 3)

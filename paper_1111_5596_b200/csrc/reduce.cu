@@ -220,6 +220,21 @@ cudaError_t launch_axpby(int prec, const Geom& g, int ncomp, void* dst, const vo
     return cudaGetLastError();
 }
 
+// element e of (Gamma b) for a fermion field in the blocked layout (component = (e / 32) % 12 = 3 spin + colour)
+template <class T2>
+__device__ __forceinline__ T2 spin_apply(const SpinMatrix& gm, const T2* __restrict__ b, unsigned e) {
+    const int sp = (int)((e >> 5) % 12u) / 3;
+    const T2 v = __ldg(b + (long long)e + 96 * (gm.perm[sp] - sp));
+    T2 r;
+    switch (gm.ph[sp]) {                       // multiply by i^ph
+        case 0: r.x = v.x; r.y = v.y; break;
+        case 1: r.x = -v.y; r.y = v.x; break;
+        case 2: r.x = -v.x; r.y = -v.y; break;
+        default: r.x = v.y; r.y = -v.x; break;
+    }
+    return r;
+}
+
 // ---- time-slice inner products -----------------------------------
 // out[t] = sum over the sites with x3 = t of conj(a) . b.  In the blocked layout the half-indices of
 // a time-slice are one run [t*s3, (t+1)*s3) per parity half, so when s3 is a multiple of 32 a slice
@@ -228,10 +243,13 @@ cudaError_t launch_axpby(int prec, const Geom& g, int ncomp, void* dst, const vo
 // elements whose site has x3 = t.  One partial per block, summed in block order by the finish
 // kernel: deterministic, fp64.
 constexpr int kTsBlocks = 16;
-template <class T2, bool FAST>
+// GAMMA: a is paired with (Gamma b), Gamma a phased permutation of the spin index (fermions only):
+// (Gamma b)_{s c} = i^ph[s] b_{perm[s] c}, which in the blocked layout is the element 96 * (perm[s] - s)
+// places further on.
+template <class T2, bool FAST, bool GAMMA>
 __global__ void __launch_bounds__(kReduceThreads) inner_ts_kernel(Geom g, int ncomp, const T2* __restrict__ a,
                                                                  const T2* __restrict__ b, int subset,
-                                                                 double* __restrict__ partials) {
+                                                                 double* __restrict__ partials, SpinMatrix gm) {
     __shared__ double sm[2][kReduceThreads / 32];
     const int t = blockIdx.y;
     const unsigned stride = gridDim.x * kReduceThreads;
@@ -243,7 +261,9 @@ __global__ void __launch_bounds__(kReduceThreads) inner_ts_kernel(Geom g, int nc
             const T2 *pa = a + begin, *pb = b + begin;
 #pragma unroll 4
             for (unsigned e = blockIdx.x * kReduceThreads + threadIdx.x; e < n; e += stride) {
-                const T2 va = __ldg(pa + e), vb = __ldg(pb + e);
+                const T2 va = __ldg(pa + e);
+                T2 vb;
+                if (GAMMA) vb = spin_apply(gm, pb, e); else vb = __ldg(pb + e);
                 acc[0] += (double)va.x * (double)vb.x + (double)va.y * (double)vb.y;
                 acc[1] += (double)va.x * (double)vb.y - (double)va.y * (double)vb.x;
             }
@@ -253,7 +273,9 @@ __global__ void __launch_bounds__(kReduceThreads) inner_ts_kernel(Geom g, int nc
             for (unsigned e = blockIdx.x * kReduceThreads + threadIdx.x; e < n; e += stride) {
                 const int h = (int)(e / (ncomp * 32u)) * 32 + (int)(e & 31u);
                 if (h >= g.Vh || h / g.s3 != t) continue;
-                const T2 va = __ldg(a + begin + e), vb = __ldg(b + begin + e);
+                const T2 va = __ldg(a + begin + e);
+                T2 vb;
+                if (GAMMA) vb = spin_apply(gm, b + begin, e); else vb = __ldg(b + begin + e);
                 acc[0] += (double)va.x * (double)vb.x + (double)va.y * (double)vb.y;
                 acc[1] += (double)va.x * (double)vb.y - (double)va.y * (double)vb.x;
             }
@@ -273,16 +295,19 @@ __global__ void inner_ts_finish_kernel(int nblk, const double* __restrict__ part
 }
 
 cudaError_t launch_inner_timeslices(int prec, const Geom& g, int ncomp, const void* a, const void* b, int subset,
-                                    double* partials, double* out_dev, cudaStream_t st) {
+                                    double* partials, double* out_dev, cudaStream_t st, const SpinMatrix* gamma) {
     dim3 grid(kTsBlocks, g.L3);
     const bool fast = (g.s3 & 31) == 0;
+    SpinMatrix gm = gamma ? *gamma : SpinMatrix{{0, 1, 2, 3}, {0, 0, 0, 0}};
+#define QDP_TS(T2, F, G) inner_ts_kernel<T2, F, G><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const T2*)a, (const T2*)b, subset, partials, gm)
     if (prec) {
-        if (fast) inner_ts_kernel<double2, true><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const double2*)a, (const double2*)b, subset, partials);
-        else      inner_ts_kernel<double2, false><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const double2*)a, (const double2*)b, subset, partials);
+        if (gamma) { if (fast) QDP_TS(double2, true, true); else QDP_TS(double2, false, true); }
+        else       { if (fast) QDP_TS(double2, true, false); else QDP_TS(double2, false, false); }
     } else {
-        if (fast) inner_ts_kernel<float2, true><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const float2*)a, (const float2*)b, subset, partials);
-        else      inner_ts_kernel<float2, false><<<grid, kReduceThreads, 0, st>>>(g, ncomp, (const float2*)a, (const float2*)b, subset, partials);
+        if (gamma) { if (fast) QDP_TS(float2, true, true); else QDP_TS(float2, false, true); }
+        else       { if (fast) QDP_TS(float2, true, false); else QDP_TS(float2, false, false); }
     }
+#undef QDP_TS
     inner_ts_finish_kernel<<<g.L3, 2, 0, st>>>(kTsBlocks, partials, out_dev);
     g_launch_count += 2;
     return cudaGetLastError();

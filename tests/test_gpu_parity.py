@@ -634,3 +634,30 @@ def test_unusual_shapes_one_pass(qdp, dims):
     qdp.qdp_matmul(m, 0, u, 1, 0, u, 0, 1, 1, -1)
     want = oracle.matmul(dims, np.zeros((synth.volume(dims), 3, 3), dtype=np.complex128), 0, hu, 1, 0, hu, 0, 1, 1, -1)
     assert site_rel_err(qdp.field_to_host(m), want).max() <= TOL_SITE["f64"]
+
+
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 2, 6, 4), (10, 6, 4, 2), C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_inner_timeslices_gamma(qdp, lat_cache, dims, prec):
+    """qdp_inner_timeslices_gamma (row f3): all 16 spin matrices vs the oracle, subsets on gamma_5."""
+    lat = lat_cache(dims)
+    ha = synth.round_to(synth.spinor(dims, _seed(dims) + 111), prec)
+    hb = synth.round_to(synth.spinor(dims, _seed(dims) + 112, 1), prec)
+    a, b = qdp.field_from_host(lat, 2, ha), qdp.field_from_host(lat, 2, hb)
+    scale = (oracle.norm2(dims, _as64(ha)) + oracle.norm2(dims, _as64(hb))) / dims[3]
+    for n in range(16):
+        got = qdp.qdp_inner_timeslices_gamma(a, b, n)
+        want = oracle.inner_timeslices_gamma(dims, _as64(ha), _as64(hb), n)
+        assert np.abs(got - want).max() <= TOL_SUM[prec] * scale, n
+    assert np.array_equal(qdp.qdp_inner_timeslices_gamma(a, b, 0), qdp.qdp_inner_timeslices(a, b))
+    for sub in (1, 2):
+        got = qdp.qdp_inner_timeslices_gamma(a, b, 15, sub)
+        assert np.abs(got - oracle.inner_timeslices_gamma(dims, _as64(ha), _as64(hb), 15, sub)).max() <= TOL_SUM[prec] * scale
+    # pion correlator form: a^dag a per slice is real and positive
+    pion = qdp.qdp_inner_timeslices_gamma(a, a, 0)
+    assert np.all(pion.real > 0) and np.abs(pion.imag).max() <= 1e-12 * scale * dims[3]
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_inner_timeslices_gamma(a, b, 16)
+    with pytest.raises(qdp.QdpError):
+        m = qdp.qdp_field_alloc(lat, 0, 1 if prec == "f64" else 0)
+        qdp.qdp_inner_timeslices_gamma(m, m, 5)
