@@ -39,14 +39,33 @@ METRIC = "site-updates/s"
 UNIT = "site-updates/s"
 OPS_PER_STEP = 7          # shift, plaquette, ape, hop(even+odd), inner, axpy_hop+norm2, norm2
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
-# ape_kernel<double> is bound by the plain fp64 pipe, not by HBM.
-# Peak: 64 fp64 FMA lanes per clock per SM x 148 SMs x 1.965 GHz x 2 flop = 37.2 TFLOP/s (unit counts and
-# clocks of the guides; a DFMA-only microbenchmark measured 17.07 T DFMA/s = 34.1 TFLOP/s on this pool).
-FP64_PEAK_TFLOPS = 64 * 148 * 1.965e9 * 2 / 1e12
-# fp64 flops per site of one spatial APE step as implemented: 24 3x3 complex products, the blend and three
-# SU(3) projections = 3300 DFMA + 491 DMUL + 92 DADD per site (SASS of ape_kernel<double,false>: straight-line
-# code, every instruction executes once per site; profiles/r1d_ncu_full.md) = 7183 flop.
-APE_FLOPS_PER_SITE_F64 = 3300 * 2 + 491 + 92
+# fp64 instructions per site of the fused kernels as implemented (SASS, straight-line code: every instruction
+# executes once per site; profiles/r2_sass.md): (DFMA, DMUL, DADD).  The "alu" view of the roofline divides the
+# resulting flop rate by the DFMA rate measured in the same run (paper_1111_5596_b200/csrc/probe.cu).
+FP64_INSTR_PER_SITE = {
+    "ape": (3300, 491, 92),          # 24 3x3 complex products, blend, three SU(3) projections
+    "plaquette": (1188, 219, 18),    # 12 products + 6 traces
+}
+
+
+def fp64_flops_per_site(op: str) -> int:
+    dfma, dmul, dadd = FP64_INSTR_PER_SITE[op]
+    return 2 * dfma + dmul + dadd
+
+
+def probe_dfma_rate(device: int, stream) -> float | None:
+    """DFMA per second (thread-level) of the plain fp64 pipe, measured now on this device (bench-only probe library)."""
+    import ctypes
+    from paper_1111_5596_b200.build import PROBE_LIB
+    try:
+        lib = ctypes.CDLL(PROBE_LIB)
+    except OSError:
+        return None
+    lib.qdp_probe_dfma.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+    lib.qdp_probe_dfma.restype = ctypes.c_int
+    out = ctypes.c_double()
+    rc = lib.qdp_probe_dfma(device, stream, 5, ctypes.byref(out))
+    return out.value if rc == 0 else None
 
 
 def algorithmic_bytes(V: int, eb: int) -> dict:
@@ -73,11 +92,12 @@ def measured_peak() -> tuple[float, str]:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(kernel: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture."""
+def ncu_traffic(config: str, prec: str, kernel: str):
+    """dram__bytes_read + write per launch of `kernel` from the committed ncu --set full capture of exactly this
+    (config, precision); None when no capture of that combination is committed."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(kernel)
+            return json.load(f).get(f"{config}/{prec}", {}).get(kernel)
     except Exception:
         return None
 
@@ -150,6 +170,86 @@ def whole_job_value(units_per_rank: int, world: int, ms: float) -> float:
     return units_per_rank * world / (ms * 1e-3)
 
 
+class Workload:
+    """One seeded synthetic lattice of a BASELINE config resident in HBM, and the 7-op step on it."""
+
+    def __init__(self, q, torch, config: str, prec: str, device: int, seed: int):
+        import synth
+        self.q, self.torch, self.config, self.prec = q, torch, config, prec
+        self.dims = synth.CONFIGS[config]
+        self.V = synth.volume(self.dims)
+        self.P = q.QDP_F64 if prec == "f64" else q.QDP_F32
+        self.eb = 16 if prec == "f64" else 8
+        self.hu = synth.round_to(synth.gauge_hot(self.dims, seed), prec)
+        self.hp = synth.round_to(synth.spinor(self.dims, seed), prec)
+        self.a, self.b = synth.scalars_ab(seed)
+        self.stream = torch.cuda.Stream()
+        self.lat = q.qdp_lattice_create(self.dims, device)
+        q.qdp_lattice_set_stream(self.lat, self.stream.cuda_stream)
+        self.u = q.field_from_host(self.lat, q.QDP_GAUGE, self.hu)
+        self.psi = q.field_from_host(self.lat, q.QDP_FERMION, self.hp)
+        self.u2 = q.qdp_field_alloc(self.lat, q.QDP_GAUGE, self.P)
+        self.chi = q.qdp_field_alloc(self.lat, q.QDP_FERMION, self.P)
+        self.sh = q.qdp_field_alloc(self.lat, q.QDP_FERMION, self.P)
+        u, psi, u2, chi, sh, a, b = self.u, self.psi, self.u2, self.chi, self.sh, self.a, self.b
+        self.ops = [
+            ("shift", lambda k: q.qdp_shift(sh, psi, k % 4, 1 if (k // 4) % 2 == 0 else -1)),
+            ("plaquette", lambda k: q.qdp_plaquette(u)),
+            ("ape", lambda k: q.qdp_ape_smear_step(u2, u, 0.5, 3)),
+            ("hop_even", lambda k: q.qdp_hop(chi, u, psi, q.QDP_EVEN)),
+            ("hop_odd", lambda k: q.qdp_hop(chi, u, psi, q.QDP_ODD)),
+            ("inner", lambda k: q.qdp_inner(psi, chi)),
+            ("axpy_hop_norm2", lambda k: q.qdp_axpy_hop(chi, a, b, u, psi, q.QDP_ALL, want_norm2=True)),
+            ("norm2", lambda k: q.qdp_norm2(chi)),
+        ]
+        self.results = {}
+
+    def step(self, k, evs=None):
+        for i, (name, fn) in enumerate(self.ops):
+            if evs is not None:
+                evs[i].record(self.stream)
+            self.results[name] = fn(k)
+        if evs is not None:
+            evs[len(self.ops)].record(self.stream)
+
+    def timed(self, K: int, warmup: int, barrier=None, sampler=None):
+        """W untimed steps, then exactly K steps bracketed by `barrier`; CUDA events on the lattice's stream around
+        every op.  Returns (total ms, per-op mean ms, kernels launched)."""
+        torch, q = self.torch, self.q
+        for k in range(warmup):
+            self.step(k)
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(len(self.ops) + 1)] for _ in range(K)]
+        (barrier or torch.cuda.synchronize)()
+        launches0 = q.qdp_kernel_launch_count()
+        if sampler is not None:
+            sampler.start()
+        for k in range(K):
+            self.step(k, evs[k])
+        torch.cuda.synchronize()
+        self.clocks = sampler.stop() if sampler is not None else None
+        launches = q.qdp_kernel_launch_count() - launches0
+        (barrier or torch.cuda.synchronize)()
+        total_ms = evs[0][0].elapsed_time(evs[K - 1][len(self.ops)])
+        per_op_ms = {name: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)]))
+                     for i, (name, _) in enumerate(self.ops)}
+        return total_ms, per_op_ms, launches
+
+    def op_report(self, per_op_ms: dict, peak: float) -> dict:
+        alg = algorithmic_bytes(self.V, self.eb)
+        rep = {}
+        for name, ms in per_op_ms.items():
+            gbs = alg[name] / ms / 1e6
+            sites = self.V // 2 if name.startswith("hop_") else self.V
+            rep[name] = {"ms": round(ms, 5), "gbs": round(gbs, 1), "frac": round(gbs / peak, 4),
+                         "site_updates_per_s": sites / ms * 1e3}
+        return rep
+
+    def free(self):
+        for f in (self.u, self.psi, self.u2, self.chi, self.sh):
+            self.q.qdp_field_free(f)
+        self.q.qdp_lattice_destroy(self.lat)
+
+
 def run_ours(args) -> dict | None:
     import torch
     import synth
@@ -167,42 +267,12 @@ def run_ours(args) -> dict | None:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
 
-    dims = synth.CONFIGS[args.config]
-    V = synth.volume(dims)
     prec = args.prec
-    P = q.QDP_F64 if prec == "f64" else q.QDP_F32
-    eb = 16 if prec == "f64" else 8
-    seed = synth.BASE_SEED + 3 + rank
-    hu = synth.round_to(synth.gauge_hot(dims, seed), prec)
-    hp = synth.round_to(synth.spinor(dims, seed), prec)
-    a, b = synth.scalars_ab(seed)
-
-    stream = torch.cuda.Stream()
-    lat = q.qdp_lattice_create(dims, local)
-    q.qdp_lattice_set_stream(lat, stream.cuda_stream)
-    u, psi = q.field_from_host(lat, q.QDP_GAUGE, hu), q.field_from_host(lat, q.QDP_FERMION, hp)
-    u2 = q.qdp_field_alloc(lat, q.QDP_GAUGE, P)
-    chi, sh = q.qdp_field_alloc(lat, q.QDP_FERMION, P), q.qdp_field_alloc(lat, q.QDP_FERMION, P)
-
-    ops = [
-        ("shift", lambda k: q.qdp_shift(sh, psi, k % 4, 1 if (k // 4) % 2 == 0 else -1)),
-        ("plaquette", lambda k: q.qdp_plaquette(u)),
-        ("ape", lambda k: q.qdp_ape_smear_step(u2, u, 0.5, 3)),
-        ("hop_even", lambda k: q.qdp_hop(chi, u, psi, q.QDP_EVEN)),
-        ("hop_odd", lambda k: q.qdp_hop(chi, u, psi, q.QDP_ODD)),
-        ("inner", lambda k: q.qdp_inner(psi, chi)),
-        ("axpy_hop_norm2", lambda k: q.qdp_axpy_hop(chi, a, b, u, psi, q.QDP_ALL, want_norm2=True)),
-        ("norm2", lambda k: q.qdp_norm2(chi)),
-    ]
-    results = {}
-
-    def step(k, evs=None):
-        for i, (name, fn) in enumerate(ops):
-            if evs is not None:
-                evs[i].record(stream)
-            results[name] = fn(k)
-        if evs is not None:
-            evs[len(ops)].record(stream)
+    w = Workload(q, torch, args.config, prec, local, synth.BASE_SEED + 3 + rank)
+    dims, V, P, eb = w.dims, w.V, w.P, w.eb
+    hu, hp, a, b = w.hu, w.hp, w.a, w.b
+    stream, lat, u, psi, u2, chi, sh = w.stream, w.lat, w.u, w.psi, w.u2, w.chi, w.sh
+    results = w.results
 
     def barrier():
         torch.cuda.synchronize()
@@ -210,23 +280,10 @@ def run_ours(args) -> dict | None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for k in range(args.warmup):
-        step(k)
     K = args.steps
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(len(ops) + 1)] for _ in range(K)]
-    sampler = ClockSampler(local)
-    barrier()
-    launches0 = q.qdp_kernel_launch_count()
-    sampler.start()
-    for k in range(K):
-        step(k, evs[k])
-    torch.cuda.synchronize()
-    clocks = sampler.stop()
-    launches = q.qdp_kernel_launch_count() - launches0
-    barrier()
-    total_ms = evs[0][0].elapsed_time(evs[K - 1][len(ops)])
-    per_op_ms = {name: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)]))
-                 for i, (name, _) in enumerate(ops)}
+    total_ms, per_op_ms, launches = w.timed(K, args.warmup, barrier, ClockSampler(local))
+    clocks = w.clocks
+    dfma_rate = probe_dfma_rate(local, stream.cuda_stream) if rank == 0 else None
 
     # ---- rows widened beyond the step: timed separately, not part of `value` -------
     extra_ms = {}
@@ -321,33 +378,50 @@ def run_ours(args) -> dict | None:
 
     total_ms, e2e_ms = max_over_ranks([total_ms, e2e_s * 1e3], dist, f"cuda:{local}")
 
+    # ---- the other BASELINE configs that fit the time budget, same 7-op step, per-op roofline fractions only -------
+    # (parity-test configurations, not bench lines: they do not enter `value`.)
+    other = {}
+    if world == 1 and not args.no_other_configs and args.config == "C4" and prec == "f64":
+        peak_o, _ = measured_peak()
+        for cfg, pr in (("C4", "f32"), ("C3", "f64"), ("C3", "f32")):
+            wo = Workload(q, torch, cfg, pr, local, synth.BASE_SEED + 3)
+            ko = max(3, min(K, 10))
+            tot, per_op, _ = wo.timed(ko, 3)
+            other[f"{cfg}/{pr}"] = {"ms_per_step": round(tot / ko, 5), "steps": ko,
+                                    "site_updates_per_s": OPS_PER_STEP * wo.V * ko / (tot * 1e-3),
+                                    "ops": {n: {"ms": r["ms"], "frac": r["frac"]} for n, r in wo.op_report(per_op, peak_o).items()}}
+            wo.free()
+            del wo
+            torch.cuda.empty_cache()
+
     out = None
     if rank == 0:
         peak, peak_src = measured_peak()
         alg = algorithmic_bytes(V, eb)
-        op_report = {}
-        for name, ms in per_op_ms.items():
-            gbs = alg[name] / ms / 1e6
-            sites = V // 2 if name.startswith("hop_") else V
-            op_report[name] = {"ms": round(ms, 5), "gbs": round(gbs, 1), "frac": round(gbs / peak, 4),
-                               "site_updates_per_s": sites / ms * 1e3}
+        op_report = w.op_report(per_op_ms, peak)
         dom = max(per_op_ms, key=per_op_ms.get)
         dom_kernel = {"ape": "ape_kernel", "plaquette": "plaquette_kernel", "axpy_hop_norm2": "hop_kernel",
                       "hop_even": "hop_kernel", "hop_odd": "hop_kernel"}.get(dom, dom + "_kernel")
-        if dom == "ape" and prec == "f64":
-            tf = APE_FLOPS_PER_SITE_F64 * V / per_op_ms[dom] / 1e9
-            roofline = {"bound": "alu", "kernel": dom_kernel, "op": dom, "achieved": round(tf, 2),
-                        "peak": round(FP64_PEAK_TFLOPS, 2), "unit": "TFLOP/s", "frac": round(tf / FP64_PEAK_TFLOPS, 4),
-                        "peak_source": "derived: 64 fp64 FMA lanes/clk/SM x 148 SMs x 1.965 GHz x 2 (DESIGN.md section 4)",
-                        "flops_per_launch": APE_FLOPS_PER_SITE_F64 * V, "traffic": ncu_traffic(dom_kernel),
-                        "hbm": {"achieved": op_report[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                                "frac": op_report[dom]["frac"], "peak_source": peak_src,
-                                "algorithmic_bytes_per_launch": alg[dom]}}
-        else:
-            roofline = {"bound": "hbm", "kernel": dom_kernel, "op": dom,
-                        "achieved": op_report[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                        "frac": op_report[dom]["frac"], "peak_source": peak_src,
-                        "algorithmic_bytes_per_launch": alg[dom], "traffic": ncu_traffic(dom_kernel)}
+        # roofline of the dominant kernel in the metric's own unit: algorithmic bytes (SURVEY.md 8(d) per-site figure
+        # x sites of one launch) / CUDA-event time / measured HBM copy peak.  A reader can recompute frac from
+        # algorithmic_bytes_per_launch, ops[op].ms and peak.  The fp64-pipe ("alu") view of the same launch is beside it.
+        roofline = {"bound": "hbm", "kernel": dom_kernel, "op": dom,
+                    "achieved": op_report[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": op_report[dom]["frac"], "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": alg[dom], "ms_per_launch": op_report[dom]["ms"],
+                    "traffic": ncu_traffic(args.config, prec, dom_kernel)}
+        alu = {}
+        if prec == "f64" and dfma_rate:
+            for name in FP64_INSTR_PER_SITE:
+                tf = fp64_flops_per_site(name) * V / per_op_ms[name] / 1e9
+                slots = sum(FP64_INSTR_PER_SITE[name]) * V / (per_op_ms[name] * 1e-3) / dfma_rate
+                alu[name] = {"achieved": round(tf, 2), "peak": round(2 * dfma_rate / 1e12, 2), "unit": "TFLOP/s",
+                             "frac": round(tf / (2 * dfma_rate / 1e12), 4), "fp64_pipe_slots_frac": round(slots, 4),
+                             "peak_source": "measured in this run: DFMA-only kernel of csrc/probe.cu, "
+                                            f"{dfma_rate / 1e12:.2f} T DFMA/s x 2 flop",
+                             "fp64_instr_per_site": dict(zip(("dfma", "dmul", "dadd"), FP64_INSTR_PER_SITE[name]))}
+            if dom in alu:
+                roofline["alu"] = alu[dom]
         out = {
             "metric": METRIC, "value": whole_job_value(OPS_PER_STEP * V * K, world, total_ms), "unit": UNIT,
             "n_gpus": world, "steps": K, "warmup": args.warmup, "ms_per_step": total_ms / K,
@@ -370,6 +444,8 @@ def run_ours(args) -> dict | None:
             "gpu_launches": int(launches),
             "roofline": roofline,
             "ops": op_report,
+            "alu": alu,
+            "other_configs": other,
             "extra_ops": {"smear_hop": {"ms": round(extra_ms["smear_hop"], 5),
                                         "gbs": round(V * 51 * eb / extra_ms["smear_hop"] / 1e6, 1),
                                         "frac": round(V * 51 * eb / extra_ms["smear_hop"] / 1e6 / peak, 4),
@@ -480,6 +556,7 @@ def main():
     ap.add_argument("--cpu-fraction", type=int, default=1, help="cpu_baseline runs on V/fraction sites (1: one whole pass, ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the C4 f32 / C3 f64 / C3 f32 per-op block")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     out = run_reference(args) if args.impl == "reference" else run_ours(args)

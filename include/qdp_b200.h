@@ -102,6 +102,15 @@ int qdp_lattice_set_stream(qdp_lattice* lat, void* cuda_stream);
  * (SURVEY.md 8(a) rows a1, a10). */
 int qdp_lattice_set_sweep_slab(qdp_lattice* lat, int x2_extent);
 
+/* Kernel variant of qdp_plaquette and qdp_ape_smear_step: a tuning knob, results agree to rounding.
+ * on = 1: on lattices whose x0 rows tile a 32-site block (L0/2 a power of two <= 32 and
+ * L0/2 * L1 a multiple of 32, e.g. 32^3 x 64) and for the ALL subset, run the warp-specialised
+ * kernels that stage lattice tiles in shared memory with cp.async.bulk + mbarrier rings
+ * (BASELINE.json north_star: "shared-memory halo staging of a lattice tile").
+ * on = 0 (default, the faster variant as measured: DESIGN.md section 4): always run the thread-per-site kernels
+ * (the only variant on other lattices and subsets). */
+int qdp_lattice_set_staged(qdp_lattice* lat, int on);
+
 /* Replace the device allocator used by qdp_field_alloc and the library's scratch
  * buffers (default cudaMalloc/cudaFree).  alloc(bytes, ctx) returns a device
  * pointer aligned to >= 256 bytes or NULL; free_(ptr, ctx) releases it.  Lets
@@ -119,13 +128,21 @@ int qdp_lattice_neighbor_table(qdp_lattice* lat, int mu, int sign, int32_t* host
 int qdp_lattice_parity_mask(qdp_lattice* lat, uint8_t* host_out);
 int qdp_lattice_volume(const qdp_lattice* lat, int64_t* out);
 
+/* Thread safety: a lattice handle (its stream, scratch partials, result and staging buffers) and
+ * the fields on it must be used by one host thread at a time; different lattices may be driven
+ * from different threads concurrently.  Calls that return host scalars serialise on the lattice's
+ * scratch buffers by synchronising its stream.  qdp_last_error() is thread-local;
+ * qdp_kernel_launch_count() is atomic; qdp_set_allocator is process-wide (set it before threads start). */
+
 /* ---- fields -------------------------------------------------------------- */
 
 /* Allocate a field on the lattice's device (library-owned, contents undefined). */
 int qdp_field_alloc(qdp_lattice* lat, qdp_kind kind, qdp_prec prec, qdp_field** out);
 /* Wrap caller-owned device memory (e.g. a torch tensor) as a field.  `bytes` must
  * be at least qdp_field_bytes(); dev_ptr must be 256-byte aligned and must stay
- * valid until qdp_field_free, which does not free it. */
+ * valid until qdp_field_free, which does not free it.  qdp_field_free (of either kind of
+ * field) first waits for the work enqueued on the lattice's stream, so after it returns the
+ * memory may be released or reused on any stream. */
 int qdp_field_wrap(qdp_lattice* lat, qdp_kind kind, qdp_prec prec, void* dev_ptr, size_t bytes,
                    qdp_field** out);
 int qdp_field_free(qdp_field* f);
@@ -197,7 +214,10 @@ int qdp_matvec(qdp_field* chi, const qdp_field* a, int slot_a, int adj_a, const 
  *   method QDP_REUNIT_GRAM_SCHMIDT (1): row0 normalised, row1 orthogonalised against it and
  *                                       normalised, row2 = conj(row0 x row1) (cheaper, not covariant).
  * u_out, u_in: QDP_GAUGE or QDP_COLOR_MATRIX of the same kind and precision; site-local, so
- * u_out == u_in is allowed.  Arithmetic in fp64 for both precisions.  Asynchronous. */
+ * u_out == u_in is allowed.  Arithmetic in fp64 for both precisions.  Asynchronous.
+ * Conditioning: Proj is invariant under V -> c V (c > 0) and is evaluated on V / |V|_F, then
+ * polished by Newton-Schulz steps until V^dag V = 1 to ~50 ulp; the result is accurate to about
+ * cond(V) * 2^-52 per matrix for cond(V) up to ~1e5 (singular V: undefined, no error is raised). */
 enum { QDP_REUNIT_POLAR = 0, QDP_REUNIT_GRAM_SCHMIDT = 1 };
 int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset);
 

@@ -14,7 +14,7 @@ __all__ = [
     "QdpError", "Lattice", "Field", "LIB_PATH", "DECLARED_SYMBOLS",
     "QDP_ALL", "QDP_EVEN", "QDP_ODD", "QDP_F32", "QDP_F64",
     "QDP_COLOR_MATRIX", "QDP_GAUGE", "QDP_FERMION",
-    "qdp_lattice_create", "qdp_lattice_destroy", "qdp_lattice_set_stream", "qdp_lattice_set_sweep_slab", "qdp_lattice_volume",
+    "qdp_lattice_create", "qdp_lattice_destroy", "qdp_lattice_set_stream", "qdp_lattice_set_sweep_slab", "qdp_lattice_set_staged", "qdp_lattice_volume",
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
@@ -48,6 +48,7 @@ DECLARED_SYMBOLS = {
     "qdp_lattice_destroy": ([_P], _I),
     "qdp_lattice_set_stream": ([_P, _P], _I),
     "qdp_lattice_set_sweep_slab": ([_P, _I], _I),
+    "qdp_lattice_set_staged": ([_P, _I], _I),
     "qdp_set_allocator": ([_P, _P, _P], _I),
     "qdp_lattice_neighbor_table": ([_P, _I, _I, _P], _I),
     "qdp_lattice_parity_mask": ([_P, _P], _I),
@@ -152,6 +153,10 @@ def qdp_lattice_set_sweep_slab(lat: Lattice, x2_extent: int) -> None:
     _check(_lib.qdp_lattice_set_sweep_slab(lat.handle, int(x2_extent)))
 
 
+def qdp_lattice_set_staged(lat: Lattice, on: bool) -> None:
+    _check(_lib.qdp_lattice_set_staged(lat.handle, int(bool(on))))
+
+
 def qdp_lattice_sync(lat: Lattice) -> None:
     _check(_lib.qdp_lattice_sync(lat.handle))
 
@@ -221,8 +226,9 @@ def _host_ptr(f: Field, host) -> int:
             raise ValueError("host array has the wrong number of elements")
         return host.ctypes.data
     nbytes = host.numel() * host.element_size()
-    if nbytes != qdp_field_bytes(f.lat, f.kind, f.prec) or not host.is_contiguous() or host.is_cuda:
-        raise ValueError("host tensor must be a contiguous CPU tensor of the field's byte size")
+    want = int(np.prod(f.host_shape)) * np.dtype(f.host_dtype).itemsize    # host AoS size: V * ncomp complex numbers
+    if nbytes != want or not host.is_contiguous() or host.is_cuda:
+        raise ValueError(f"host tensor must be a contiguous CPU tensor of {want} bytes (V x components, array of structures)")
     return host.data_ptr()
 
 

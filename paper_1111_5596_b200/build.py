@@ -13,7 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqdp_b200.so")
-SOURCES = ["api.cu", "layout.cu", "shift.cu", "reduce.cu", "hop.cu", "plaquette.cu", "ape.cu", "reunit.cu", "matmul.cu"]
+PROBE_LIB = os.path.join(HERE, "libqdp_probe.so")   # bench-only peak probes (csrc/probe.cu), not part of the C ABI
+SOURCES = ["api.cu", "layout.cu", "shift.cu", "reduce.cu", "hop.cu", "plaquette.cu", "plaquette_tma.cu", "ape.cu", "reunit.cu", "matmul.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xptxas", "-v",
@@ -58,6 +59,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objs = [os.path.join(OBJ, s.replace(".cu", ".o")) for s in SOURCES]
     if jobs or force or not os.path.exists(LIB):
         subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    probe_src = os.path.join(CSRC, "probe.cu")
+    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < os.path.getmtime(probe_src):
+        subprocess.check_call([nvcc, *[f for f in NVCC_FLAGS if f not in ("-Xptxas", "-v")], "-shared", probe_src, "-o", PROBE_LIB])
     return LIB
 
 

@@ -164,7 +164,7 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     // partials: K <= 4 values per block (streaming reductions: at most kMaxPartialBlocks) or per
     // warp of 32 sites plus per group of kWarpGroup warps (fused kernels, reduce.cuh); qdp_sum
     // 2*36*64 values.  counters: one per group plus one.
-    const size_t nwarp_max = (size_t)l->geom.V / 32 + 64, ngroup_max = nwarp_max / kWarpGroup + 2;
+    const size_t nwarp_max = (size_t)l->geom.V / 32 + 64 + 8192 /* persistent staged kernels: warps of one CTA per SM */, ngroup_max = nwarp_max / kWarpGroup + 2;
     size_t npart = (size_t)4 * kMaxPartialBlocks;
     if (npart < 4 * (nwarp_max + ngroup_max)) npart = 4 * (nwarp_max + ngroup_max);
     if (npart < (size_t)2 * 36 * 64) npart = (size_t)2 * 36 * 64;
@@ -220,6 +220,12 @@ extern "C" int qdp_lattice_set_sweep_slab(qdp_lattice* l, int c2) {
         return fail(QDP_ERR_ARG, "qdp_lattice_set_sweep_slab: extent %d must divide L2 = %d and L0/2*L1 = %d be a multiple of 32",
                     c2, g.L2, g.s2);
     g.slab_c2 = c2; g.slab_ipr = g.s2 >> 5;
+    return QDP_OK;
+}
+
+extern "C" int qdp_lattice_set_staged(qdp_lattice* l, int on) {
+    if (!ok_lat(l)) return fail(QDP_ERR_ARG, "qdp_lattice_set_staged: not a lattice");
+    l->geom.staged = on ? 1 : 0;
     return QDP_OK;
 }
 
@@ -316,10 +322,10 @@ extern "C" int qdp_field_wrap(qdp_lattice* l, qdp_kind kind, qdp_prec prec, void
 extern "C" int qdp_field_free(qdp_field* f) {
     if (!ok_field(f)) return fail(QDP_ERR_ARG, "qdp_field_free: not a field");
     ENTER(f->lat);
-    if (f->owned) {
-        cudaStreamSynchronize(f->lat->stream);
-        dev_free(f->data, f->from_hook);
-    }
+    // Kernels enqueued on the lattice's stream may still use the memory: wait for them before the
+    // owner (this library, or the caller of qdp_field_wrap) can release or reuse it.
+    cudaStreamSynchronize(f->lat->stream);
+    if (f->owned) dev_free(f->data, f->from_hook);
     f->lat->live_fields--;
     f->magic = 0;
     delete f;
@@ -613,6 +619,6 @@ extern "C" int qdp_sum(const qdp_field* f, qdp_subset subset, double* out) {
     return fetch_result(l, 2 * f->ncomp, out);
 }
 
-extern "C" int64_t qdp_kernel_launch_count(void) { return g_launch_count; }
+extern "C" int64_t qdp_kernel_launch_count(void) { return g_launch_count.load(); }
 
 extern "C" const char* qdp_last_error(void) { return t_err; }

@@ -1,5 +1,6 @@
 // internal.h -- declarations shared by api.cu and the kernel translation units.
 #pragma once
+#include <atomic>
 #include <cstddef>
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -9,7 +10,9 @@
 
 namespace qdp {
 
-extern long long g_launch_count;   // kernels launched by this library
+extern std::atomic<long long> g_launch_count;   // kernels launched by this library (lattices may be driven from several host threads)
+// multiprocessors of the current device (cached per device)
+int device_sm_count();
 
 // All launchers enqueue on `st` and return cudaGetLastError().
 // prec: 0 = fp32, 1 = fp64 (qdp_prec).  subset: 0 all, 1 even, 2 odd.
@@ -51,9 +54,11 @@ cudaError_t launch_hop(int prec, const Geom& g, void* chi, const void* u, const 
                        bool axpy, double a, double b, bool want_norm2, const ReduceBuf& rb,
                        cudaStream_t st, int ndir = 4);
 
-// plaquette.cu
+// plaquette.cu (thread per site) and plaquette_tma.cu (shared-memory staged; ALL subset, lattices whose x0 rows tile a block)
 cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb,
                              cudaStream_t st);
+bool plaquette_tma_applicable(const Geom& g, int subset);
+cudaError_t launch_plaquette_tma(int prec, const Geom& g, const void* u, const ReduceBuf& rb, int sms, cudaStream_t st);
 
 // matmul.cu: dst slot id = op(a slot ia)(x) * op(b slot ib)(x + sign*mu); mu < 0: no shift; n* = components per site
 cudaError_t launch_matmul(int prec, const Geom& g, void* dst, int nd, int id, const void* a, int na, int ia, bool adj_a,

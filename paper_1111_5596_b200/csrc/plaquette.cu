@@ -119,13 +119,10 @@ cudaError_t launch_plaquette(int prec, const Geom& g, const void* u, int subset,
     int n = subset == 0 ? g.V : g.Vh;
     int items = subset == 0 ? 2 * g.Vhp : g.Vh;
     int grid = (items + kPlaqThreads - 1) / kPlaqThreads;
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (sms <= 0) sms = 148;
-    }
+    const int sms = device_sm_count();
+#ifndef QDP_NO_TMA_PLAQUETTE
+    if (plaquette_tma_applicable(g, subset)) return launch_plaquette_tma(prec, g, u, rb, sms, st);
+#endif
     const int per_sm = prec ? PlaqCfg<double>::kBlocks : PlaqCfg<float>::kBlocks;
     if (grid > sms * per_sm) grid = sms * per_sm;
     PlaqScale sc;

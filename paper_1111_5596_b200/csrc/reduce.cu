@@ -20,7 +20,9 @@ constexpr int kUnroll = RED_UNROLL;
 static int stream_grid(size_t n) {
     size_t per_block = (size_t)kReduceThreads * kUnroll;
     size_t b = (n + per_block - 1) / per_block;
-    if (b > (size_t)148 * RED_BLOCKS_PER_SM) b = (size_t)148 * RED_BLOCKS_PER_SM;
+    size_t cap = (size_t)device_sm_count() * RED_BLOCKS_PER_SM;
+    if (cap > (size_t)kMaxPartialBlocks) cap = kMaxPartialBlocks;   // size of the partials buffer
+    if (b > cap) b = cap;
     if (b < 1) b = 1;
     return (int)b;
 }

@@ -12,7 +12,7 @@
 namespace qdp {
 
 constexpr int kReduceThreads = 256;   // default block size of the reducing kernels
-constexpr int kMaxPartialBlocks = 148 * 16;
+constexpr int kMaxPartialBlocks = 2368;   // capacity of the partials buffer (blocks of a streaming reduction)
 
 struct ReduceBuf {
     double* partials;        // [K][number of blocks or warps], then [K][number of groups]; K <= 4

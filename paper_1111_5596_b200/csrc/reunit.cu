@@ -1,6 +1,6 @@
 // reunit.cu -- every 3x3 matrix of a field projected back to SU(3) (SURVEY.md 8(f) row f2:
 // alternative projections).  method 0: Proj(V) = polar factor times exp(-i arg(det V)/3), the
-// projection of the APE step (su3.cuh: proj_stage_a/b/c); method 1: Gram-Schmidt on rows 0, 1 and
+// projection of the APE step made robust for general matrices (su3.cuh: proj_su3_general); method 1: Gram-Schmidt on rows 0, 1 and
 // row 2 = conj(row 0 x row 1).  Site-local, so it may run in place.  One thread per (site, matrix):
 // 144 B in, 144 B out (fp64), HBM-bound for Gram-Schmidt (~90 fp64 instructions per matrix).
 // Arithmetic in fp64 for both field precisions.
@@ -54,10 +54,7 @@ __global__ void __launch_bounds__(256) reunit_kernel(Geom g, int ncomp, typename
     }
     Mat3<double> W;
     if (METHOD == 0) {
-        ProjScalars ps[1];
-        proj_stage_a(V, ps[0]);
-        proj_stage_b<1>(ps);
-        W = proj_stage_c(V, ps[0]);
+        W = proj_su3_general(V);
     } else {
         W = gram_schmidt_su3(V);
     }

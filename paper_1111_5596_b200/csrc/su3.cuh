@@ -2,10 +2,10 @@
 // vectors, field loads/stores in the site-fastest SoA layout, and the SU(3)
 // projection.  (8(c) definitions 2-5.)
 //
-// Device field layout: component plane c holds V complex
-// numbers, dev[c*V + s], s the internal site index, complex = (re, im) adjacent:
-// fp64 -> one double2 = one 128-bit access per thread, a warp moves 512
-// contiguous bytes per plane; fp32 -> float2, 256 contiguous bytes per warp.
+// Device field layout (geom.cuh): blocked site-fastest structure of arrays,
+// element(c, s) = ((s >> 5) * ncomp + c) * 32 + (s & 31), s the internal site index, complex =
+// (re, im) adjacent: fp64 -> one double2 = one 128-bit access per thread, a warp moves 512
+// contiguous bytes per component; fp32 -> float2, 256 contiguous bytes per warp.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -96,20 +96,6 @@ __device__ __forceinline__ Spinor<T> ld_spinor(const typename Vec2<T>::type* __r
     return r;
 }
 
-// Read back what this thread stored earlier in the kernel.  An ordinary load would let the
-// compiler forward the stored registers to the use and keep them live in between, which is
-// exactly what parking a value in memory is meant to avoid.
-__device__ __forceinline__ double2 ld_parked(const double2* p) {
-    double2 v;
-    asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
-    return v;
-}
-__device__ __forceinline__ float2 ld_parked(const float2* p) {
-    float2 v;
-    asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
-    return v;
-}
-
 // ---- matrix algebra --------------------------------------------------------
 template <class T> __device__ __forceinline__ Mat3<T> mat_zero() {
     Mat3<T> r;
@@ -159,13 +145,6 @@ template <class T> __device__ __forceinline__ void mad_mul(Mat3<T>& acc, const M
         for (int j = 0; j < 3; j++)
 #pragma unroll
             for (int k = 0; k < 3; k++) cmad(acc.e[i * 3 + j], a.e[i * 3 + k], b.e[k * 3 + j]);
-}
-// Re tr(A * B^dag) = sum_ij Re(A_ij conj(B_ij))
-template <class T> __device__ __forceinline__ T re_tr_mul_adj(const Mat3<T>& a, const Mat3<T>& b) {
-    T s = 0;
-#pragma unroll
-    for (int i = 0; i < 9; i++) { s = fma(a.e[i].re, b.e[i].re, s); s = fma(a.e[i].im, b.e[i].im, s); }
-    return s;
 }
 template <class T> __device__ __forceinline__ Cx<T> det(const Mat3<T>& a) {
     Cx<T> c0 = a.e[4] * a.e[8] - a.e[5] * a.e[7];
@@ -356,6 +335,43 @@ __device__ __forceinline__ Mat3<double> proj_stage_c(const Mat3<double>& V, cons
     R.e[2] = r02 * z; R.e[6] = conj(r02) * z;
     R.e[5] = r12 * z; R.e[7] = conj(r12) * z;
     return mul(V, R);
+}
+
+// Proj for general 3x3 matrices (qdp_reunitarize): the closed form above assumes SU(3)-scaled, moderately conditioned
+// input (the blended links of an APE step: cond(V) <= ~11 on hot fields).  Proj is invariant under V -> c V, c > 0, so
+// V is first scaled to Frobenius norm sqrt(3) (the fp32 seeds then cannot overflow or underflow), and the result X is
+// polished by Newton-Schulz steps X <- X (3 - X^dag X)/2 while max |X^dag X - 1| exceeds ~50 ulp (at most four).
+// X = V p(H) z has the polar factor of V times z for every positive polynomial p of H = V^dag V, so the steps remove
+// the error an ill-conditioned V leaves in the coefficients f0, f1, f2 without changing what X converges to.
+// Supported range: cond(V) up to ~1e5 (beyond that the closed form's error exceeds the Newton-Schulz basin).
+__device__ __forceinline__ Mat3<double> proj_su3_general(Mat3<double> V) {
+    double n2 = 0;
+#pragma unroll
+    for (int c = 0; c < 9; c++) n2 = fma(V.e[c].re, V.e[c].re, fma(V.e[c].im, V.e[c].im, n2));
+    const double sc = 1.7320508075688772 / sqrt(n2);
+#pragma unroll
+    for (int c = 0; c < 9; c++) V.e[c] = cx<double>(V.e[c].re * sc, V.e[c].im * sc);
+    ProjScalars ps[1];
+    proj_stage_a(V, ps[0]);
+    proj_stage_b<1>(ps);
+    Mat3<double> X = proj_stage_c(V, ps[0]);
+    for (int it = 0; it < 4; it++) {
+        Mat3<double> M;      // (3 - X^dag X) / 2
+        double r = 0;
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int j = 0; j < 3; j++) {
+                Cx<double> y = cx<double>(0, 0);
+#pragma unroll
+                for (int k = 0; k < 3; k++) cmad_conj_a(y, X.e[k * 3 + i], X.e[k * 3 + j]);
+                r = fmax(r, fmax(fabs(y.re - (i == j ? 1.0 : 0.0)), fabs(y.im)));
+                M.e[i * 3 + j] = cx<double>((i == j ? 1.5 : 0.0) - 0.5 * y.re, -0.5 * y.im);
+            }
+        if (!(r > 1e-14)) break;
+        X = mul(X, M);
+    }
+    return X;
 }
 
 // ---- fp32 projection for fp32 fields -------------------------------------------------------------

@@ -77,17 +77,28 @@ def _check_step(qdp, dims, prec, seed, n_ape_steps=1, warm=False):
     assert np.abs(g @ np.conj(np.swapaxes(g, 1, 2)) - np.eye(3)).max() <= unit_bar
     assert np.abs(np.linalg.det(g) - 1).max() <= unit_bar
 
-    # ---- further APE steps (ping-pong, A16): plaquette rises, links stay in SU(3)
+    # ---- further APE steps (ping-pong, A16): plaquette rises, links stay in SU(3); the last step is compared
+    # with the oracle on the sampled sites, restarted from the downloaded field of the step before it
     if n_ape_steps > 1:
         bufs = [u2, qdp.qdp_field_alloc(lat, 1, _prec_id(prec))]
         prev = qdp.qdp_plaquette(bufs[0])[1]
-        for _ in range(n_ape_steps - 1):
+        for k in range(n_ape_steps - 1):
+            last = k == n_ape_steps - 2
+            if last:
+                before = _as64(qdp.field_to_host(bufs[0]))
             qdp.qdp_ape_smear_step(bufs[1], bufs[0], 0.5, 3)
             bufs.reverse()
             cur = qdp.qdp_plaquette(bufs[0])[1]
             assert cur > prev
             prev = cur
-        g = _as64(qdp.field_to_host(bufs[0])[sites, :3]).reshape(-1, 3, 3)
+        got_last = qdp.field_to_host(bufs[0])
+        for mu in range(3):
+            want = np.stack([oracle.ape_site(dims, before, int(s), mu, 0.5, 3) for s in sites])
+            fixed, n_centre = z3_fix(_as64(got_last[sites, mu]), want)
+            assert n_centre == 0
+            assert site_rel_err(fixed, want).max() <= TOL_SITE[prec], ("last APE step", mu)
+        assert np.array_equal(got_last[:, 3], hu[:, 3])
+        g = _as64(got_last[sites, :3]).reshape(-1, 3, 3)
         assert np.abs(g @ np.conj(np.swapaxes(g, 1, 2)) - np.eye(3)).max() <= unit_bar
         assert np.abs(np.linalg.det(g) - 1).max() <= unit_bar
 
@@ -157,31 +168,35 @@ def test_c3_sweep_and_normalised_iteration(qdp, prec):
     _check_step(qdp, dims, prec, seed, warm=True)
     lat = qdp.qdp_lattice_create(dims)
     hu = synth.round_to(synth.gauge_hot(dims, seed), prec)
-    hp = synth.round_to(synth.spinor(dims, seed, 1), prec)
     a, b = synth.scalars_ab(seed)
     u = qdp.field_from_host(lat, 1, hu)
-    bufs = [qdp.field_from_host(lat, 2, hp), qdp.qdp_field_alloc(lat, 2, _prec_id(prec))]
-    ref, u64 = _as64(hp), _as64(hu)
-    scale = 1.0
-    norms = []
-    for k in range(50):
-        ak, bk = a * scale, b * scale
-        if prec == "f32":
-            ak, bk = float(np.float32(ak)), float(np.float32(bk))
-        n_k = qdp.qdp_axpy_hop(bufs[1], ak, bk, u, bufs[0], 0, want_norm2=True)
-        bufs.reverse()
-        norms.append(n_k)
-        if k < 3:
-            ref = oracle.axpy_hop(dims, ak, bk, u64, ref)
-            got = _as64(qdp.field_to_host(bufs[0]))
-            assert site_rel_err(got, ref).max() <= (k + 1) * TOL_SITE[prec], k
-            assert abs(n_k - oracle.norm2(dims, ref)) <= TOL_SUM[prec] * n_k
-            ref = got          # continue the oracle from the device field: per-step error, not drift
-        scale = 1.0 / np.sqrt(n_k)
-    norms = np.array(norms)
-    assert np.all(np.isfinite(norms)) and np.all(norms > 0)
-    # after the first step psi has unit norm: n_k <= (|a| + 8 |b|)^2 (||hop|| <= 8)
-    assert np.all(norms[1:] <= (abs(a) + 8 * abs(b)) ** 2 * (1 + 1e-6))
+    u64 = _as64(hu)
+    for ispinor in range(1, 5):          # reading A14: four independent spinor fields, the same (a, b)
+        hp = synth.round_to(synth.spinor(dims, seed, ispinor), prec)
+        bufs = [qdp.field_from_host(lat, 2, hp), qdp.qdp_field_alloc(lat, 2, _prec_id(prec))]
+        ref = _as64(hp)
+        scale = 1.0
+        norms = []
+        for k in range(50):
+            ak, bk = a * scale, b * scale
+            if prec == "f32":
+                ak, bk = float(np.float32(ak)), float(np.float32(bk))
+            n_k = qdp.qdp_axpy_hop(bufs[1], ak, bk, u, bufs[0], 0, want_norm2=True)
+            bufs.reverse()
+            norms.append(n_k)
+            if k < (3 if ispinor == 1 else 1):
+                ref = oracle.axpy_hop(dims, ak, bk, u64, ref)
+                got = _as64(qdp.field_to_host(bufs[0]))
+                assert site_rel_err(got, ref).max() <= (k + 1) * TOL_SITE[prec], (ispinor, k)
+                assert abs(n_k - oracle.norm2(dims, ref)) <= TOL_SUM[prec] * n_k
+                ref = got          # continue the oracle from the device field: per-step error, not drift
+            scale = 1.0 / np.sqrt(n_k)
+        norms = np.array(norms)
+        assert np.all(np.isfinite(norms)) and np.all(norms > 0)
+        # after the first step psi has unit norm: n_k <= (|a| + 8 |b|)^2 (||hop|| <= 8)
+        assert np.all(norms[1:] <= (abs(a) + 8 * abs(b)) ** 2 * (1 + 1e-6))
+        for f in bufs:
+            qdp.qdp_field_free(f)
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])

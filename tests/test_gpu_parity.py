@@ -457,9 +457,13 @@ def test_reunitarize(qdp, lat_cache, dims, prec):
     unit_bar = 1e-12 if prec == "f64" else 1e-5
     for kind, host in ((1, hg), (0, hm)):
         src = qdp.field_from_host(lat, kind, host)
+        h64 = links(_as64(host))
+        # conditioning-scaled bar: the polar factor of V moves by ~cond(V) eps under a
+        # relative perturbation eps of V, so the per-matrix bar is the north-star bar times max(1, cond(V)/10)
+        # (blended APE links have cond <= ~11); cond from the oracle's smallest eigenvalue of V^dag V.
+        lam_min = np.array([oracle.min_eig_vdv(m) for m in h64])
+        cond = np.sqrt((np.abs(h64) ** 2).sum(axis=(1, 2)) / lam_min)
         for method in (qdp.QDP_REUNIT_POLAR, qdp.QDP_REUNIT_GRAM_SCHMIDT):
-            if kind == 0 and method == qdp.QDP_REUNIT_POLAR and prec == "f32":
-                continue      # Gaussian 3x3 matrices can be arbitrarily ill conditioned: no fp32 bar for Proj
             for sub in SUBSETS:
                 sentinel = np.full_like(host, 3.0 - 2.0j)
                 dst = qdp.field_from_host(lat, kind, sentinel)
@@ -467,14 +471,26 @@ def test_reunitarize(qdp, lat_cache, dims, prec):
                 got = qdp.field_to_host(dst)
                 want = oracle.reunitarize(dims, _as64(host), method, sub, out=_as64(sentinel))
                 fixed, n_centre = z3_fix(links(_as64(got)), links(want))
-                tol = TOL_SITE[prec] * (1 if kind == 1 else 50)     # general matrices: cond up to ~50
-                assert site_rel_err(fixed, links(want)).max() <= tol, (kind, method, sub)
+                tol = TOL_SITE[prec] * np.maximum(1.0, cond / 10.0)
+                assert np.all(site_rel_err(fixed, links(want)) <= tol), (kind, method, sub)
                 assert n_centre == 0 or method == qdp.QDP_REUNIT_POLAR
             work = qdp.field_from_host(lat, kind, host)            # in place, whole lattice
             qdp.qdp_reunitarize(work, work, method)
             g = links(_as64(qdp.field_to_host(work)))
-            assert np.abs(g @ np.conj(np.swapaxes(g, 1, 2)) - np.eye(3)).max() <= unit_bar * (1 if kind == 1 else 50)
-            assert np.abs(np.linalg.det(g) - 1).max() <= unit_bar * (1 if kind == 1 else 50)
+            # the output itself is unitary to working precision whatever the conditioning of the input
+            assert np.abs(g @ np.conj(np.swapaxes(g, 1, 2)) - np.eye(3)).max() <= unit_bar
+            assert np.abs(np.linalg.det(g) - 1).max() <= unit_bar
+    # scale invariance of Proj and badly scaled input (the fp32 seeds of the closed form must not overflow)
+    if prec == "f64":
+        for scale in (1e-9, 1e7):
+            src = qdp.field_from_host(lat, 0, hm * scale)
+            dst = qdp.qdp_field_alloc(lat, 0, P)
+            qdp.qdp_reunitarize(dst, src, qdp.QDP_REUNIT_POLAR)
+            want = oracle.reunitarize(dims, _as64(hm), qdp.QDP_REUNIT_POLAR)
+            fixed, _ = z3_fix(links(_as64(qdp.field_to_host(dst))), links(want))
+            lam_min = np.array([oracle.min_eig_vdv(m) for m in links(_as64(hm))])
+            cond = np.sqrt((np.abs(links(_as64(hm))) ** 2).sum(axis=(1, 2)) / lam_min)
+            assert np.all(site_rel_err(fixed, links(want)) <= TOL_SITE[prec] * np.maximum(1.0, cond / 10.0)), scale
     psi = qdp.qdp_field_alloc(lat, 2, P)
     with pytest.raises(qdp.QdpError):
         qdp.qdp_reunitarize(psi, psi, 0)
@@ -661,3 +677,72 @@ def test_inner_timeslices_gamma(qdp, lat_cache, dims, prec):
     with pytest.raises(qdp.QdpError):
         m = qdp.qdp_field_alloc(lat, 0, 1 if prec == "f64" else 0)
         qdp.qdp_inner_timeslices_gamma(m, m, 5)
+
+
+def test_pinned_host_tensor_on_a_ragged_lattice(qdp):
+    """Upload/download through a pinned torch host tensor on 2^4, where V/2 = 8 is not a multiple of 32 and the
+    padded device size (qdp_field_bytes) is four times the host array-of-structures size: the binding must ask
+    for the host size."""
+    import torch
+    dims = (2, 2, 2, 2)
+    lat = qdp.qdp_lattice_create(dims)
+    hp = synth.spinor(dims, 77)
+    f = qdp.qdp_field_alloc(lat, 2, 1)
+    host = torch.from_numpy(hp.copy()).pin_memory()
+    assert host.numel() * host.element_size() * 4 == qdp.qdp_field_bytes(lat, 2, 1)
+    qdp.qdp_field_upload(f, host)
+    back = torch.empty_like(host).pin_memory()
+    qdp.qdp_field_download(f, back)
+    assert np.array_equal(back.numpy(), hp)
+    assert abs(qdp.qdp_norm2(f) - oracle.norm2(dims, hp)) <= 1e-12 * oracle.norm2(dims, hp)
+    with pytest.raises(ValueError):
+        qdp.qdp_field_upload(f, torch.zeros(qdp.qdp_field_bytes(lat, 2, 1), dtype=torch.uint8))
+
+
+def test_gamma_basis_one_hot(qdp):
+    """Pins single entries of Gamma(n) on the device against the literal DeGrand-Rossi matrices (typed in here from
+    include/qdp_b200.h): with a = e_{s'} and b = e_s one-hot in spin at one site, a^dag Gamma b = Gamma[s', s]."""
+    I = 1j
+    lit = {1: [[0, 0, 0, I], [0, 0, I, 0], [0, -I, 0, 0], [-I, 0, 0, 0]],
+           2: [[0, 0, 0, -1], [0, 0, 1, 0], [0, 1, 0, 0], [-1, 0, 0, 0]],
+           4: [[0, 0, I, 0], [0, 0, 0, -I], [-I, 0, 0, 0], [0, I, 0, 0]],
+           8: [[0, 0, 1, 0], [0, 0, 0, 1], [1, 0, 0, 0], [0, 1, 0, 0]],
+           15: [[1, 0, 0, 0], [0, 1, 0, 0], [0, 0, -1, 0], [0, 0, 0, -1]]}
+    dims = (2, 2, 2, 4)
+    lat = qdp.qdp_lattice_create(dims)
+    V = synth.volume(dims)
+    site, t = 5, 5 // 8          # lex 5 lies on time-slice 0
+    for n, G in lit.items():
+        G = np.array(G, dtype=complex)
+        got = np.zeros((4, 4), dtype=complex)
+        for sp in range(4):
+            for s in range(4):
+                ha = np.zeros((V, 4, 3), dtype=np.complex128)
+                hb = np.zeros((V, 4, 3), dtype=np.complex128)
+                ha[site, sp, 1] = 1.0
+                hb[site, s, 1] = 1.0
+                a, b = qdp.field_from_host(lat, 2, ha), qdp.field_from_host(lat, 2, hb)
+                got[sp, s] = qdp.qdp_inner_timeslices_gamma(a, b, n)[t]
+        assert np.array_equal(got, G), n
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (16, 16, 16, 32), (64, 8, 4, 4), (4, 16, 8, 8), (2, 32, 4, 6), (32, 4, 2, 2)])
+@pytest.mark.parametrize("prec", PRECS)
+def test_staged_kernels_match_thread_per_site_kernels(qdp, dims, prec):
+    """qdp_lattice_set_staged: on lattices whose x0 rows tile a 32-site block the shared-memory-staged kernels
+    (cp.async.bulk + mbarrier rings) and the thread-per-site kernels evaluate the same definitions; both are
+    compared with the oracle, and with each other to summation-order accuracy."""
+    hu = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 91), prec)
+    want = oracle.plaquette(dims, _as64(hu))
+    res = []
+    for staged in (True, False):
+        lat = qdp.qdp_lattice_create(dims)
+        qdp.qdp_lattice_set_staged(lat, staged)
+        u = qdp.field_from_host(lat, 1, hu)
+        before = qdp.qdp_kernel_launch_count()
+        pg = qdp.qdp_plaquette(u)
+        assert qdp.qdp_kernel_launch_count() == before + 1
+        assert np.abs(pg - want).max() <= (1e-10 if prec == "f64" else 1e-5)
+        assert np.array_equal(pg, qdp.qdp_plaquette(u))          # deterministic
+        res.append(pg)
+    assert np.abs(res[0] - res[1]).max() <= (1e-12 if prec == "f64" else 1e-5)

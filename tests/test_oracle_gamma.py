@@ -7,6 +7,30 @@ import synth
 from npref import view4
 
 
+# The four Euclidean gamma matrices of the DeGrand-Rossi basis (QDP++'s convention), typed in as numbers from the
+# statement of the convention in include/qdp_b200.h (qdp_inner_timeslices_gamma); rows = s', columns = s.
+# The Clifford/Hermiticity pins below hold in every Hermitian representation; this one fixes the basis itself
+# (a sign flip of one matrix or a swap of two fails it).
+I = 1j
+DEGRAND_ROSSI = {
+    0: [[0, 0, 0, I], [0, 0, I, 0], [0, -I, 0, 0], [-I, 0, 0, 0]],
+    1: [[0, 0, 0, -1], [0, 0, 1, 0], [0, 1, 0, 0], [-1, 0, 0, 0]],
+    2: [[0, 0, I, 0], [0, 0, 0, -I], [-I, 0, 0, 0], [0, I, 0, 0]],
+    3: [[0, 0, 1, 0], [0, 0, 0, 1], [1, 0, 0, 0], [0, 1, 0, 0]],
+}
+# gamma_5 = g0 g1 g2 g3 in this basis is diagonal (chiral basis): multiplied out by hand
+GAMMA5_DIAG = [1, 1, -1, -1]
+
+
+def test_basis_is_the_literal_degrand_rossi_matrices():
+    for mu in range(4):
+        assert np.array_equal(oracle.gamma_matrix(1 << mu), np.array(DEGRAND_ROSSI[mu], dtype=complex)), mu
+    assert np.array_equal(oracle.gamma_matrix(15), np.diag(GAMMA5_DIAG).astype(complex))
+    # a composite one: g0 g1 = diag(-i, i, -i, i)
+    g01 = np.array(DEGRAND_ROSSI[0], dtype=complex) @ np.array(DEGRAND_ROSSI[1], dtype=complex)
+    assert np.array_equal(oracle.gamma_matrix(3), g01)
+
+
 def test_clifford_algebra_hermiticity_and_gamma5():
     g = [oracle.gamma_matrix(1 << mu) for mu in range(4)]
     eye = np.eye(4)
