@@ -1,6 +1,6 @@
 """Build libqdp_b200.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_1111_5596_b200.build [--force] [--verbose]
+    python -m paper_1111_5596_b200.build [--force] [--verbose] [--bounds-check]
 """
 from __future__ import annotations
 
@@ -34,20 +34,28 @@ def _deps_mtime() -> float:
     return max(os.path.getmtime(h) for h in hdrs)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    os.makedirs(OBJ, exist_ok=True)
+BC_LIB = os.path.join(HERE, "libqdp_b200_bc.so")    # the same library compiled with -DQDP_BOUNDS_CHECK (su3.cuh: site_ptr_checked)
+
+
+def build(force: bool = False, verbose: bool = False, bounds_check: bool = False) -> str:
+    """bounds_check: build libqdp_b200_bc.so, every site address validated on the device (tests/test_gpu_bounds.py
+    runs the small-lattice parity suite against it through QDP_B200_LIB)."""
+    obj_dir = OBJ + "_bc" if bounds_check else OBJ
+    lib = BC_LIB if bounds_check else LIB
+    flags = NVCC_FLAGS + (["-DQDP_BOUNDS_CHECK"] if bounds_check else [])
+    os.makedirs(obj_dir, exist_ok=True)
     nvcc = _nvcc()
     hdr_t = _deps_mtime()
     jobs = []
     for src in SOURCES:
         s = os.path.join(CSRC, src)
-        o = os.path.join(OBJ, src.replace(".cu", ".o"))
+        o = os.path.join(obj_dir, src.replace(".cu", ".o"))
         if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr_t):
             jobs.append((s, o))
 
     def compile_one(job):
         s, o = job
-        r = subprocess.run([nvcc, *NVCC_FLAGS, "-c", s, "-o", o], capture_output=True, text=True)
+        r = subprocess.run([nvcc, *flags, "-c", s, "-o", o], capture_output=True, text=True)
         return s, r
 
     with ThreadPoolExecutor(max_workers=min(8, max(1, len(jobs)))) as ex:
@@ -56,9 +64,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 sys.stderr.write(f"== {os.path.basename(s)}\n{r.stdout}{r.stderr}\n")
             if r.returncode:
                 raise RuntimeError(f"nvcc failed on {s}")
-    objs = [os.path.join(OBJ, s.replace(".cu", ".o")) for s in SOURCES]
-    if jobs or force or not os.path.exists(LIB):
-        subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    objs = [os.path.join(obj_dir, s.replace(".cu", ".o")) for s in SOURCES]
+    if jobs or force or not os.path.exists(lib):
+        subprocess.check_call([nvcc, "-shared", "-o", lib, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    if bounds_check:
+        return lib
     probe_src = os.path.join(CSRC, "probe.cu")
     if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < os.path.getmtime(probe_src):
         subprocess.check_call([nvcc, *[f for f in NVCC_FLAGS if f not in ("-Xptxas", "-v")], "-shared", probe_src, "-o", PROBE_LIB])
@@ -66,4 +76,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, bounds_check="--bounds-check" in sys.argv))

@@ -8,6 +8,7 @@
 
 #include "../../include/qdp_b200.h"
 #include "internal.h"
+#include "su3.cuh"
 
 using namespace qdp;
 
@@ -618,6 +619,27 @@ extern "C" int qdp_sum(const qdp_field* f, qdp_subset subset, double* out) {
     CUDA_TRY(launch_sum(f->prec, l->geom, f->ncomp, f->data, subset, l->partials, l->result_dev, l->stream));
     return fetch_result(l, 2 * f->ncomp, out);
 }
+
+#ifdef QDP_BOUNDS_CHECK
+// Only in the bounds-checked build (not declared in the header): three deliberately wrong site addresses
+// (past the end, a padding lane of a ragged lattice or the last real site + 1, a component outside the
+// site) so that tests/test_gpu_bounds.py can see the checker fire.
+namespace qdp {
+__global__ void bounds_selftest_kernel(Geom g, double2* f) {
+    volatile double2* a = site_ptr(f, 12, 0, 2 * g.Vhp);
+    volatile double2* b = site_ptr(f, 12, 0, g.Vhp + g.Vh);
+    volatile double2* c = site_ptr(f, 12, 12, 0);
+    (void)a; (void)b; (void)c;
+}
+}  // namespace qdp
+extern "C" int qdp_bc_selftest(qdp_field* f) {
+    if (!ok_field(f) || f->kind != QDP_FERMION || f->prec != QDP_F64) return QDP_ERR_ARG;
+    ENTER(f->lat);
+    qdp::bounds_selftest_kernel<<<1, 1, 0, f->lat->stream>>>(f->lat->geom, (double2*)f->data);
+    CUDA_TRY(cudaStreamSynchronize(f->lat->stream));
+    return QDP_OK;
+}
+#endif
 
 extern "C" int64_t qdp_kernel_launch_count(void) { return g_launch_count.load(); }
 

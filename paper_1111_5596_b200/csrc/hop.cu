@@ -24,8 +24,8 @@ __device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
                                         const typename Vec2<T>::type* __restrict__ psi, Spinor<T>& acc) {
     {   // forward: U_mu(x) psi(x+mu)
         const int sf = site_step<MU, +1>(g, x).index(g);
-        Mat3<T> U = ld_mat<T>(u, 36, MU, s);
-        Spinor<T> p = ld_spinor<T>(psi, sf);
+        Mat3<T> U = ld_mat_at<T>(site_ptr(u, 36, MU * 9, s));
+        Spinor<T> p = ld_spinor_at<T>(site_ptr(psi, 12, 0, sf));
 #pragma unroll
         for (int sp = 0; sp < 4; sp++)
 #pragma unroll
@@ -35,8 +35,8 @@ __device__ __forceinline__ void hop_dir(const Geom& g, const Site& x, int s,
     }
     {   // backward: U_mu(x-mu)^dag psi(x-mu)
         const int sb = site_step<MU, -1>(g, x).index(g);
-        Mat3<T> U = ld_mat<T>(u, 36, MU, sb);
-        Spinor<T> p = ld_spinor<T>(psi, sb);
+        Mat3<T> U = ld_mat_at<T>(site_ptr(u, 36, MU * 9, sb));
+        Spinor<T> p = ld_spinor_at<T>(site_ptr(psi, 12, 0, sb));
 #pragma unroll
         for (int sp = 0; sp < 4; sp++)
 #pragma unroll
@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(kHopThreads, HopCfg<T>::kBlocks) hop_kernel(Ge
         hop_dir<T, 2>(g, x, s, u, psi, acc);
         if (NDIR == 4) hop_dir<T, 3>(g, x, s, u, psi, acc);
         if (AXPY) {
-            Spinor<T> p = ld_spinor<T>(psi, s);
+            Spinor<T> p = ld_spinor_at<T>(site_ptr(psi, 12, 0, s));
 #pragma unroll
             for (int c = 0; c < 12; c++) {
                 // a*psi + b*hop: two roundings per part, like the definition

@@ -165,6 +165,10 @@ plaquette_tma_kernel(PlaqTmaGeo pg, const typename Vec2<T>::type* __restrict__ u
                         mbar_wait(&sm.own_empty[s], ((own_item / kPtOwnSlots) & 1) ^ 1);
                         mbar_arrive_expect_tx(&sm.own_full[s], 2 * S::kGaugeBytes);
                         const int jb = j == pg.P ? 0 : j;   // the x1 wrap: the plane's first pair again
+#ifdef QDP_BOUNDS_CHECK
+                        if (q * pg.P + jb >= pg.nblk_half || q2 * pg.P + pg.P > pg.nblk_half || q3 * pg.P + pg.P > pg.nblk_half)
+                            printf("QDP_BOUNDS plaquette_tma: plane %d/%d/%d block %d of %d\n", q, q2, q3, jb, pg.nblk_half);
+#endif
                         for (int p = 0; p < 2; p++)
                             bulk_g2s(sm.own[s][p], u + (size_t)(p * pg.nblk_half + q * pg.P + jb) * S::kGauge, S::kGaugeBytes,
                                      &sm.own_full[s]);

@@ -7,7 +7,9 @@
 // (re, im) adjacent: fp64 -> one double2 = one 128-bit access per thread, a warp moves 512
 // contiguous bytes per component; fp32 -> float2, 256 contiguous bytes per warp.
 #pragma once
+#include <cstdio>
 #include <cuda_runtime.h>
+#include "geom.cuh"
 
 namespace qdp {
 
@@ -56,9 +58,28 @@ template <class T> struct Spinor {
 constexpr int kLane = 32;   // sites per block
 
 template <class T2>
-__device__ __forceinline__ T2* site_ptr(T2* f, int ncomp, int c0, int s) {
+__device__ __forceinline__ T2* site_ptr_raw(T2* f, int ncomp, int c0, int s) {
     return f + ((size_t)(s >> 5) * ncomp + c0) * kLane + (s & 31);
 }
+#ifdef QDP_BOUNDS_CHECK
+// Bounds-checked build (python -m paper_1111_5596_b200.build --bounds-check -> libqdp_b200_bc.so; compute-sanitizer is
+// closed on this GPU pool): every site address is validated against the lattice in scope (`g`): the site index
+// must be a real site of one of the two parity halves (not a padding lane) and the first component must lie inside
+// the site.  A violation is reported through device printf ("QDP_BOUNDS ...") and the access is redirected to site 0,
+// so the run continues without an illegal access and tests/test_gpu_bounds.py can count the reports.
+template <class T2>
+__device__ __noinline__ T2* site_ptr_checked(const Geom& g, T2* f, int ncomp, int c0, int s, int line) {
+    const int hs = s >= g.Vhp ? s - g.Vhp : s;
+    if (s < 0 || s >= 2 * g.Vhp || hs >= g.Vh || c0 < 0 || c0 >= ncomp) {
+        printf("QDP_BOUNDS line %d: site %d (Vhp %d, Vh %d) component %d of %d\n", line, s, g.Vhp, g.Vh, c0, ncomp);
+        s = 0; c0 = 0;
+    }
+    return site_ptr_raw(f, ncomp, c0, s);
+}
+#define site_ptr(f, ncomp, c0, s) ::qdp::site_ptr_checked(g, (f), (ncomp), (c0), (s), __LINE__)
+#else
+#define site_ptr(f, ncomp, c0, s) ::qdp::site_ptr_raw((f), (ncomp), (c0), (s))
+#endif
 // 3x3 matrix whose first component is at p
 template <class T>
 __device__ __forceinline__ Mat3<T> ld_mat_at(const typename Vec2<T>::type* __restrict__ p) {
@@ -79,14 +100,9 @@ __device__ __forceinline__ void st_mat_at(typename Vec2<T>::type* __restrict__ p
         p[c * kLane] = o;
     }
 }
-// colour matrix number `m` of a field with ncomp components (gauge: 36, m = mu; colour matrix: 9, m = 0)
+// spinor whose first component is at p
 template <class T>
-__device__ __forceinline__ Mat3<T> ld_mat(const typename Vec2<T>::type* __restrict__ f, int ncomp, int m, int s) {
-    return ld_mat_at<T>(site_ptr(f, ncomp, m * 9, s));
-}
-template <class T>
-__device__ __forceinline__ Spinor<T> ld_spinor(const typename Vec2<T>::type* __restrict__ f, int s) {
-    const typename Vec2<T>::type* p = site_ptr(f, 12, 0, s);
+__device__ __forceinline__ Spinor<T> ld_spinor_at(const typename Vec2<T>::type* __restrict__ p) {
     Spinor<T> r;
 #pragma unroll
     for (int c = 0; c < 12; c++) {
