@@ -54,6 +54,9 @@ def _get():
             "orc_matvec": ([P, P, P, I, I, I, P, I, I, I], None),
             "orc_matmul": ([P, P, I, I, P, I, I, I, P, I, I, I, I, I, I], None),
             "orc_reunitarize": ([P, I, P, P, I, I], None),
+            "orc_trace_mul": ([P, P, P, I, I, I, P, I, I, I, I, I, I], None),
+            "orc_staple_field": ([P, P, I, I, I, P], None),
+            "orc_ape_blend_field": ([P, P, I, D, I, I, P], None),
             "orc_staple_site": ([P, P, Z, I, I, P], I),
             "orc_ape_blend_site": ([P, P, Z, I, D, I, P], None),
             "orc_ape_site": ([P, P, Z, I, D, I, P], None),
@@ -166,6 +169,33 @@ def matvec(dims, a, ia, adj_a, psi, mu=-1, sign=1, subset=ALL, chi=None):
     _get().orc_matvec(_dims(dims), out.ctypes.data, a.ctypes.data, a.size // (9 * volume(dims)), ia, int(adj_a),
                       psi.ctypes.data, mu, sign, subset)
     return out
+
+
+def trace_mul(dims, a, ia, adj_a, b, ib, adj_b, mu=-1, sign=1, subset=ALL, out=None):
+    """out(x) = tr[op(a[:, ia])(x) @ op(b[:, ib])(x + sign*mu)] on the subset, [V] complex128 (row f1: `trace`;
+    `real` of it is .real); fields are [V,3,3] (index 0) or [V,4,3,3]."""
+    a, b = _c128(a), _c128(b)
+    V = volume(dims)
+    res = np.zeros(V, dtype=np.complex128) if out is None else _c128(out).copy()
+    _get().orc_trace_mul(_dims(dims), res.ctypes.data, a.ctypes.data, a.size // (9 * V), ia, int(adj_a),
+                         b.ctypes.data, b.size // (9 * V), ib, int(adj_b), mu, sign, subset)
+    return res
+
+
+def staple_field(dims, u, mu, t_dir=3, subset=ALL, out=None):
+    """out(x) = S_mu(x), the staple sum around link mu (def. 3), as a colour-matrix field [V,3,3]."""
+    u = _c128(u)
+    res = np.zeros((volume(dims), 3, 3), dtype=np.complex128) if out is None else _c128(out).copy()
+    _get().orc_staple_field(_dims(dims), u.ctypes.data, mu, t_dir, subset, res.ctypes.data)
+    return res
+
+
+def ape_blend_field(dims, u, mu, alpha, t_dir=3, subset=ALL, out=None):
+    """out(x) = (1-alpha) U_mu(x) + (alpha/n) S_mu(x): the APE link before projection, [V,3,3]."""
+    u = _c128(u)
+    res = np.zeros((volume(dims), 3, 3), dtype=np.complex128) if out is None else _c128(out).copy()
+    _get().orc_ape_blend_field(_dims(dims), u.ctypes.data, mu, alpha, t_dir, subset, res.ctypes.data)
+    return res
 
 
 def gram_schmidt_su3(V):

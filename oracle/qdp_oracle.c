@@ -327,6 +327,28 @@ void orc_matvec(const int *L, double *chi, const double *A, int na, int ia, int 
     }
 }
 
+/* ---- trace / real and the whole-field forms used by the expression layer ("adj, trace, real,
+ * colour-matrix x colour-matrix on arbitrary fields, shift of leaves"; expressions that look like
+ * their mathematical counterparts, evaluated site by site without temporaries) -----------------------------------
+ *   orc_trace_mul:       out(x) = tr[ opA(A(x)) opB(B(x + sign*mu)) ]   one complex number per site, x in subset;
+ *                        real(...) of it is the .re member (the QDP++ `real`), taken by the caller.
+ *   orc_staple_field:    out(x) = S_mu(x) of orc_staple_site, a colour-matrix field, x in subset.
+ *   orc_ape_blend_field: out(x) = (1-alpha) U_mu(x) + (alpha/n) S_mu(x), x in subset.
+ * Sites outside the subset keep their previous contents of `out`. */
+void orc_trace_mul(const int *L, double *out, const double *A, int na, int ia, int adj_a,
+                   const double *B, int nb, int ib, int adj_b, int mu, int sign, int subset) {
+    for (size_t s = 0; s < volume(L); s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        size_t sbn = mu < 0 ? s : hop_lex(L, x, mu, sign);
+        const cplx *a = (const cplx *)A + (s * na + ia) * 9, *b = (const cplx *)B + (sbn * nb + ib) * 9;
+        cplx ta[9], tb[9], r[9];
+        if (adj_a) m_adj(a, ta); else memcpy(ta, a, sizeof ta);
+        if (adj_b) m_adj(b, tb); else memcpy(tb, b, sizeof tb);
+        m_mul(ta, tb, r);
+        ((cplx *)out)[s] = m_trace(r);
+    }
+}
 /* ---- reunitarisation of whole fields (alternative projections) ----------
  * Gram-Schmidt: row0 = v0/|v0|; row1 = v1 - (row0 . v1) row0, normalised, with (a . b) = sum_j conj(a_j) b_j;
  * row2 = conj(row0 x row1).  The result is in SU(3) by construction; unlike Proj it is not gauge
@@ -438,6 +460,22 @@ void orc_ape_site(const int *L, const double *u, size_t lex, int mu, double alph
     double V[18];
     orc_ape_blend_site(L, u, lex, mu, alpha, t_dir, V);
     orc_proj_su3(V, out18);
+}
+
+/* whole-field forms of the two functions above (expression layer, row f1; see orc_trace_mul) */
+void orc_staple_field(const int *L, const double *u, int mu, int t_dir, int subset, double *out) {
+    for (size_t s = 0; s < volume(L); s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        orc_staple_site(L, u, s, mu, t_dir, out + s * 18);
+    }
+}
+void orc_ape_blend_field(const int *L, const double *u, int mu, double alpha, int t_dir, int subset, double *out) {
+    for (size_t s = 0; s < volume(L); s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        orc_ape_blend_site(L, u, s, mu, alpha, t_dir, out + s * 18);
+    }
 }
 
 void orc_ape_smear_step_range(const int *L, const double *u_in, double *u_out, double alpha,
