@@ -286,13 +286,33 @@ def run_ours(args) -> dict | None:
     dfma_rate = probe_dfma_rate(local, stream.cuda_stream) if rank == 0 else None
 
     # ---- rows widened beyond the step: timed separately, not part of `value` -------
+    # name -> (call, complex numbers moved per site (algorithmic), note)
+    cm = q.qdp_field_alloc(lat, q.QDP_COLOR_MATRIX, P)
+    extra_defs = {
+        "smear_hop": (lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3), 51,
+                      "qdp_smear_hop, t_dir = 3 (row f2): u 27 + psi 12 + chi 12 complex per site"),
+        "inner_timeslices": (lambda: q.qdp_inner_timeslices(psi, chi), 24,
+                             "qdp_inner_timeslices (row f3): 2 x 12 complex per site, includes the host round trip"),
+        "reunitarize_gs": (lambda: q.qdp_reunitarize(u2, u, q.QDP_REUNIT_GRAM_SCHMIDT), 60,
+                           "qdp_reunitarize, Gram-Schmidt (row f2): 24 complex read (rows 0, 1 of four links; row 2 is "
+                           "not an input) + 36 written per site"),
+        "matmul": (lambda: q.qdp_matmul(u2, 0, u, 0, 0, u, 1, 1, 0, 1), 27,
+                   "qdp_matmul u2[0] = u[0] * adj(u[1])(x+0) (row f1): 2 x 9 complex read + 9 written per site"),
+        "axpby": (lambda: q.qdp_axpby(sh, a, psi, b, chi), 36,
+                  "qdp_axpby on spinors (PAPER.md:96): 2 x 12 complex read + 12 written per site"),
+        "expr_plaquette": (lambda: q.qdp_expr_plaquette(u), 36,
+                           "qdp_expr_plaquette (row f1): the plaquette written as one expression of the compile-time "
+                           "layer, one kernel; compare ops.plaquette (hand-fused)"),
+        "expr_staple": (lambda: q.qdp_expr_staple(cm, u, 0, 3), 36,
+                        "qdp_expr_staple mu = 0, spatial (row f1): the staple sum as one expression; 27 complex read "
+                        "(three links) + 9 written per site"),
+        "plaquette_staged": (None, 36, "qdp_plaquette with qdp_lattice_set_staged(1): cp.async.bulk + mbarrier "
+                                       "shared-memory rings (plaquette_tma.cu); compare ops.plaquette"),
+    }
     extra_ms = {}
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    for name, fn in (("smear_hop", lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3)),
-                     ("inner_timeslices", lambda: q.qdp_inner_timeslices(psi, chi)),
-                     ("reunitarize_gs", lambda: q.qdp_reunitarize(u2, u, q.QDP_REUNIT_GRAM_SCHMIDT)),
-                     ("matmul", lambda: q.qdp_matmul(u2, 0, u, 0, 0, u, 1, 1, 0, 1)),
-                     ("axpby", lambda: q.qdp_axpby(sh, a, psi, b, chi))):
+
+    def time_extra(fn):
         for _ in range(3):
             fn()
         ev0.record(stream)
@@ -300,7 +320,15 @@ def run_ours(args) -> dict | None:
             fn()
         ev1.record(stream)
         torch.cuda.synchronize()
-        extra_ms[name] = ev0.elapsed_time(ev1) / K
+        return ev0.elapsed_time(ev1) / K
+
+    for name, (fn, _, _) in extra_defs.items():
+        if fn is not None:
+            extra_ms[name] = time_extra(fn)
+    q.qdp_lattice_set_staged(lat, True)
+    extra_ms["plaquette_staged"] = time_extra(lambda: q.qdp_plaquette(u))
+    q.qdp_lattice_set_staged(lat, False)
+    q.qdp_field_free(cm)
 
     # ---- end to end through the C ABI from pinned host buffers ----------------------
     ke = max(1, min(args.e2e_steps, K))
@@ -446,31 +474,11 @@ def run_ours(args) -> dict | None:
             "ops": op_report,
             "alu": alu,
             "other_configs": other,
-            "extra_ops": {"smear_hop": {"ms": round(extra_ms["smear_hop"], 5),
-                                        "gbs": round(V * 51 * eb / extra_ms["smear_hop"] / 1e6, 1),
-                                        "frac": round(V * 51 * eb / extra_ms["smear_hop"] / 1e6 / peak, 4),
-                                        "note": "qdp_smear_hop, t_dir = 3 (row f2): u 27 + psi 12 + chi 12 complex per site; "
-                                                "not part of the step"},
-                          "inner_timeslices": {"ms": round(extra_ms["inner_timeslices"], 5),
-                                               "gbs": round(V * 24 * eb / extra_ms["inner_timeslices"] / 1e6, 1),
-                                               "frac": round(V * 24 * eb / extra_ms["inner_timeslices"] / 1e6 / peak, 4),
-                                               "note": "qdp_inner_timeslices (row f3): 2 x 12 complex per site, includes the "
-                                                       "host round trip; not part of the step"},
-                          "reunitarize_gs": {"ms": round(extra_ms["reunitarize_gs"], 5),
-                                             "gbs": round(V * 60 * eb / extra_ms["reunitarize_gs"] / 1e6, 1),
-                                             "frac": round(V * 60 * eb / extra_ms["reunitarize_gs"] / 1e6 / peak, 4),
-                                             "note": "qdp_reunitarize, Gram-Schmidt (row f2): 24 complex read (rows 0, 1 of four "
-                                                     "links; row 2 is not an input) + 36 written per site; not part of the step"},
-                          "matmul": {"ms": round(extra_ms["matmul"], 5),
-                                     "gbs": round(V * 27 * eb / extra_ms["matmul"] / 1e6, 1),
-                                     "frac": round(V * 27 * eb / extra_ms["matmul"] / 1e6 / peak, 4),
-                                     "note": "qdp_matmul u2[0] = u[0] * adj(u[1])(x+0) (row f1): 2 x 9 complex read + 9 written "
-                                             "per site; not part of the step"},
-                          "axpby": {"ms": round(extra_ms["axpby"], 5),
-                                    "gbs": round(V * 36 * eb / extra_ms["axpby"] / 1e6, 1),
-                                    "frac": round(V * 36 * eb / extra_ms["axpby"] / 1e6 / peak, 4),
-                                    "note": "qdp_axpby on spinors (PAPER.md:96): 2 x 12 complex read + 12 written per site; "
-                                            "not part of the step"}},
+            "extra_ops": {name: {"ms": round(extra_ms[name], 5),
+                                 "gbs": round(V * nc * eb / extra_ms[name] / 1e6, 1),
+                                 "frac": round(V * nc * eb / extra_ms[name] / 1e6 / peak, 4),
+                                 "note": note + "; not part of the step"}
+                          for name, (_, nc, note) in extra_defs.items()},
             "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
         }
         if world == 1 and not args.no_cpu_baseline:

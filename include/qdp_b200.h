@@ -32,6 +32,7 @@
  *         QDP_COLOR_MATRIX  host[(lex*3 + row)*3 + col]
  *         QDP_GAUGE         host[((lex*4 + mu)*3 + row)*3 + col]
  *         QDP_FERMION       host[(lex*4 + spin)*3 + colour]
+ *         QDP_COMPLEX       host[lex]
  *     (U psi)_row = sum_col U[row][col] psi[col].
  *   - Subsets: parity(x) = (x0+x1+x2+x3) & 1; QDP_EVEN = parity 0.  An operation
  *     under a subset writes only the subset's sites of its destination (all
@@ -71,7 +72,10 @@ typedef enum { QDP_F32 = 0, QDP_F64 = 1 } qdp_prec;
 typedef enum {
     QDP_COLOR_MATRIX = 0,  /* 3x3 complex per site (9 complex)          */
     QDP_GAUGE = 1,         /* 4 colour matrices per site (36 complex)   */
-    QDP_FERMION = 2        /* 4 spin x 3 colour per site (12 complex)   */
+    QDP_FERMION = 2,       /* 4 spin x 3 colour per site (12 complex)   */
+    QDP_COMPLEX = 3        /* one complex number per site: the value of trace(...) in the expression layer.
+                              Supported by alloc/wrap/free/bytes/upload/download/copy, qdp_sum and as the
+                              destination of qdp_expr_trace_mul; every other call returns QDP_ERR_KIND. */
 } qdp_kind;
 
 typedef struct qdp_lattice qdp_lattice;   /* opaque */
@@ -277,6 +281,35 @@ int qdp_inner_timeslices(const qdp_field* a, const qdp_field* b, qdp_subset subs
  * With a, b columns of quark propagators this is the building block of meson two-point functions
  * (HAD stage).  n = 0 equals qdp_inner_timeslices.  Synchronous. */
 int qdp_inner_timeslices_gamma(const qdp_field* a, const qdp_field* b, int n, qdp_subset subset, double* out);
+
+/* ---- the expression layer ---------------------------------------------
+ * The paper turns every QDP++ expression (PETE expression templates, "expressions that look like their
+ * mathematical counterparts") into one generated kernel.  Here the
+ * expression is a C++ type built with *, +, adj, trace, real, shift (csrc/expr.cuh) and nvcc
+ * instantiates ONE kernel per expression at build time, with an optional fused global sum; no
+ * temporaries, no JIT.  The calls below are named instantiations; their definitions are the same as
+ * those of the hand-fused calls above (def. 2, def. 3 of SURVEY.md 8(c)).
+ *
+ *   qdp_expr_plaquette:  sum_x real(trace(u[mu] * shift(u[nu],+mu) * adj(shift(u[mu],+nu)) * adj(u[nu]))) summed over
+ *                        the six planes in one kernel; out[3] normalised exactly as qdp_plaquette.  Synchronous.
+ *   qdp_expr_staple:     dst(x) = sum_{nu != mu, nu != t_dir} [ u[nu] * shift(u[mu],+nu) * adj(shift(u[nu],+mu))
+ *                                 + shift(adj(u[nu]) * u[mu] * shift(u[nu],+mu), -nu) ](x), x in subset: the staple sum
+ *                        S_mu of def. 3 (t_dir = 3: spatial, 4 staples; -1: all directions, 6).  dst: QDP_COLOR_MATRIX,
+ *                        u: QDP_GAUGE, same lattice and precision; mu must be a smeared direction.  Asynchronous.
+ *   qdp_expr_ape_blend:  dst = (1-alpha) * u[mu] + (alpha/n) * S_mu, n = 4 or 6: the APE link before projection
+ *                        (qdp_reunitarize(dst, dst, QDP_REUNIT_POLAR) then gives the link of qdp_ape_smear_step).
+ *   qdp_expr_trace_mul:  dst(x) = trace(opA(a[slot_a])(x) * opB(b[slot_b])(x + sign*mu)), dst: QDP_COMPLEX; slots, op and
+ *                        mu = -1 (no shift) as in qdp_matmul.  Asynchronous.
+ *   qdp_expr_sum_trace_mul: out = (re, im) of sum_{x in subset} of that trace (fp64 accumulation, fixed order); with
+ *                        a = u', b = u, adj_b = 1 it is the link overlap sum tr(U' U^dag) used to monitor smearing.
+ *                        Synchronous. */
+int qdp_expr_plaquette(const qdp_field* u, qdp_subset subset, double out[3]);
+int qdp_expr_staple(qdp_field* dst, const qdp_field* u, int mu, int t_dir, qdp_subset subset);
+int qdp_expr_ape_blend(qdp_field* dst, const qdp_field* u, int mu, double alpha, int t_dir, qdp_subset subset);
+int qdp_expr_trace_mul(qdp_field* dst, const qdp_field* a, int slot_a, int adj_a, const qdp_field* b, int slot_b,
+                       int adj_b, int mu, int sign, qdp_subset subset);
+int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a, const qdp_field* b, int slot_b, int adj_b,
+                           int mu, int sign, qdp_subset subset, double out[2]);
 
 /* Block the host until every call enqueued on the lattice's stream has finished. */
 int qdp_lattice_sync(qdp_lattice* lat);

@@ -13,21 +13,21 @@ import numpy as np
 __all__ = [
     "QdpError", "Lattice", "Field", "LIB_PATH", "DECLARED_SYMBOLS",
     "QDP_ALL", "QDP_EVEN", "QDP_ODD", "QDP_F32", "QDP_F64",
-    "QDP_COLOR_MATRIX", "QDP_GAUGE", "QDP_FERMION",
+    "QDP_COLOR_MATRIX", "QDP_GAUGE", "QDP_FERMION", "QDP_COMPLEX",
     "qdp_lattice_create", "qdp_lattice_destroy", "qdp_lattice_set_stream", "qdp_lattice_set_sweep_slab", "qdp_lattice_set_staged", "qdp_lattice_volume",
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
-    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_matmul", "qdp_matvec", "qdp_axpby", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
+    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_matmul", "qdp_matvec", "qdp_axpby", "qdp_expr_plaquette", "qdp_expr_staple", "qdp_expr_ape_blend", "qdp_expr_trace_mul", "qdp_expr_sum_trace_mul", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
 ]
 
 QDP_ALL, QDP_EVEN, QDP_ODD = 0, 1, 2
 QDP_F32, QDP_F64 = 0, 1
-QDP_COLOR_MATRIX, QDP_GAUGE, QDP_FERMION = 0, 1, 2
-_NCOMP = {QDP_COLOR_MATRIX: 9, QDP_GAUGE: 36, QDP_FERMION: 12}
-_SHAPE = {QDP_COLOR_MATRIX: (3, 3), QDP_GAUGE: (4, 3, 3), QDP_FERMION: (4, 3)}
+QDP_COLOR_MATRIX, QDP_GAUGE, QDP_FERMION, QDP_COMPLEX = 0, 1, 2, 3
+_NCOMP = {QDP_COLOR_MATRIX: 9, QDP_GAUGE: 36, QDP_FERMION: 12, QDP_COMPLEX: 1}
+_SHAPE = {QDP_COLOR_MATRIX: (3, 3), QDP_GAUGE: (4, 3, 3), QDP_FERMION: (4, 3), QDP_COMPLEX: ()}
 
 # QDP_B200_LIB selects another build of the same library (e.g. a debug or tuning build)
 LIB_PATH = os.environ.get("QDP_B200_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libqdp_b200.so")
@@ -72,6 +72,11 @@ DECLARED_SYMBOLS = {
     "qdp_axpby": ([_P, _D, _P, _D, _P, _I, _P], _I),
     "qdp_matvec": ([_P, _P, _I, _I, _P, _I, _I, _I], _I),
     "qdp_matmul": ([_P, _I, _P, _I, _I, _P, _I, _I, _I, _I, _I], _I),
+    "qdp_expr_plaquette": ([_P, _I, ctypes.POINTER(_D)], _I),
+    "qdp_expr_staple": ([_P, _P, _I, _I, _I], _I),
+    "qdp_expr_ape_blend": ([_P, _P, _I, _D, _I, _I], _I),
+    "qdp_expr_trace_mul": ([_P, _P, _I, _I, _P, _I, _I, _I, _I, _I], _I),
+    "qdp_expr_sum_trace_mul": ([_P, _I, _I, _P, _I, _I, _I, _I, _I, ctypes.POINTER(_D)], _I),
     "qdp_norm2": ([_P, _I, _P], _I),
     "qdp_inner": ([_P, _P, _I, _P], _I),
     "qdp_sum": ([_P, _I, _P], _I),
@@ -286,6 +291,35 @@ def qdp_matmul(dst: Field, slot_d: int, a: Field, slot_a: int, adj_a: bool, b: F
     """dst[slot_d](x) = op(a[slot_a])(x) @ op(b[slot_b])(x + sign*mu); mu = -1: no shift."""
     _check(_lib.qdp_matmul(dst.handle, slot_d, a.handle, slot_a, int(bool(adj_a)), b.handle, slot_b, int(bool(adj_b)),
                            mu, sign, subset))
+
+
+def qdp_expr_plaquette(u: Field, subset: int = QDP_ALL) -> np.ndarray:
+    """The plaquette as one expression kernel (row f1); same normalisation as qdp_plaquette."""
+    out = (_D * 3)()
+    _check(_lib.qdp_expr_plaquette(u.handle, subset, out))
+    return np.array(out[:], dtype=np.float64)
+
+
+def qdp_expr_staple(dst: Field, u: Field, mu: int, t_dir: int = 3, subset: int = QDP_ALL) -> None:
+    _check(_lib.qdp_expr_staple(dst.handle, u.handle, mu, t_dir, subset))
+
+
+def qdp_expr_ape_blend(dst: Field, u: Field, mu: int, alpha: float, t_dir: int = 3, subset: int = QDP_ALL) -> None:
+    _check(_lib.qdp_expr_ape_blend(dst.handle, u.handle, mu, float(alpha), t_dir, subset))
+
+
+def qdp_expr_trace_mul(dst: Field, a: Field, slot_a: int, adj_a: bool, b: Field, slot_b: int, adj_b: bool,
+                       mu: int = -1, sign: int = 1, subset: int = QDP_ALL) -> None:
+    _check(_lib.qdp_expr_trace_mul(dst.handle, a.handle, slot_a, int(bool(adj_a)), b.handle, slot_b, int(bool(adj_b)),
+                                   mu, sign, subset))
+
+
+def qdp_expr_sum_trace_mul(a: Field, slot_a: int, adj_a: bool, b: Field, slot_b: int, adj_b: bool,
+                           mu: int = -1, sign: int = 1, subset: int = QDP_ALL) -> complex:
+    out = (_D * 2)()
+    _check(_lib.qdp_expr_sum_trace_mul(a.handle, slot_a, int(bool(adj_a)), b.handle, slot_b, int(bool(adj_b)), mu, sign,
+                                       subset, out))
+    return complex(out[0], out[1])
 
 
 def qdp_reunitarize(u_out: Field, u_in: Field, method: int = QDP_REUNIT_POLAR, subset: int = QDP_ALL) -> None:

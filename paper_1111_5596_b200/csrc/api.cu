@@ -87,6 +87,7 @@ static int kind_ncomp(int kind) {
         case QDP_COLOR_MATRIX: return 9;
         case QDP_GAUGE: return 36;
         case QDP_FERMION: return 12;
+        case QDP_COMPLEX: return 1;
         default: return 0;
     }
 }
@@ -409,6 +410,7 @@ extern "C" int qdp_shift(qdp_field* dst, const qdp_field* src, int mu, int sign,
     int rc = check_pair("qdp_shift", dst, src);
     if (rc != QDP_OK) return rc;
     if (dst->kind != src->kind) return fail(QDP_ERR_KIND, "qdp_shift: kinds differ");
+    if (dst->kind == QDP_COMPLEX) return fail(QDP_ERR_KIND, "qdp_shift: not available for QDP_COMPLEX fields");
     if (overlaps(dst, src)) return fail(QDP_ERR_ALIAS, "qdp_shift: dst aliases src");
     ENTER(dst->lat);
     CUDA_TRY(launch_shift(dst->prec, dst->lat->geom, dst->ncomp, dst->data, src->data, mu, sign, subset, dst->lat->stream));
@@ -528,6 +530,7 @@ extern "C" int qdp_smear_hop(qdp_field* chi, double a, double b, const qdp_field
 
 extern "C" int qdp_norm2(const qdp_field* f, qdp_subset subset, double* out) {
     if (!ok_field(f) || !out || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_norm2: bad argument");
+    if (f->kind == QDP_COMPLEX) return fail(QDP_ERR_KIND, "qdp_norm2: not available for QDP_COMPLEX fields (use qdp_sum)");
     qdp_lattice* l = f->lat;
     ENTER(l);
     CUDA_TRY(launch_norm2(f->prec, l->geom, f->ncomp, f->data, subset, reduce_buf(l), l->stream));
@@ -539,6 +542,7 @@ extern "C" int qdp_inner(const qdp_field* a, const qdp_field* b, qdp_subset subs
     int rc = check_pair("qdp_inner", a, b);
     if (rc != QDP_OK) return rc;
     if (a->kind != b->kind) return fail(QDP_ERR_KIND, "qdp_inner: kinds differ");
+    if (a->kind == QDP_COMPLEX) return fail(QDP_ERR_KIND, "qdp_inner: not available for QDP_COMPLEX fields");
     qdp_lattice* l = a->lat;
     ENTER(l);
     CUDA_TRY(launch_inner(a->prec, l->geom, a->ncomp, a->data, b->data, subset, reduce_buf(l), l->stream));
@@ -552,6 +556,7 @@ extern "C" int qdp_axpby(qdp_field* dst, double a, const qdp_field* x, double b,
     if (rc == QDP_OK) rc = check_pair("qdp_axpby", dst, y);
     if (rc != QDP_OK) return rc;
     if (dst->kind != x->kind || dst->kind != y->kind) return fail(QDP_ERR_KIND, "qdp_axpby: kinds differ");
+    if (dst->kind == QDP_COMPLEX) return fail(QDP_ERR_KIND, "qdp_axpby: not available for QDP_COMPLEX fields");
     if ((overlaps(dst, x) && dst->data != x->data) || (overlaps(dst, y) && dst->data != y->data))
         return fail(QDP_ERR_ALIAS, "qdp_axpby: dst partially overlaps an operand");
     qdp_lattice* l = dst->lat;
@@ -601,6 +606,7 @@ static int inner_timeslices_common(const char* who, const qdp_field* a, const qd
     int rc = check_pair(who, a, b);
     if (rc != QDP_OK) return rc;
     if (a->kind != b->kind) return fail(QDP_ERR_KIND, "%s: kinds differ", who);
+    if (a->kind == QDP_COMPLEX) return fail(QDP_ERR_KIND, "%s: not available for QDP_COMPLEX fields", who);
     qdp_lattice* l = a->lat;
     ENTER(l);
     const int L3 = l->geom.L3;
@@ -618,6 +624,68 @@ extern "C" int qdp_sum(const qdp_field* f, qdp_subset subset, double* out) {
     ENTER(l);
     CUDA_TRY(launch_sum(f->prec, l->geom, f->ncomp, f->data, subset, l->partials, l->result_dev, l->stream));
     return fetch_result(l, 2 * f->ncomp, out);
+}
+
+// ---- the expression layer (csrc/expr.cuh, expr.cu): named instantiations --------------------------
+extern "C" int qdp_expr_plaquette(const qdp_field* u, qdp_subset subset, double out[3]) {
+    if (!ok_field(u) || !out || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_expr_plaquette: bad argument");
+    if (u->kind != QDP_GAUGE) return fail(QDP_ERR_KIND, "qdp_expr_plaquette: u must be a gauge field");
+    qdp_lattice* l = u->lat;
+    ENTER(l);
+    CUDA_TRY(launch_expr_plaquette(u->prec, l->geom, u->data, subset, reduce_buf(l), l->stream));
+    double r[2];
+    int rc = fetch_result(l, 2, r);
+    if (rc != QDP_OK) return rc;
+    out[0] = 0.5 * (r[0] + r[1]); out[1] = r[0]; out[2] = r[1];
+    return QDP_OK;
+}
+
+static int expr_staple_common(const char* who, qdp_field* dst, const qdp_field* u, int mu, int t_dir, bool blend, double alpha,
+                              qdp_subset subset) {
+    if (!ok_field(dst) || !ok_field(u) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "%s: bad argument", who);
+    if (t_dir != 3 && t_dir != -1) return fail(QDP_ERR_ARG, "%s: t_dir must be 3 or -1", who);
+    if (mu < 0 || mu > 3 || mu == t_dir) return fail(QDP_ERR_ARG, "%s: mu must be a smeared direction", who);
+    int rc = check_pair(who, dst, u);
+    if (rc != QDP_OK) return rc;
+    if (dst->kind != QDP_COLOR_MATRIX || u->kind != QDP_GAUGE) return fail(QDP_ERR_KIND, "%s: dst colour matrix, u gauge field", who);
+    qdp_lattice* l = u->lat;
+    ENTER(l);
+    CUDA_TRY(launch_expr_staple(u->prec, l->geom, dst->data, u->data, mu, t_dir, blend, alpha, subset, l->stream));
+    return QDP_OK;
+}
+extern "C" int qdp_expr_staple(qdp_field* dst, const qdp_field* u, int mu, int t_dir, qdp_subset subset) {
+    return expr_staple_common("qdp_expr_staple", dst, u, mu, t_dir, false, 0.0, subset);
+}
+extern "C" int qdp_expr_ape_blend(qdp_field* dst, const qdp_field* u, int mu, double alpha, int t_dir, qdp_subset subset) {
+    return expr_staple_common("qdp_expr_ape_blend", dst, u, mu, t_dir, true, alpha, subset);
+}
+
+static int expr_trace_mul_common(const char* who, qdp_field* dst, const qdp_field* a, int slot_a, int adj_a, const qdp_field* b,
+                                 int slot_b, int adj_b, int mu, int sign, qdp_subset subset, double* out) {
+    if (!ok_field(a) || !ok_field(b) || !ok_subset(subset) || (dst && !ok_field(dst)) || (!dst && !out))
+        return fail(QDP_ERR_ARG, "%s: bad argument", who);
+    if (mu > 3 || (mu >= 0 && sign != 1 && sign != -1)) return fail(QDP_ERR_ARG, "%s: mu must be -1..3, sign +-1", who);
+    int rc = check_pair(who, a, b);
+    if (rc == QDP_OK && dst) rc = check_pair(who, dst, a);
+    if (rc != QDP_OK) return rc;
+    auto matrix_kind = [](const qdp_field* f) { return f->kind == QDP_COLOR_MATRIX || f->kind == QDP_GAUGE; };
+    if (!matrix_kind(a) || !matrix_kind(b) || (dst && dst->kind != QDP_COMPLEX))
+        return fail(QDP_ERR_KIND, "%s: a, b colour matrices or gauge fields, dst QDP_COMPLEX", who);
+    if (slot_a < 0 || slot_a >= a->ncomp / 9 || slot_b < 0 || slot_b >= b->ncomp / 9) return fail(QDP_ERR_ARG, "%s: slot out of range", who);
+    qdp_lattice* l = a->lat;
+    ENTER(l);
+    CUDA_TRY(launch_expr_trace_mul(a->prec, l->geom, dst ? dst->data : nullptr, a->data, a->ncomp, slot_a, adj_a != 0, b->data,
+                                   b->ncomp, slot_b, adj_b != 0, mu, sign, subset, reduce_buf(l), l->stream));
+    return dst ? QDP_OK : fetch_result(l, 2, out);
+}
+extern "C" int qdp_expr_trace_mul(qdp_field* dst, const qdp_field* a, int slot_a, int adj_a, const qdp_field* b, int slot_b,
+                                  int adj_b, int mu, int sign, qdp_subset subset) {
+    if (!dst) return fail(QDP_ERR_ARG, "qdp_expr_trace_mul: bad argument");
+    return expr_trace_mul_common("qdp_expr_trace_mul", dst, a, slot_a, adj_a, b, slot_b, adj_b, mu, sign, subset, nullptr);
+}
+extern "C" int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a, const qdp_field* b, int slot_b, int adj_b,
+                                      int mu, int sign, qdp_subset subset, double out[2]) {
+    return expr_trace_mul_common("qdp_expr_sum_trace_mul", nullptr, a, slot_a, adj_a, b, slot_b, adj_b, mu, sign, subset, out);
 }
 
 #ifdef QDP_BOUNDS_CHECK

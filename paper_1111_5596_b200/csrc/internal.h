@@ -72,6 +72,13 @@ cudaError_t launch_matvec(int prec, const Geom& g, void* chi, const void* a, int
 cudaError_t launch_reunit(int prec, const Geom& g, int ncomp, void* out, const void* in, int method, int subset,
                           cudaStream_t st);
 
+// expr.cu: named instantiations of the compile-time expression layer (expr.cuh)
+cudaError_t launch_expr_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb, cudaStream_t st);
+cudaError_t launch_expr_staple(int prec, const Geom& g, void* dst, const void* u, int mu, int t_dir, bool blend, double alpha,
+                               int subset, cudaStream_t st);
+cudaError_t launch_expr_trace_mul(int prec, const Geom& g, void* dst, const void* A, int na, int ia, bool adj_a, const void* B,
+                                  int nb, int ib, bool adj_b, int mu, int sign, int subset, const ReduceBuf& rb, cudaStream_t st);
+
 // ape.cu
 cudaError_t launch_ape(int prec, const Geom& g, void* u_out, const void* u_in, double alpha, int t_dir,
                        int subset, cudaStream_t st);

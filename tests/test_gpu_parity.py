@@ -746,3 +746,79 @@ def test_staged_kernels_match_thread_per_site_kernels(qdp, dims, prec):
         assert np.array_equal(pg, qdp.qdp_plaquette(u))          # deterministic
         res.append(pg)
     assert np.abs(res[0] - res[1]).max() <= (1e-12 if prec == "f64" else 1e-5)
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_expression_layer(qdp, lat_cache, dims, prec):
+    """Row f1: the named instantiations of the compile-time expression layer (csrc/expr.cuh).  Each expression is ONE
+    kernel; values against the oracle's definitions (def. 2, def. 3, trace/real) and against the hand-fused calls."""
+    lat = lat_cache(dims)
+    P = 1 if prec == "f64" else 0
+    V = synth.volume(dims)
+    hu = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 101), prec)
+    hm = synth.round_to(synth.color_matrix(dims, _seed(dims) + 102), prec)
+    u, m = qdp.field_from_host(lat, 1, hu), qdp.field_from_host(lat, 0, hm)
+    u64, m64 = _as64(hu), _as64(hm)
+    tol = TOL_SITE[prec]
+    # ---- sum(real(trace(u[mu] * shift(u[nu],mu) * adj(shift(u[mu],nu)) * adj(u[nu])))): the plaquette
+    for sub in SUBSETS:
+        n0 = qdp.qdp_kernel_launch_count()
+        got = qdp.qdp_expr_plaquette(u, sub)
+        assert qdp.qdp_kernel_launch_count() == n0 + 1
+        bar = 1e-10 if prec == "f64" else 1e-5
+        assert np.abs(got - oracle.plaquette(dims, u64, sub)).max() <= bar, sub
+        assert np.abs(got - qdp.qdp_plaquette(u, sub)).max() <= bar
+    # ---- the staple sum and the APE blend as one expression each
+    for t_dir in (3, -1):
+        for mu in range(3 if t_dir == 3 else 4):
+            for sub in SUBSETS if mu == 0 else [0]:
+                sentinel = np.full_like(hm, 1.0 - 2.0j)
+                dst = qdp.field_from_host(lat, 0, sentinel)
+                n0 = qdp.qdp_kernel_launch_count()
+                qdp.qdp_expr_staple(dst, u, mu, t_dir, sub)
+                assert qdp.qdp_kernel_launch_count() == n0 + 1
+                want = oracle.staple_field(dims, u64, mu, t_dir, sub, out=_as64(sentinel))
+                assert site_rel_err(_as64(qdp.field_to_host(dst)), want).max() <= tol, (t_dir, mu, sub)
+            dst = qdp.qdp_field_alloc(lat, 0, P)
+            qdp.qdp_expr_ape_blend(dst, u, mu, 0.5, t_dir)
+            want = oracle.ape_blend_field(dims, u64, mu, 0.5, t_dir)
+            assert site_rel_err(_as64(qdp.field_to_host(dst)), want).max() <= tol, (t_dir, mu)
+        # Proj of the blend = the link of the fused APE step (def. 3-4)
+        qdp.qdp_reunitarize(dst, dst, qdp.QDP_REUNIT_POLAR)
+        u2 = qdp.qdp_field_alloc(lat, 1, P)
+        qdp.qdp_ape_smear_step(u2, u, 0.5, t_dir)
+        mu_last = 2 if t_dir == 3 else 3
+        fixed, _ = z3_fix(links(_as64(qdp.field_to_host(dst))), links(_as64(qdp.field_to_host(u2)[:, mu_last])))
+        assert site_rel_err(fixed, links(_as64(qdp.field_to_host(u2)[:, mu_last]))).max() <= 4 * tol
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_expr_staple(qdp.qdp_field_alloc(lat, 0, P), u, 3, 3)         # mu = t_dir is not smeared
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_expr_staple(u2, u, 0, 3)                                     # dst must be a colour matrix
+    # ---- trace(opA(a) * opB(shift(b))) into a QDP_COMPLEX field, and its fused sum
+    scale = np.sqrt(oracle.norm2(dims, m64) * 3 / V) * 3
+    for adj_a in (0, 1):
+        for adj_b in (0, 1):
+            for mu, sign in ((-1, 1), (0, 1), (1, -1), (2, 1), (3, -1)):
+                for sub in SUBSETS if (adj_a, adj_b, mu) == (0, 1, 0) else [0]:
+                    sentinel = np.full(V, 5.0 + 1.0j, dtype=hm.dtype)
+                    dst = qdp.field_from_host(lat, qdp.QDP_COMPLEX, sentinel)
+                    qdp.qdp_expr_trace_mul(dst, u, 1, adj_a, m, 0, adj_b, mu, sign, sub)
+                    want = oracle.trace_mul(dims, u64, 1, adj_a, m64, 0, adj_b, mu, sign, sub, out=_as64(sentinel))
+                    got = _as64(qdp.field_to_host(dst))
+                    assert np.abs(got - want).max() <= tol * scale, (adj_a, adj_b, mu, sign, sub)
+                    live = want != _as64(sentinel)
+                    s = qdp.qdp_expr_sum_trace_mul(u, 1, adj_a, m, 0, adj_b, mu, sign, sub)
+                    assert abs(s - want[live].sum()) <= TOL_SUM[prec] * scale * live.sum()
+    # trace(u u^dag) = 3 on SU(3) links: the link overlap of a field with itself is 3 V
+    assert abs(qdp.qdp_expr_sum_trace_mul(u, 2, 0, u, 2, 1) - 3.0 * V) <= (1e-10 if prec == "f64" else 1e-5) * 3 * V
+    # the complex kind: round trip, qdp_sum; calls instantiated for 9/12/36 components refuse it
+    hz = synth.round_to(synth.color_matrix(dims, _seed(dims) + 103)[:, 0, 0].copy(), prec)
+    z = qdp.field_from_host(lat, qdp.QDP_COMPLEX, hz)
+    assert np.array_equal(qdp.field_to_host(z), hz)
+    zs = qdp.qdp_sum(z)
+    assert abs(complex(zs.ravel()[0]) - _as64(hz).sum()) <= TOL_SUM[prec] * np.abs(hz).sum()
+    for bad in (lambda: qdp.qdp_norm2(z), lambda: qdp.qdp_shift(qdp.qdp_field_alloc(lat, qdp.QDP_COMPLEX, P), z, 0, 1),
+                lambda: qdp.qdp_expr_trace_mul(m, u, 0, 0, u, 0, 1)):
+        with pytest.raises(qdp.QdpError):
+            bad()
