@@ -54,6 +54,9 @@ def _get():
             "orc_matvec": ([P, P, P, I, I, I, P, I, I, I], None),
             "orc_matmul": ([P, P, I, I, P, I, I, I, P, I, I, I, I, I, I], None),
             "orc_reunitarize": ([P, I, P, P, I, I], None),
+            "orc_max_retr_su3": ([P, I, P, P], None),
+            "orc_project_max_retr": ([P, I, P, P, I, I], None),
+            "orc_baryon_timeslices": ([P, I, P, P, P, I, I, P], None),
             "orc_trace_mul": ([P, P, P, I, I, I, P, I, I, I, I, I, I], None),
             "orc_staple_field": ([P, P, I, I, I, P], None),
             "orc_ape_blend_field": ([P, P, I, D, I, I, P], None),
@@ -215,6 +218,42 @@ def reunitarize(dims, f, method=POLAR, subset=ALL, out=None):
     nmat = f.size // (volume(dims) * 9)
     _get().orc_reunitarize(_dims(dims), nmat, f.ctypes.data, res.ctypes.data, method, subset)
     return res
+
+
+def max_retr_su3(V, iters, with_trace=False):
+    """Cabibbo-Marinari-style projection of one matrix (row f2): X_0 = Gram-Schmidt(V), then `iters` sweeps over the
+    SU(2) subgroups (0,1), (1,2), (0,2), each maximising Re tr(X V^dag).  with_trace: also Re tr(X V^dag) after X_0 and
+    after each of the 3*iters updates."""
+    V = _c128(V)
+    out = np.empty((3, 3), dtype=np.complex128)
+    tr = np.empty(1 + 3 * iters)
+    _get().orc_max_retr_su3(V.ctypes.data, int(iters), out.ctypes.data, tr.ctypes.data if with_trace else None)
+    return (out, tr) if with_trace else out
+
+
+def project_max_retr(dims, f, iters, subset=ALL, out=None):
+    """Every 3x3 matrix of the field ([V,4,3,3] or [V,3,3]) replaced by its max-Re-tr projection after `iters` sweeps."""
+    f = _c128(f)
+    res = np.zeros_like(f) if out is None else _c128(out).copy()
+    nmat = f.size // (volume(dims) * 9)
+    _get().orc_project_max_retr(_dims(dims), nmat, f.ctypes.data, res.ctypes.data, int(iters), subset)
+    return res
+
+
+def baryon_timeslices(dims, q1, q2, q3, n, subset=ALL):
+    """out[t, g] of orc_baryon_timeslices; q1, q2, q3: one fermion field each ([V,4,3]; no source contraction) or lists
+    of three fields each (one per source colour; eps_{a'b'c'} over them)."""
+    def pack(q):
+        fields = [_c128(q)] if isinstance(q, np.ndarray) else [_c128(f) for f in q]
+        return fields, (ctypes.c_void_p * len(fields))(*[f.ctypes.data for f in fields])
+    f1, p1 = pack(q1)
+    f2, p2 = pack(q2)
+    f3, p3 = pack(q3)
+    if not (len(f1) == len(f2) == len(f3)) or len(f1) not in (1, 3):
+        raise ValueError("one or three fields per quark")
+    out = np.empty((dims[3], 4), dtype=np.complex128)
+    _get().orc_baryon_timeslices(_dims(dims), len(f1), p1, p2, p3, int(n), subset, out.ctypes.data)
+    return out
 
 
 def min_eig_vdv(V):

@@ -395,6 +395,54 @@ void orc_reunitarize(const int *L, int nmat, const double *in, double *out, int 
     }
 }
 
+/* ---- iterative max-Re-tr projection ("iterative max-Re-tr"; Cabibbo-Marinari sweeps) -----
+ * Finds X in SU(3) that increases Re tr(X V^dag) by exact maximisation over one SU(2) subgroup at a time.
+ * Reading (f2): X_0 = Gram-Schmidt(V); one iteration = the three subgroups acting on the index
+ * pairs (0,1), (1,2), (0,2) in that order.  For the pair (i,j) let M = X V^dag and m its 2x2 block
+ * [[M_ii, M_ij], [M_ji, M_jj]].  Writing m = alpha_0 1 + sum_k alpha_k sigma_k with complex alpha and an SU(2) element
+ * a = a_0 1 + i sum_k a_k sigma_k (a real, |a| = 1):  Re tr(a m) = 2 (a_0 Re alpha_0 - sum_k a_k Im alpha_k), which is
+ * maximal for (a_0, a_k) = (Re alpha_0, -Im alpha_k) / norm, i.e. with
+ *     r0 = Re(m00 + m11), r1 = -Im(m01 + m10), r2 = -Re(m01 - m10), r3 = -Im(m00 - m11)
+ *     a = [[r0 + i r3, r2 + i r1], [-r2 + i r1, r0 - i r3]] / |r|.
+ * X <- A X, A = a embedded in rows/columns (i,j).  Every update leaves X in SU(3) and cannot decrease Re tr(X V^dag).
+ * retr (nullable) receives Re tr(X V^dag) after X_0 and after each of the 3*iters updates (1 + 3*iters values). */
+void orc_max_retr_su3(const double *Vin, int iters, double *out, double *retr) {
+    const cplx *V = (const cplx *)Vin;
+    cplx X[9], Vd[9], M[9];
+    orc_gram_schmidt_su3(Vin, (double *)X);
+    m_adj(V, Vd);
+    int nrec = 0;
+    m_mul(X, Vd, M);
+    if (retr) retr[nrec++] = m_trace(M).re;
+    static const int pi[3] = { 0, 1, 0 }, pj[3] = { 1, 2, 2 };
+    for (int it = 0; it < iters; it++)
+        for (int sg = 0; sg < 3; sg++) {
+            const int i = pi[sg], j = pj[sg];
+            m_mul(X, Vd, M);
+            const cplx m00 = M[i * 3 + i], m01 = M[i * 3 + j], m10 = M[j * 3 + i], m11 = M[j * 3 + j];
+            double r0 = m00.re + m11.re, r1 = -(m01.im + m10.im), r2 = -(m01.re - m10.re), r3 = -(m00.im - m11.im);
+            const double nr = sqrt(r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3);
+            if (nr > 0) { r0 /= nr; r1 /= nr; r2 /= nr; r3 /= nr; } else { r0 = 1; r1 = r2 = r3 = 0; }
+            const cplx a00 = { r0, r3 }, a01 = { r2, r1 }, a10 = { -r2, r1 }, a11 = { r0, -r3 };
+            for (int c = 0; c < 3; c++) {          /* rows i and j of X are mixed */
+                const cplx xi = X[i * 3 + c], xj = X[j * 3 + c];
+                X[i * 3 + c] = c_add(c_mul(a00, xi), c_mul(a01, xj));
+                X[j * 3 + c] = c_add(c_mul(a10, xi), c_mul(a11, xj));
+            }
+            if (retr) { m_mul(X, Vd, M); retr[nrec++] = m_trace(M).re; }
+        }
+    memcpy(out, X, sizeof X);
+}
+/* whole fields: out(x) = orc_max_retr_su3(in(x)) for every matrix of the subset's sites (nmat per site) */
+void orc_project_max_retr(const int *L, int nmat, const double *in, double *out, int iters, int subset) {
+    for (size_t s = 0; s < volume(L); s++) {
+        int x[4]; coords_of(L, s, x);
+        if (!in_subset(x, subset)) continue;
+        for (int m = 0; m < nmat; m++)
+            orc_max_retr_su3(in + (s * nmat + m) * 18, iters, out + (s * nmat + m) * 18, NULL);
+    }
+}
+
 /* smallest singular value^2 of V (lambda_min of V^dag V), for reading A10 */
 double orc_min_eig_vdv(const double *Vin) {
     const cplx *V = (const cplx *)Vin;
@@ -690,6 +738,51 @@ void orc_inner_timeslices_gamma(const int *L, const double *a, const double *b, 
         }
         out[2 * t] = k_val(&kr);
         out[2 * t + 1] = k_val(&ki);
+    }
+}
+
+/* ---- baryon building block ("meson/baryon colour-spin contractions"; HAD stage) ---
+ * Three quark fields contracted to a colour singlet with the antisymmetric tensor, a diquark spin matrix Gamma(n)
+ * between the first two, summed over each time-slice:
+ *   out[t][g] = sum_{x in subset, x3 = t} sum_{(a',b',c')} eps_{a'b'c'} sum_{a b c} eps_{abc}
+ *               [ sum_{al be} q1[a']_{al a}(x) Gamma(n)_{al be} q2[b']_{be b}(x) ] q3[c']_{g c}(x),     g = 0..3 (open spin).
+ * nsrc = 3: q1, q2, q3 are arrays of three fermion fields each, one per SOURCE colour (columns of a quark propagator
+ * with fixed source spin), and (a',b',c') runs over the six permutations with their signs: the eps_{abc} eps_{a'b'c'}
+ * colour contraction of the nucleon two-point function.  nsrc = 1: one field per quark, no source contraction (the
+ * colour-singlet operator eps_{abc} (q1^T Gamma q2)_{ab} q3_c of three spinor fields).  No conjugation anywhere.
+ * out: [L3][4] complex. */
+void orc_baryon_timeslices(const int *L, int nsrc, const double *const *q1, const double *const *q2,
+                           const double *const *q3, int n, int subset, double *out) {
+    cplx G[16];
+    orc_gamma_matrix(n, (double *)G);
+    static const int perm[6][3] = { {0,1,2}, {1,2,0}, {2,0,1}, {0,2,1}, {2,1,0}, {1,0,2} };
+    static const double psign[6] = { 1, 1, 1, -1, -1, -1 };
+    const int nperm = nsrc == 3 ? 6 : 1;
+    for (int t = 0; t < L[3]; t++) {
+        ksum k[8];
+        memset(k, 0, sizeof k);
+        for (size_t s = 0; s < volume(L); s++) {
+            int x[4]; coords_of(L, s, x);
+            if (x[3] != t || !in_subset(x, subset)) continue;
+            for (int ps = 0; ps < nperm; ps++) {
+                const int sa = nsrc == 3 ? perm[ps][0] : 0, sb = nsrc == 3 ? perm[ps][1] : 0, sc = nsrc == 3 ? perm[ps][2] : 0;
+                const cplx *A = (const cplx *)q1[sa] + s * 12, *B = (const cplx *)q2[sb] + s * 12,
+                           *C = (const cplx *)q3[sc] + s * 12;
+                for (int pc = 0; pc < 6; pc++) {                /* sink colours (a,b,c) = a permutation of (0,1,2) */
+                    const int a = perm[pc][0], b = perm[pc][1], c = perm[pc][2];
+                    cplx dq = { 0, 0 };                         /* q1^T Gamma q2 for colours (a, b) */
+                    for (int al = 0; al < 4; al++)
+                        for (int be = 0; be < 4; be++)
+                            dq = c_add(dq, c_mul(c_mul(A[al * 3 + a], G[al * 4 + be]), B[be * 3 + b]));
+                    for (int g = 0; g < 4; g++) {
+                        cplx v = c_scale(psign[ps] * psign[pc], c_mul(dq, C[g * 3 + c]));
+                        k_add(&k[2 * g], v.re);
+                        k_add(&k[2 * g + 1], v.im);
+                    }
+                }
+            }
+        }
+        for (int i = 0; i < 8; i++) out[t * 8 + i] = k_val(&k[i]);
     }
 }
 
