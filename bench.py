@@ -306,6 +306,11 @@ def run_ours(args) -> dict | None:
         "expr_staple": (lambda: q.qdp_expr_staple(cm, u, 0, 3), 36,
                         "qdp_expr_staple mu = 0, spatial (row f1): the staple sum as one expression; 27 complex read "
                         "(three links) + 9 written per site"),
+        "project_max_retr": (lambda: q.qdp_project_max_retr(u2, u, 3), 72,
+                             "qdp_project_max_retr, 3 sweeps (row f2): 36 complex read + 36 written per site"),
+        "baryon_timeslices": (lambda: q.qdp_baryon_timeslices([psi, chi, sh], [chi, sh, psi], [sh, psi, chi], 5), 36,
+                              "qdp_baryon_timeslices, nsrc = 3 (row f3): here 3 distinct spinor fields stand in for the 9 "
+                              "propagator columns (36 complex per site algorithmic), includes the host round trip"),
         "plaquette_staged": (None, 36, "qdp_plaquette with qdp_lattice_set_staged(1): cp.async.bulk + mbarrier "
                                        "shared-memory rings (plaquette_tma.cu); compare ops.plaquette"),
     }

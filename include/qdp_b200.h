@@ -225,6 +225,17 @@ int qdp_matvec(qdp_field* chi, const qdp_field* a, int slot_a, int adj_a, const 
 enum { QDP_REUNIT_POLAR = 0, QDP_REUNIT_GRAM_SCHMIDT = 1 };
 int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset);
 
+/* Row f2, iterative max-Re-tr projection (Cabibbo-Marinari sweeps): every 3x3 matrix V of the subset's sites is
+ * replaced by X in SU(3) obtained as follows (reading in DESIGN.md section 2, f2; the paper only names "smearing"):
+ *   X_0 = Gram-Schmidt(V) (QDP_REUNIT_GRAM_SCHMIDT above); one iteration = the SU(2) subgroups acting on the index
+ *   pairs (0,1), (1,2), (0,2) in that order; for the pair (i,j), with m the 2x2 block of M = X V^dag in rows and
+ *   columns (i,j):  r0 = Re(m00 + m11), r1 = -Im(m01 + m10), r2 = -Re(m01 - m10), r3 = -Im(m00 - m11),
+ *   a = [[r0 + i r3, r2 + i r1], [-r2 + i r1, r0 - i r3]] / |r|  (the SU(2) element maximising Re tr(a m)),
+ *   X <- A X with A = a embedded in (i,j).  No update can decrease Re tr(X V^dag); an SU(3) input is a fixed point.
+ * `iterations` (0..1000) sweeps are always executed (no convergence test, so the result is a function of V and the
+ * count only).  Same fields / aliasing rules as qdp_reunitarize; fp64 arithmetic for both precisions.  Asynchronous. */
+int qdp_project_max_retr(qdp_field* u_out, const qdp_field* u_in, int iterations, qdp_subset subset);
+
 /* def. 5: chi(x)_{s a} = sum_mu sum_b [ U_mu(x)_{ab} psi(x+mu)_{s b}
  *                                      + conj(U_mu(x-mu)_{ba}) psi(x-mu)_{s b} ]
  * for x in subset (no gamma matrices, no kappa, periodic in all directions).
@@ -281,6 +292,20 @@ int qdp_inner_timeslices(const qdp_field* a, const qdp_field* b, qdp_subset subs
  * With a, b columns of quark propagators this is the building block of meson two-point functions
  * (HAD stage).  n = 0 equals qdp_inner_timeslices.  Synchronous. */
 int qdp_inner_timeslices_gamma(const qdp_field* a, const qdp_field* b, int n, qdp_subset subset, double* out);
+
+/* Row f3, baryon contractions (HAD stage: "hadron spectrum (mesonic and baryonic)"): three quark
+ * fields contracted to a colour singlet with the antisymmetric tensor, the spin matrix Gamma(n) (as in
+ * qdp_inner_timeslices_gamma) between the first two, summed per time-slice; the third quark's spin index g stays open:
+ *   out[t][g] = sum_{x in subset, x3 = t} sum_{(a',b',c')} eps_{a'b'c'} sum_{a b c} eps_{abc}
+ *               [ sum_{al be} q1[a']_{al a}(x) Gamma(n)_{al be} q2[b']_{be b}(x) ] q3[c']_{g c}(x).
+ * nsrc = 3: q1, q2, q3 point to three QDP_FERMION fields each, one per SOURCE colour a', b', c' (columns of a quark
+ * propagator with fixed source spin), and (a',b',c') runs over the six permutations with their signs: the
+ * eps_{abc} eps_{a'b'c'} colour contraction of a nucleon-type two-point function, all nine fields read in one pass.
+ * nsrc = 1: one field per quark and no source contraction (the colour-singlet operator of three spinor fields).
+ * No complex conjugation is applied to any field.  out: host, 8*L3 doubles, out[(t*4 + g)*2 + (0: re, 1: im)].
+ * fp64 accumulation, fixed summation order.  All fields on one lattice and of one precision.  Synchronous. */
+int qdp_baryon_timeslices(const qdp_field* const* q1, const qdp_field* const* q2, const qdp_field* const* q3,
+                          int nsrc, int n, qdp_subset subset, double* out);
 
 /* ---- the expression layer ---------------------------------------------
  * The paper turns every QDP++ expression (PETE expression templates, "expressions that look like their

@@ -18,7 +18,7 @@ __all__ = [
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
-    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_matmul", "qdp_matvec", "qdp_axpby", "qdp_expr_plaquette", "qdp_expr_staple", "qdp_expr_ape_blend", "qdp_expr_trace_mul", "qdp_expr_sum_trace_mul", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
+    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_project_max_retr", "qdp_baryon_timeslices", "qdp_matmul", "qdp_matvec", "qdp_axpby", "qdp_expr_plaquette", "qdp_expr_staple", "qdp_expr_ape_blend", "qdp_expr_trace_mul", "qdp_expr_sum_trace_mul", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
 ]
@@ -72,6 +72,8 @@ DECLARED_SYMBOLS = {
     "qdp_axpby": ([_P, _D, _P, _D, _P, _I, _P], _I),
     "qdp_matvec": ([_P, _P, _I, _I, _P, _I, _I, _I], _I),
     "qdp_matmul": ([_P, _I, _P, _I, _I, _P, _I, _I, _I, _I, _I], _I),
+    "qdp_project_max_retr": ([_P, _P, _I, _I], _I),
+    "qdp_baryon_timeslices": ([_PP, _PP, _PP, _I, _I, _I, _P], _I),
     "qdp_expr_plaquette": ([_P, _I, ctypes.POINTER(_D)], _I),
     "qdp_expr_staple": ([_P, _P, _I, _I, _I], _I),
     "qdp_expr_ape_blend": ([_P, _P, _I, _D, _I, _I], _I),
@@ -324,6 +326,27 @@ def qdp_expr_sum_trace_mul(a: Field, slot_a: int, adj_a: bool, b: Field, slot_b:
 
 def qdp_reunitarize(u_out: Field, u_in: Field, method: int = QDP_REUNIT_POLAR, subset: int = QDP_ALL) -> None:
     _check(_lib.qdp_reunitarize(u_out.handle, u_in.handle, int(method), subset))
+
+
+def qdp_project_max_retr(u_out: Field, u_in: Field, iterations: int, subset: int = QDP_ALL) -> None:
+    _check(_lib.qdp_project_max_retr(u_out.handle, u_in.handle, int(iterations), subset))
+
+
+def qdp_baryon_timeslices(q1, q2, q3, n: int, subset: int = QDP_ALL) -> np.ndarray:
+    """q1, q2, q3: a Field each (no source contraction) or a sequence of three Fields each (one per source colour).
+    Returns out[t, g], complex, [L3, 4]."""
+    def pack(q):
+        fields = [q] if isinstance(q, Field) else list(q)
+        return fields, (ctypes.c_void_p * len(fields))(*[f.handle for f in fields])
+    f1, p1 = pack(q1)
+    f2, p2 = pack(q2)
+    f3, p3 = pack(q3)
+    if not (len(f1) == len(f2) == len(f3)):
+        raise ValueError("the same number of fields (1 or 3) per quark")
+    L3 = f1[0].lat.dims[3]
+    out = np.empty(8 * L3)
+    _check(_lib.qdp_baryon_timeslices(p1, p2, p3, len(f1), int(n), subset, out.ctypes.data))
+    return (out[0::2] + 1j * out[1::2]).reshape(L3, 4)
 
 
 def qdp_hop(chi: Field, u: Field, psi: Field, subset: int = QDP_ALL) -> None:

@@ -170,7 +170,7 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
     size_t npart = (size_t)4 * kMaxPartialBlocks;
     if (npart < 4 * (nwarp_max + ngroup_max)) npart = 4 * (nwarp_max + ngroup_max);
     if (npart < (size_t)2 * 36 * 64) npart = (size_t)2 * 36 * 64;
-    if (npart < (size_t)34 * dims[3]) npart = (size_t)34 * dims[3];   // qdp_inner_timeslices: 2*16*L3 partials + 2*L3 results
+    if (npart < (size_t)136 * dims[3]) npart = (size_t)136 * dims[3];   // qdp_baryon_timeslices: 8*16*L3 partials + 8*L3 results (qdp_inner_timeslices: 2*16*L3 + 2*L3)
     const size_t counter_bytes = (ngroup_max + 1) * sizeof(unsigned int);
     // everything below is released by release_lattice() on any failure
     auto attempt = [&]() -> int {
@@ -482,20 +482,27 @@ extern "C" int qdp_matvec(qdp_field* chi, const qdp_field* a, int slot_a, int ad
     return QDP_OK;
 }
 
-extern "C" int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset) {
-    if (!ok_field(u_out) || !ok_field(u_in) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_reunitarize: bad argument");
-    if (method != QDP_REUNIT_POLAR && method != QDP_REUNIT_GRAM_SCHMIDT)
-        return fail(QDP_ERR_ARG, "qdp_reunitarize: unknown method %d", method);
-    if (u_in->kind == QDP_FERMION || u_out->kind != u_in->kind)
-        return fail(QDP_ERR_KIND, "qdp_reunitarize: need two gauge fields or two colour matrices");
-    int rc = check_pair("qdp_reunitarize", u_out, u_in);
+static int reunit_common(const char* who, qdp_field* u_out, const qdp_field* u_in, int method, int iters, qdp_subset subset) {
+    if (!ok_field(u_out) || !ok_field(u_in) || !ok_subset(subset)) return fail(QDP_ERR_ARG, "%s: bad argument", who);
+    if ((u_in->kind != QDP_GAUGE && u_in->kind != QDP_COLOR_MATRIX) || u_out->kind != u_in->kind)
+        return fail(QDP_ERR_KIND, "%s: need two gauge fields or two colour matrices", who);
+    int rc = check_pair(who, u_out, u_in);
     if (rc != QDP_OK) return rc;
     if (u_out != u_in && u_out->data != u_in->data && overlaps(u_out, u_in))
-        return fail(QDP_ERR_ALIAS, "qdp_reunitarize: u_out partially overlaps u_in");
+        return fail(QDP_ERR_ALIAS, "%s: u_out partially overlaps u_in", who);
     qdp_lattice* l = u_out->lat;
     ENTER(l);
-    CUDA_TRY(launch_reunit(u_out->prec, l->geom, u_out->ncomp, u_out->data, u_in->data, method, subset, l->stream));
+    CUDA_TRY(launch_reunit(u_out->prec, l->geom, u_out->ncomp, u_out->data, u_in->data, method, subset, l->stream, iters));
     return QDP_OK;
+}
+extern "C" int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset) {
+    if (method != QDP_REUNIT_POLAR && method != QDP_REUNIT_GRAM_SCHMIDT)
+        return fail(QDP_ERR_ARG, "qdp_reunitarize: unknown method %d", method);
+    return reunit_common("qdp_reunitarize", u_out, u_in, method, 0, subset);
+}
+extern "C" int qdp_project_max_retr(qdp_field* u_out, const qdp_field* u_in, int iterations, qdp_subset subset) {
+    if (iterations < 0 || iterations > 1000) return fail(QDP_ERR_ARG, "qdp_project_max_retr: iterations must be 0..1000");
+    return reunit_common("qdp_project_max_retr", u_out, u_in, 2, iterations, subset);
 }
 
 static int hop_common(const char* who, qdp_field* chi, const qdp_field* u, const qdp_field* psi, qdp_subset subset,
@@ -614,6 +621,33 @@ static int inner_timeslices_common(const char* who, const qdp_field* a, const qd
     CUDA_TRY(launch_inner_timeslices(a->prec, l->geom, a->ncomp, a->data, b->data, subset, l->partials, out_dev,
                                      l->stream, gamma));
     CUDA_TRY(cudaMemcpyAsync(out, out_dev, (size_t)2 * L3 * sizeof(double), cudaMemcpyDeviceToHost, l->stream));
+    CUDA_TRY(cudaStreamSynchronize(l->stream));
+    return QDP_OK;
+}
+
+extern "C" int qdp_baryon_timeslices(const qdp_field* const* q1, const qdp_field* const* q2, const qdp_field* const* q3,
+                                     int nsrc, int n, qdp_subset subset, double* out) {
+    if (!q1 || !q2 || !q3 || !out || !ok_subset(subset)) return fail(QDP_ERR_ARG, "qdp_baryon_timeslices: bad argument");
+    if (nsrc != 1 && nsrc != 3) return fail(QDP_ERR_ARG, "qdp_baryon_timeslices: nsrc must be 1 or 3");
+    if (n < 0 || n > 15) return fail(QDP_ERR_ARG, "qdp_baryon_timeslices: n must be 0..15");
+    const qdp_field* const* qs[3] = {q1, q2, q3};
+    const void* ptr[3][3] = {};
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < nsrc; j++) {
+            const qdp_field* f = qs[i][j];
+            if (!ok_field(f)) return fail(QDP_ERR_ARG, "qdp_baryon_timeslices: not a field");
+            if (f->kind != QDP_FERMION) return fail(QDP_ERR_KIND, "qdp_baryon_timeslices: fermion fields needed");
+            int rc = check_pair("qdp_baryon_timeslices", qs[0][0], f);
+            if (rc != QDP_OK) return rc;
+            ptr[i][j] = f->data;
+        }
+    qdp_lattice* l = q1[0]->lat;
+    ENTER(l);
+    const SpinMatrix m = spin_matrix(n);
+    const int L3 = l->geom.L3;
+    double* out_dev = l->partials + (size_t)8 * 16 * L3;   // behind the per-block partials
+    CUDA_TRY(launch_baryon_timeslices(q1[0]->prec, l->geom, ptr, nsrc, m, subset, l->partials, out_dev, l->stream));
+    CUDA_TRY(cudaMemcpyAsync(out, out_dev, (size_t)8 * L3 * sizeof(double), cudaMemcpyDeviceToHost, l->stream));
     CUDA_TRY(cudaStreamSynchronize(l->stream));
     return QDP_OK;
 }

@@ -68,9 +68,14 @@ cudaError_t launch_matmul(int prec, const Geom& g, void* dst, int nd, int id, co
 cudaError_t launch_matvec(int prec, const Geom& g, void* chi, const void* a, int na, int ia, bool adj_a, const void* psi,
                           int mu, int sign, int subset, cudaStream_t st);
 
-// reunit.cu: method 0 = Proj (polar factor, determinant phase removed), 1 = Gram-Schmidt; in place allowed
+// reunit.cu: method 0 = Proj (polar factor, determinant phase removed), 1 = Gram-Schmidt, 2 = `iters` max-Re-tr sweeps
+// from the Gram-Schmidt start; in place allowed
 cudaError_t launch_reunit(int prec, const Geom& g, int ncomp, void* out, const void* in, int method, int subset,
-                          cudaStream_t st);
+                          cudaStream_t st, int iters = 0);
+
+// baryon.cu: q[quark][source colour] (nsrc = 1 or 3 fields per quark); partials 8 * 16 * L3 doubles, out_dev 8 * L3
+cudaError_t launch_baryon_timeslices(int prec, const Geom& g, const void* const q[3][3], int nsrc, const SpinMatrix& gm,
+                                     int subset, double* partials, double* out_dev, cudaStream_t st);
 
 // expr.cu: named instantiations of the compile-time expression layer (expr.cuh)
 cudaError_t launch_expr_plaquette(int prec, const Geom& g, const void* u, int subset, const ReduceBuf& rb, cudaStream_t st);

@@ -822,3 +822,84 @@ def test_expression_layer(qdp, lat_cache, dims, prec):
                 lambda: qdp.qdp_expr_trace_mul(m, u, 0, 0, u, 0, 1)):
         with pytest.raises(qdp.QdpError):
             bad()
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_project_max_retr(qdp, lat_cache, dims, prec):
+    """qdp_project_max_retr (row f2): Cabibbo-Marinari sweeps, element by element against the oracle's step-by-step
+    algorithm (same start, same subgroup order, fixed iteration count); SU(3) output; SU(3) input is a fixed point."""
+    lat = lat_cache(dims)
+    P = 1 if prec == "f64" else 0
+    hg = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 111) + 0.3 * synth.gauge_hot(dims, _seed(dims) + 112), prec)
+    hm = synth.round_to(synth.color_matrix(dims, _seed(dims) + 113), prec)
+    unit_bar = 1e-12 if prec == "f64" else 1e-5
+    for kind, host in ((1, hg), (0, hm)):
+        src = qdp.field_from_host(lat, kind, host)
+        h64 = links(_as64(host))
+        cond = np.sqrt((np.abs(h64) ** 2).sum(axis=(1, 2)) / np.array([oracle.min_eig_vdv(m) for m in h64]))
+        for iters in (0, 1, 4):
+            for sub in SUBSETS if iters == 4 else [0]:
+                sentinel = np.full_like(host, 3.0 - 2.0j)
+                dst = qdp.field_from_host(lat, kind, sentinel)
+                qdp.qdp_project_max_retr(dst, src, iters, sub)
+                want = oracle.project_max_retr(dims, _as64(host), iters, sub, out=_as64(sentinel))
+                # the iteration is a contraction towards the maximiser: rounding differences do not grow with the count.
+                # The Gram-Schmidt start divides by the norm of the component of row 1 orthogonal to row 0, which
+                # amplifies rounding by up to cond(V): conditioning-scaled bar as for qdp_reunitarize (DESIGN.md "Tolerances")
+                tol = TOL_SITE[prec] * np.maximum(4.0, cond)
+                assert np.all(site_rel_err(links(_as64(qdp.field_to_host(dst))), links(want)) <= tol), (kind, iters, sub)
+        work = qdp.field_from_host(lat, kind, host)
+        qdp.qdp_project_max_retr(work, work, 6)               # in place
+        g = links(_as64(qdp.field_to_host(work)))
+        assert np.abs(g @ np.conj(np.swapaxes(g, 1, 2)) - np.eye(3)).max() <= unit_bar
+        assert np.abs(np.linalg.det(g) - 1).max() <= unit_bar
+        # more sweeps never lower Re tr(X V^dag)
+        v = links(_as64(host))
+        t6 = np.einsum("xij,xij->x", g, np.conj(v)).real
+        qdp.qdp_project_max_retr(work, qdp.field_from_host(lat, kind, host), 2)
+        g2 = links(_as64(qdp.field_to_host(work)))
+        t2 = np.einsum("xij,xij->x", g2, np.conj(v)).real
+        assert np.all(t6 >= t2 - (1e-12 if prec == "f64" else 1e-5) * np.abs(t2))
+    su3 = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 114), "f64")
+    if prec == "f64":
+        f = qdp.field_from_host(lat, 1, su3)
+        out = qdp.qdp_field_alloc(lat, 1, P)
+        qdp.qdp_project_max_retr(out, f, 3)
+        assert np.abs(qdp.field_to_host(out) - su3).max() <= 1e-14
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_project_max_retr(qdp.qdp_field_alloc(lat, 2, P), qdp.qdp_field_alloc(lat, 2, P), 1)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_project_max_retr(src, src, -1)
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", PRECS)
+def test_baryon_timeslices(qdp, lat_cache, dims, prec):
+    """qdp_baryon_timeslices (row f3): the eps-eps colour contraction with a diquark spin matrix, per time-slice, both
+    forms (one field per quark; three source colours per quark), subsets, several Gamma(n)."""
+    lat = lat_cache(dims)
+    hf = [synth.round_to(synth.spinor(dims, _seed(dims) + 121, k), prec) for k in range(9)]
+    f = [qdp.field_from_host(lat, 2, h) for h in hf]
+    h64 = [_as64(h) for h in hf]
+    scale = (sum(oracle.norm2(dims, h) for h in h64) / 9) ** 1.5 / np.sqrt(synth.volume(dims)) * 20
+    for n in (0, 5, 10, 15):
+        n0 = qdp.qdp_kernel_launch_count()
+        got = qdp.qdp_baryon_timeslices(f[0:3], f[3:6], f[6:9], n)
+        assert qdp.qdp_kernel_launch_count() == n0 + 2
+        want = oracle.baryon_timeslices(dims, h64[0:3], h64[3:6], h64[6:9], n)
+        assert np.abs(got - want).max() <= TOL_SUM[prec] * scale * 6, n
+        got1 = qdp.qdp_baryon_timeslices(f[0], f[1], f[2], n)
+        assert np.abs(got1 - oracle.baryon_timeslices(dims, h64[0], h64[1], h64[2], n)).max() <= TOL_SUM[prec] * scale, n
+    assert np.array_equal(got, qdp.qdp_baryon_timeslices(f[0:3], f[3:6], f[6:9], 15))      # deterministic
+    for sub in (1, 2):
+        gs = qdp.qdp_baryon_timeslices(f[0:3], f[3:6], f[6:9], 5, sub)
+        assert np.abs(gs - oracle.baryon_timeslices(dims, h64[0:3], h64[3:6], h64[6:9], 5, sub)).max() <= TOL_SUM[prec] * scale * 6
+    # identical quarks in a symmetric diquark vanish (Gamma(n)^T = +Gamma(n))
+    G = oracle.gamma_matrix(10)
+    if np.array_equal(G.T, G):
+        assert np.abs(qdp.qdp_baryon_timeslices(f[0], f[0], f[2], 10)).max() <= TOL_SUM[prec] * scale
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_baryon_timeslices(f[0], f[1], f[2], 16)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_baryon_timeslices(f[0], f[1], qdp.qdp_field_alloc(lat, 0, 1 if prec == "f64" else 0), 5)
