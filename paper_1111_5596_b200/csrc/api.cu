@@ -63,8 +63,9 @@ struct qdp_lattice {
     // scratch, all allocated at create time
     double* partials;        // device: 4 * kMaxPartialBlocks, also 2*36*64 for sum
     unsigned int* counter;   // device
-    double* result_host;     // pinned, mapped: 72 doubles; the reducing kernels write their results here
+    double* result_host;     // pinned, mapped: 72 doubles + the completion flag; the reducing kernels write their results here
     double* result_dev;      // the device address of result_host
+    unsigned long long seq;  // number of the last reducing launch; the kernel stores it behind the results when they are complete
     void* stage[2];          // device staging chunks for upload/download
     size_t stage_bytes;
     cudaStream_t copy_stream;
@@ -97,16 +98,38 @@ static bool ok_lat(const qdp_lattice* l) { return l && l->magic == kLatMagic; }
 static bool ok_field(const qdp_field* f) { return f && f->magic == kFieldMagic && ok_lat(f->lat); }
 static bool ok_subset(int s) { return s == QDP_ALL || s == QDP_EVEN || s == QDP_ODD; }
 
+static const int kResultSlots = 72;   // doubles of results; the completion flag follows them
 static ReduceBuf reduce_buf(qdp_lattice* l) {
     ReduceBuf rb;
     rb.partials = l->partials;
     rb.counter = l->counter;
     rb.result = l->result_dev;
+    rb.flag = reinterpret_cast<unsigned long long*>(l->result_dev + kResultSlots);
+    rb.seq = ++l->seq;
     return rb;
 }
-// The last block of a reducing kernel stores the n results straight into mapped pinned host
-// memory (no separate device-to-host copy to launch); wait for the kernel and hand them out.
+// The last block of a reducing kernel stores the n results straight into mapped pinned host memory (no separate
+// device-to-host copy to launch) and then the launch's sequence number behind them.  The host polls that number
+// (a few microseconds less than cudaStreamSynchronize per scalar-returning call: DESIGN.md section 4) and checks the
+// stream from time to time so that a failed kernel surfaces as an error instead of a hang.
 static int fetch_result(qdp_lattice* l, int n, double* out) {
+    volatile unsigned long long* flag = reinterpret_cast<volatile unsigned long long*>(l->result_host + kResultSlots);
+    for (unsigned spin = 1; *flag != l->seq; spin++) {
+        if ((spin & 0x3fff) == 0) {
+            cudaError_t q = cudaStreamQuery(l->stream);
+            if (q == cudaSuccess) {
+                if (*flag == l->seq) break;
+                return fail(QDP_ERR_CUDA, "reduction kernel finished without signalling its result");
+            }
+            if (q != cudaErrorNotReady) return fail(QDP_ERR_CUDA, "CUDA error: %s", cudaGetErrorString(q));
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    memcpy(out, l->result_host, n * sizeof(double));
+    return QDP_OK;
+}
+// for results that a kernel without the completion signal wrote (qdp_sum)
+static int fetch_result_sync(qdp_lattice* l, int n, double* out) {
     CUDA_TRY(cudaStreamSynchronize(l->stream));
     memcpy(out, l->result_host, n * sizeof(double));
     return QDP_OK;
@@ -181,7 +204,8 @@ extern "C" int qdp_lattice_create(const int dims[4], int device, qdp_lattice** o
         if ((rc = dev_alloc(counter_bytes, &p)) != QDP_OK) return rc;
         l->counter = (unsigned int*)p;
         CUDA_TRY(cudaMemset(l->counter, 0, counter_bytes));
-        CUDA_TRY(cudaHostAlloc((void**)&l->result_host, 72 * sizeof(double), cudaHostAllocMapped));
+        CUDA_TRY(cudaHostAlloc((void**)&l->result_host, (kResultSlots + 1) * sizeof(double), cudaHostAllocMapped));
+        memset(l->result_host, 0, (kResultSlots + 1) * sizeof(double));
         CUDA_TRY(cudaHostGetDevicePointer((void**)&l->result_dev, l->result_host, 0));
         l->stage_bytes = (size_t)kStageSites * 36 * 16;
         for (int i = 0; i < 2; i++) {
@@ -657,7 +681,7 @@ extern "C" int qdp_sum(const qdp_field* f, qdp_subset subset, double* out) {
     qdp_lattice* l = f->lat;
     ENTER(l);
     CUDA_TRY(launch_sum(f->prec, l->geom, f->ncomp, f->data, subset, l->partials, l->result_dev, l->stream));
-    return fetch_result(l, 2 * f->ncomp, out);
+    return fetch_result_sync(l, 2 * f->ncomp, out);
 }
 
 // ---- the expression layer (csrc/expr.cuh, expr.cu): named instantiations --------------------------

@@ -18,7 +18,17 @@ struct ReduceBuf {
     double* partials;        // [K][number of blocks or warps], then [K][number of groups]; K <= 4
     unsigned int* counter;   // [1 + number of groups], zero between launches
     double* result;          // [K] (device-visible)
+    // Completion signal for the host: after the results are stored the final thread writes `seq` to *flag (mapped pinned
+    // host memory; __threadfence_system between the two), so the host can poll instead of synchronising the stream.
+    unsigned long long* flag;   // nullptr: no signal
+    unsigned long long seq;
 };
+__device__ __forceinline__ void signal_results(const ReduceBuf& rb) {
+    if (rb.flag) {
+        __threadfence_system();
+        *reinterpret_cast<volatile unsigned long long*>(rb.flag) = rb.seq;
+    }
+}
 constexpr int kWarpGroup = 64;   // warps per group in warp_grid_reduce
 
 // NT = threads per block (multiple of 32, <= 1024)
@@ -85,6 +95,7 @@ __device__ __forceinline__ void grid_reduce(double (&v)[K], const ReduceBuf& rb,
 #pragma unroll
         for (int k = 0; k < K; k++) rb.result[k] = scale ? t[k] * scale[k] : t[k];
         *rb.counter = 0u;
+        signal_results(rb);
     }
 }
 
@@ -160,6 +171,7 @@ __device__ __forceinline__ void warp_grid_reduce(double (&v)[K], const ReduceBuf
 #pragma unroll
         for (int k = 0; k < K; k++) rb.result[k] = scale ? t[k] * scale[k] : t[k];
         rb.counter[0] = 0u;
+        signal_results(rb);
     }
 }
 
