@@ -336,6 +336,49 @@ int qdp_expr_trace_mul(qdp_field* dst, const qdp_field* a, int slot_a, int adj_a
 int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a, const qdp_field* b, int slot_b, int adj_b,
                            int mu, int sign, qdp_subset subset, double out[2]);
 
+/* ---- device memory pool and LRU residency manager --------------------------
+ * The paper's memory layer: "the pool manager grabs a large chunk of GPU memory at start-up" and a
+ * software cache "decides host/device affiliation per lattice object and spills least-recently-used objects" when an
+ * allocation does not fit; QUDA's allocations are redirected into the same pool.  On a 180 GB B200 the
+ * BASELINE workloads are resident for their lifetime, so the hot path never needs it; it is provided for working sets
+ * beyond device memory.  Host-side logic (csrc/pool.cu); the policy is stated here and modelled in oracle/pool_model.py.
+ *
+ * Pool: one cudaMalloc of `bytes` on `device` at creation, sub-allocated in units of 256 bytes: first fit = the free
+ * block with the lowest offset that is large enough; freed blocks are merged with free neighbours.  device = -1 creates
+ * an address-range-only pool (nothing is allocated or copied; returned pointers are offsets from a fake base): the
+ * allocator and the eviction policy can then be exercised without a GPU.  qdp_pool_alloc returns QDP_ERR_OOM only when
+ * no block fits after every unlocked cached object has been spilled.  qdp_pool_stats: out = {capacity, bytes in use,
+ * largest free block, number of free blocks}.  qdp_pool_hook_alloc/free have the signature qdp_set_allocator expects
+ * (ctx = the pool), so fields and scratch buffers can be drawn from the pool.
+ *
+ * Cached objects: qdp_cache_register ties `bytes` of data to a caller-owned host buffer (pinned memory makes the
+ * copies fast; it must stay valid until qdp_cache_unregister).  The data are whatever bytes the caller keeps there --
+ * for a field, its device layout (qdp_field_wrap the pointer qdp_cache_acquire returns, with qdp_field_bytes bytes).
+ * qdp_cache_acquire(c, for_write, &ptr): if c is not resident, allocate it from the pool -- when nothing fits, spill
+ * resident objects with no outstanding acquire, least recently acquired first, one at a time until a block fits (an
+ * object acquired for writing since it was paged in is first copied back to its host buffer) -- and copy the host
+ * buffer in; then lock it, mark it most recently used and return its device address.  qdp_cache_release unlocks.
+ * The copies are synchronous cudaMemcpy calls: work that still uses an object must have been synchronised
+ * (qdp_lattice_sync) before the object is released.  qdp_cache_unregister copies a modified resident object back and
+ * frees it.  qdp_pool_eviction_log lists the ids (qdp_cache_id: registration order, from 0) of the objects spilled so
+ * far, oldest first; *n receives their number.  Not thread-safe: one host thread per pool. */
+typedef struct qdp_pool qdp_pool;       /* opaque */
+typedef struct qdp_cached qdp_cached;   /* opaque */
+int qdp_pool_create(int device, size_t bytes, qdp_pool** out);
+int qdp_pool_destroy(qdp_pool* pool);
+int qdp_pool_alloc(qdp_pool* pool, size_t bytes, void** out);
+int qdp_pool_free(qdp_pool* pool, void* ptr);
+int qdp_pool_stats(const qdp_pool* pool, size_t out[4]);
+void* qdp_pool_hook_alloc(size_t bytes, void* pool);
+void qdp_pool_hook_free(void* ptr, void* pool);
+int qdp_cache_register(qdp_pool* pool, void* host_buf, size_t bytes, qdp_cached** out);
+int qdp_cache_acquire(qdp_cached* c, int for_write, void** dev_ptr);
+int qdp_cache_release(qdp_cached* c);
+int qdp_cache_unregister(qdp_cached* c);
+int qdp_cache_is_resident(const qdp_cached* c);
+int64_t qdp_cache_id(const qdp_cached* c);
+int qdp_pool_eviction_log(const qdp_pool* pool, int64_t* ids, int max, int* n);
+
 /* Block the host until every call enqueued on the lattice's stream has finished. */
 int qdp_lattice_sync(qdp_lattice* lat);
 

@@ -21,6 +21,9 @@ __all__ = [
     "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_project_max_retr", "qdp_baryon_timeslices", "qdp_matmul", "qdp_matvec", "qdp_axpby", "qdp_expr_plaquette", "qdp_expr_staple", "qdp_expr_ape_blend", "qdp_expr_trace_mul", "qdp_expr_sum_trace_mul", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
+    "Pool", "Cached", "qdp_pool_create", "qdp_pool_destroy", "qdp_pool_alloc", "qdp_pool_free", "qdp_pool_stats",
+    "qdp_pool_hook_alloc", "qdp_pool_hook_free", "qdp_pool_eviction_log", "qdp_cache_register", "qdp_cache_acquire",
+    "qdp_cache_release", "qdp_cache_unregister", "qdp_cache_is_resident", "qdp_cache_id",
 ]
 
 QDP_ALL, QDP_EVEN, QDP_ODD = 0, 1, 2
@@ -85,6 +88,20 @@ DECLARED_SYMBOLS = {
     "qdp_lattice_sync": ([_P], _I),
     "qdp_kernel_launch_count": ([], ctypes.c_int64),
     "qdp_last_error": ([], ctypes.c_char_p),
+    "qdp_pool_create": ([_I, _Z, _PP], _I),
+    "qdp_pool_destroy": ([_P], _I),
+    "qdp_pool_alloc": ([_P, _Z, _PP], _I),
+    "qdp_pool_free": ([_P, _P], _I),
+    "qdp_pool_stats": ([_P, ctypes.POINTER(_Z)], _I),
+    "qdp_pool_hook_alloc": ([_Z, _P], _P),
+    "qdp_pool_hook_free": ([_P, _P], None),
+    "qdp_cache_register": ([_P, _P, _Z, _PP], _I),
+    "qdp_cache_acquire": ([_P, _I, _PP], _I),
+    "qdp_cache_release": ([_P], _I),
+    "qdp_cache_unregister": ([_P], _I),
+    "qdp_cache_is_resident": ([_P], _I),
+    "qdp_cache_id": ([_P], ctypes.c_int64),
+    "qdp_pool_eviction_log": ([_P, ctypes.POINTER(ctypes.c_int64), _I, ctypes.POINTER(_I)], _I),
 }
 for _name, (_args, _res) in DECLARED_SYMBOLS.items():
     _f = getattr(_lib, _name)
@@ -408,3 +425,98 @@ def qdp_sum(f: Field, subset: int = QDP_ALL) -> np.ndarray:
     out = np.empty(2 * _NCOMP[f.kind])
     _check(_lib.qdp_sum(f.handle, subset, out.ctypes.data))
     return (out[0::2] + 1j * out[1::2]).reshape(_SHAPE[f.kind])
+
+
+# ---- row f4: device memory pool and LRU residency manager (csrc/pool.cu) -----------------------
+class Pool:
+    def __init__(self, handle: int, device: int, nbytes: int):
+        self.handle, self.device, self.nbytes = handle, device, nbytes
+
+
+class Cached:
+    def __init__(self, handle: int, pool: Pool, host, nbytes: int):
+        self.handle, self.pool, self.host, self.nbytes = handle, pool, host, nbytes    # `host` keeps the buffer alive
+
+
+def qdp_pool_create(device: int, nbytes: int) -> Pool:
+    """device = -1: address-range-only pool (allocator and eviction policy without a GPU)."""
+    out = ctypes.c_void_p()
+    _check(_lib.qdp_pool_create(int(device), int(nbytes), ctypes.byref(out)))
+    return Pool(out.value, device, nbytes)
+
+
+def qdp_pool_destroy(pool: Pool) -> None:
+    if pool.handle:
+        _check(_lib.qdp_pool_destroy(pool.handle))     # fails (and keeps the pool) while objects are registered
+        pool.handle = None
+
+
+def qdp_pool_alloc(pool: Pool, nbytes: int) -> int:
+    out = ctypes.c_void_p()
+    _check(_lib.qdp_pool_alloc(pool.handle, int(nbytes), ctypes.byref(out)))
+    return out.value
+
+
+def qdp_pool_free(pool: Pool, ptr: int) -> None:
+    _check(_lib.qdp_pool_free(pool.handle, ptr))
+
+
+def qdp_pool_stats(pool: Pool) -> dict:
+    out = (_Z * 4)()
+    _check(_lib.qdp_pool_stats(pool.handle, out))
+    return {"capacity": out[0], "in_use": out[1], "largest_free": out[2], "free_blocks": out[3]}
+
+
+def qdp_pool_hook_alloc():
+    """The pool's qdp_set_allocator-compatible entry points as raw function addresses: (alloc, free)."""
+    return ctypes.cast(_lib.qdp_pool_hook_alloc, _P).value, ctypes.cast(_lib.qdp_pool_hook_free, _P).value
+
+
+def qdp_pool_hook_free():
+    return qdp_pool_hook_alloc()[1]
+
+
+def qdp_pool_eviction_log(pool: Pool) -> list:
+    n = _I()
+    _check(_lib.qdp_pool_eviction_log(pool.handle, None, 0, ctypes.byref(n)))
+    ids = (ctypes.c_int64 * max(1, n.value))()
+    _check(_lib.qdp_pool_eviction_log(pool.handle, ids, n.value, ctypes.byref(n)))
+    return [int(ids[i]) for i in range(n.value)]
+
+
+def qdp_cache_register(pool: Pool, host, nbytes: int | None = None) -> Cached:
+    """host: a (pinned) CPU torch tensor or a numpy array holding the object's bytes, or None with an explicit size
+    for an address-range-only pool."""
+    if host is None:
+        ptr, size = None, int(nbytes)
+    elif isinstance(host, np.ndarray):
+        ptr, size = host.ctypes.data, host.nbytes
+    else:
+        ptr, size = host.data_ptr(), host.numel() * host.element_size()
+    out = ctypes.c_void_p()
+    _check(_lib.qdp_cache_register(pool.handle, ptr, size, ctypes.byref(out)))
+    return Cached(out.value, pool, host, size)
+
+
+def qdp_cache_acquire(c: Cached, for_write: bool = False) -> int:
+    out = ctypes.c_void_p()
+    _check(_lib.qdp_cache_acquire(c.handle, int(bool(for_write)), ctypes.byref(out)))
+    return out.value
+
+
+def qdp_cache_release(c: Cached) -> None:
+    _check(_lib.qdp_cache_release(c.handle))
+
+
+def qdp_cache_unregister(c: Cached) -> None:
+    h, c.handle = c.handle, None
+    if h:
+        _check(_lib.qdp_cache_unregister(h))
+
+
+def qdp_cache_is_resident(c: Cached) -> bool:
+    return bool(_lib.qdp_cache_is_resident(c.handle))
+
+
+def qdp_cache_id(c: Cached) -> int:
+    return int(_lib.qdp_cache_id(c.handle))

@@ -22,6 +22,7 @@ static int fail(int code, const char* fmt, ...) {
     va_end(ap);
     return code;
 }
+namespace qdp { int set_error(int code, const char* msg) { return fail(code, "%s", msg); } }   // for pool.cu
 #define CUDA_TRY(expr)                                                                     \
     do {                                                                                   \
         cudaError_t e_ = (expr);                                                           \

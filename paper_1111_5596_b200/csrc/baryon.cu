@@ -43,16 +43,20 @@ __global__ void __launch_bounds__(kBtThreads) baryon_ts_kernel(Geom g, BaryonArg
             Cx<T> o[4];
 #pragma unroll
             for (int i = 0; i < 4; i++) o[i] = cx<T>(0, 0);
-#pragma unroll
+            // not unrolled: unrolled, ptxas hoists the loads of all six permutations and spills ~1.8 KB per thread
+#pragma unroll 1
             for (int ps = 0; ps < NPERM; ps++) {
                 // source colours (a', b', c'): the even permutations first, as in the definition
                 const int sa = NSRC == 3 ? (ps < 3 ? ps : (ps == 3 ? 0 : (ps == 4 ? 2 : 1))) : 0;
                 const int sb = NSRC == 3 ? (ps < 3 ? (ps + 1) % 3 : (ps == 3 ? 2 : (ps == 4 ? 1 : 0))) : 0;
                 const int sc = NSRC == 3 ? 3 - sa - sb : 0;
                 const T sgn = ps < 3 ? T(1) : T(-1);
-                const T2* pa = site_ptr(static_cast<const T2*>(args.q[0][sa]), 12, 0, s);
-                const T2* pb = site_ptr(static_cast<const T2*>(args.q[1][sb]), 12, 0, s);
-                const T2* pc = site_ptr(static_cast<const T2*>(args.q[2][sc]), 12, 0, s);
+                auto pick = [&](int quark, int col) {      // select chain: a run-time index into the parameter struct would copy it to local memory
+                    return static_cast<const T2*>(col == 0 ? args.q[quark][0] : (col == 1 ? args.q[quark][1] : args.q[quark][2]));
+                };
+                const T2* pa = site_ptr(pick(0, sa), 12, 0, s);
+                const T2* pb = site_ptr(pick(1, sb), 12, 0, s);
+                const T2* pc = site_ptr(pick(2, sc), 12, 0, s);
                 Cx<T> M[9];
 #pragma unroll
                 for (int i = 0; i < 9; i++) M[i] = cx<T>(0, 0);
