@@ -336,6 +336,20 @@ int qdp_expr_trace_mul(qdp_field* dst, const qdp_field* a, int slot_a, int adj_a
 int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a, const qdp_field* b, int slot_b, int adj_b,
                            int mu, int sign, qdp_subset subset, double out[2]);
 
+/* ---- faces for an x3-slab decomposition over several GPUs ----------------------
+ * The paper is single-GPU (multi-GPU "future work") and BASELINE.json fixes one GPU, so bench.py runs
+ * replicas only; these calls are the device half of the decomposition SURVEY.md 8(e) describes: every rank owns a slab
+ * of L3/N time-slices as a lattice of its own, a shift along x3 becomes one exchange of a boundary time-slice and a
+ * global sum becomes an all-reduce of doubles (paper_1111_5596_b200/slab.py does the exchange with torch.distributed).
+ *   qdp_field_get_timeslice: dev_buf <- the sites with x3 = t of f (both parities), qdp_field_timeslice_bytes(f) bytes
+ *                            of device memory in a private layout that qdp_field_set_timeslice of any lattice with
+ *                            the same L0, L1, L2 and a field of the same kind and precision understands.
+ *   qdp_field_set_timeslice: the sites with x3 = t of f that belong to `subset` <- dev_buf; other sites untouched.
+ * Both asynchronous on the lattice's stream. */
+int qdp_field_timeslice_bytes(const qdp_field* f, size_t* out);
+int qdp_field_get_timeslice(const qdp_field* f, int t, void* dev_buf, size_t bytes);
+int qdp_field_set_timeslice(qdp_field* f, int t, const void* dev_buf, size_t bytes, qdp_subset subset);
+
 /* ---- device memory pool and LRU residency manager --------------------------
  * The paper's memory layer: "the pool manager grabs a large chunk of GPU memory at start-up" and a
  * software cache "decides host/device affiliation per lattice object and spills least-recently-used objects" when an

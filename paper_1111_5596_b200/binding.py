@@ -21,6 +21,7 @@ __all__ = [
     "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_project_max_retr", "qdp_baryon_timeslices", "qdp_matmul", "qdp_matvec", "qdp_axpby", "qdp_expr_plaquette", "qdp_expr_staple", "qdp_expr_ape_blend", "qdp_expr_trace_mul", "qdp_expr_sum_trace_mul", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
+    "qdp_field_timeslice_bytes", "qdp_field_get_timeslice", "qdp_field_set_timeslice",
     "Pool", "Cached", "qdp_pool_create", "qdp_pool_destroy", "qdp_pool_alloc", "qdp_pool_free", "qdp_pool_stats",
     "qdp_pool_hook_alloc", "qdp_pool_hook_free", "qdp_pool_eviction_log", "qdp_cache_register", "qdp_cache_acquire",
     "qdp_cache_release", "qdp_cache_unregister", "qdp_cache_is_resident", "qdp_cache_id",
@@ -88,6 +89,9 @@ DECLARED_SYMBOLS = {
     "qdp_lattice_sync": ([_P], _I),
     "qdp_kernel_launch_count": ([], ctypes.c_int64),
     "qdp_last_error": ([], ctypes.c_char_p),
+    "qdp_field_timeslice_bytes": ([_P, ctypes.POINTER(_Z)], _I),
+    "qdp_field_get_timeslice": ([_P, _I, _P, _Z], _I),
+    "qdp_field_set_timeslice": ([_P, _I, _P, _Z, _I], _I),
     "qdp_pool_create": ([_I, _Z, _PP], _I),
     "qdp_pool_destroy": ([_P], _I),
     "qdp_pool_alloc": ([_P, _Z, _PP], _I),
@@ -425,6 +429,20 @@ def qdp_sum(f: Field, subset: int = QDP_ALL) -> np.ndarray:
     out = np.empty(2 * _NCOMP[f.kind])
     _check(_lib.qdp_sum(f.handle, subset, out.ctypes.data))
     return (out[0::2] + 1j * out[1::2]).reshape(_SHAPE[f.kind])
+
+
+def qdp_field_timeslice_bytes(f: Field) -> int:
+    out = _Z()
+    _check(_lib.qdp_field_timeslice_bytes(f.handle, ctypes.byref(out)))
+    return out.value
+
+
+def qdp_field_get_timeslice(f: Field, t: int, dev_ptr: int, nbytes: int) -> None:
+    _check(_lib.qdp_field_get_timeslice(f.handle, int(t), dev_ptr, int(nbytes)))
+
+
+def qdp_field_set_timeslice(f: Field, t: int, dev_ptr: int, nbytes: int, subset: int = QDP_ALL) -> None:
+    _check(_lib.qdp_field_set_timeslice(f.handle, int(t), dev_ptr, int(nbytes), subset))
 
 
 # ---- row f4: device memory pool and LRU residency manager (csrc/pool.cu) -----------------------

@@ -427,6 +427,29 @@ extern "C" int qdp_field_copy(qdp_field* dst, const qdp_field* src) {
     return QDP_OK;
 }
 
+// ---- time-slice faces for an x3-slab decomposition (row f4 / SURVEY.md 8(e)) ---------------------
+static int timeslice_common(const char* who, qdp_field* f, int t, void* dev_buf, size_t bytes, int subset, bool to_face) {
+    if (!ok_field(f) || !dev_buf || !ok_subset(subset)) return fail(QDP_ERR_ARG, "%s: bad argument", who);
+    qdp_lattice* l = f->lat;
+    if (t < 0 || t >= l->geom.L3) return fail(QDP_ERR_ARG, "%s: t = %d outside 0..%d", who, t, l->geom.L3 - 1);
+    const size_t need = (size_t)2 * f->ncomp * l->geom.s3 * elem_bytes(f->prec);
+    if (bytes < need) return fail(QDP_ERR_ARG, "%s: buffer of %zu bytes, %zu needed", who, bytes, need);
+    ENTER(l);
+    CUDA_TRY(launch_timeslice(f->prec, l->geom, f->ncomp, f->data, dev_buf, t, subset, to_face, l->stream));
+    return QDP_OK;
+}
+extern "C" int qdp_field_get_timeslice(const qdp_field* f, int t, void* dev_buf, size_t bytes) {
+    return timeslice_common("qdp_field_get_timeslice", const_cast<qdp_field*>(f), t, dev_buf, bytes, QDP_ALL, true);
+}
+extern "C" int qdp_field_set_timeslice(qdp_field* f, int t, const void* dev_buf, size_t bytes, qdp_subset subset) {
+    return timeslice_common("qdp_field_set_timeslice", f, t, const_cast<void*>(dev_buf), bytes, subset, false);
+}
+extern "C" int qdp_field_timeslice_bytes(const qdp_field* f, size_t* out) {
+    if (!ok_field(f) || !out) return fail(QDP_ERR_ARG, "qdp_field_timeslice_bytes: bad argument");
+    *out = (size_t)2 * f->ncomp * f->lat->geom.s3 * elem_bytes(f->prec);
+    return QDP_OK;
+}
+
 // ---- expressions ---------------------------------------------------------------
 extern "C" int qdp_shift(qdp_field* dst, const qdp_field* src, int mu, int sign, qdp_subset subset) {
     if (!ok_field(dst) || !ok_field(src)) return fail(QDP_ERR_ARG, "qdp_shift: not a field");

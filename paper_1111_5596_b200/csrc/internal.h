@@ -25,6 +25,10 @@ cudaError_t launch_soa_to_aos(int prec, const Geom& g, int ncomp, const void* fi
 cudaError_t launch_neighbor_table(const Geom& g, int mu, int sign, int32_t* out_lex, cudaStream_t st);
 cudaError_t launch_parity_mask(const Geom& g, uint8_t* out_lex, cudaStream_t st);
 
+// face of the sites with x3 = t: field -> buf (to_face) or buf -> field on the sites of `subset`; buf holds 2 * ncomp * s3 elements
+cudaError_t launch_timeslice(int prec, const Geom& g, int ncomp, void* field, void* buf, int t, int subset, bool to_face,
+                             cudaStream_t st);
+
 // shift.cu
 cudaError_t launch_shift(int prec, const Geom& g, int ncomp, void* dst, const void* src, int mu,
                          int sign, int subset, cudaStream_t st);

@@ -85,6 +85,40 @@ cudaError_t launch_soa_to_aos(int prec, const Geom& g, int ncomp, const void* fi
                 : launch_transpose<float2, false>(g, ncomp, stage, (void*)field, lex_begin, nsites, st);
 }
 
+// ---- time-slice faces (the face an x3-slab decomposition exchanges) --------------
+// The sites with x3 = t are the half-indices [t s3, (t+1) s3) of each parity.  Face buffer layout (private, only
+// meaningful for lattices with the same L0, L1, L2), indexed by the SPATIAL parity q = (x0 + x1 + x2) & 1 = (p + t) & 1
+// so that a face does not depend on the slice it was taken from or is written to (a site and its x3 neighbour have the
+// same half-index offset k inside their slices but opposite parities):
+//     buf[(q * ncomp + c) * s3 + k] = element(c, p Vhp + t s3 + k),   p = (q + t) & 1.
+// TO_FACE: field -> buffer (both parities); else buffer -> field, writing only the sites of `subset`.
+template <class T2, bool TO_FACE>
+__global__ void __launch_bounds__(256) timeslice_kernel(Geom g, int ncomp, T2* __restrict__ field, T2* __restrict__ buf, int t,
+                                                       int subset) {
+    const int n = 2 * ncomp * g.s3;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+        const int k = e % g.s3, qc = e / g.s3, c = qc % ncomp, p = (qc / ncomp + t) & 1;
+        if (!TO_FACE && subset != 0 && p != (subset == 2)) continue;
+        const size_t fe = field_elem(ncomp, c, p * g.Vhp + t * g.s3 + k);
+        if (TO_FACE) buf[e] = field[fe]; else field[fe] = buf[e];
+    }
+}
+cudaError_t launch_timeslice(int prec, const Geom& g, int ncomp, void* field, void* buf, int t, int subset, bool to_face,
+                             cudaStream_t st) {
+    const int n = 2 * ncomp * g.s3;
+    int blocks = (n + 255) / 256;
+    if (blocks > 4096) blocks = 4096;
+    if (prec) {
+        if (to_face) timeslice_kernel<double2, true><<<blocks, 256, 0, st>>>(g, ncomp, (double2*)field, (double2*)buf, t, subset);
+        else         timeslice_kernel<double2, false><<<blocks, 256, 0, st>>>(g, ncomp, (double2*)field, (double2*)buf, t, subset);
+    } else {
+        if (to_face) timeslice_kernel<float2, true><<<blocks, 256, 0, st>>>(g, ncomp, (float2*)field, (float2*)buf, t, subset);
+        else         timeslice_kernel<float2, false><<<blocks, 256, 0, st>>>(g, ncomp, (float2*)field, (float2*)buf, t, subset);
+    }
+    g_launch_count++;
+    return cudaGetLastError();
+}
+
 // out[lex(x)] = lex(x + sign*mu_hat): decoded and stepped with the very functions
 // the expression kernels use, so the parity test of the table pins them.
 __global__ void neighbor_table_kernel(Geom g, int mu, int sign, int32_t* __restrict__ out) {
