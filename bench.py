@@ -55,17 +55,11 @@ def fp64_flops_per_site(op: str) -> int:
 
 def probe_dfma_rate(device: int, stream) -> float | None:
     """DFMA per second (thread-level) of the plain fp64 pipe, measured now on this device (bench-only probe library)."""
-    import ctypes
-    from paper_1111_5596_b200.build import PROBE_LIB
     try:
-        lib = ctypes.CDLL(PROBE_LIB)
-    except OSError:
+        from paper_1111_5596_b200 import probe
+        return probe.dfma_rate(device, stream)
+    except (OSError, RuntimeError):
         return None
-    lib.qdp_probe_dfma.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
-    lib.qdp_probe_dfma.restype = ctypes.c_int
-    out = ctypes.c_double()
-    rc = lib.qdp_probe_dfma(device, stream, 5, ctypes.byref(out))
-    return out.value if rc == 0 else None
 
 
 def algorithmic_bytes(V: int, eb: int) -> dict:

@@ -1,0 +1,70 @@
+"""Peak and overlap probes (csrc/probe.cu -> libqdp_probe.so; bench-only, not part of the C ABI of include/qdp_b200.h).
+
+    python -m paper_1111_5596_b200.probe            # prints the tables quoted in profiles/r2_microbench.md
+
+bench.py uses dfma_rate() as the measured denominator of the fp64 ("alu") roofline view."""
+from __future__ import annotations
+
+import ctypes
+
+from .build import PROBE_LIB
+
+_lib = None
+
+
+def _get():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(PROBE_LIB)
+        D = ctypes.POINTER(ctypes.c_double)
+        lib.qdp_probe_dfma.argtypes, lib.qdp_probe_dfma.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, D], ctypes.c_int
+        lib.qdp_probe_mix.argtypes, lib.qdp_probe_mix.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
+        lib.qdp_probe_dfma_chain.argtypes, lib.qdp_probe_dfma_chain.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _call(fn, *args) -> float:
+    out = ctypes.c_double()
+    rc = fn(*args, ctypes.byref(out))
+    if rc != 0:
+        raise RuntimeError(f"{fn.__name__} failed with cudaError {rc}")
+    return out.value
+
+
+def dfma_rate(device: int = 0, stream=None, reps: int = 5) -> float:
+    """Thread-level DFMA per second of the plain fp64 pipe at saturation."""
+    return _call(_get().qdp_probe_dfma, device, stream, reps)
+
+
+def mix_ms_per_step(mode: int, nlds: int = 36, device: int = 0, stream=None) -> float:
+    """mode: bit 0 LDS.128, bit 1 DFMA, bit 2 bulk copies into shared memory; see csrc/probe.cu."""
+    return _call(_get().qdp_probe_mix, device, stream, mode, nlds)
+
+
+def dfma_chain_ns(warps: int, chains: int, device: int = 0, stream=None) -> float:
+    return _call(_get().qdp_probe_dfma_chain, device, stream, warps, chains)
+
+
+def main() -> None:
+    import torch
+    dev = torch.cuda.current_device()
+    props = torch.cuda.get_device_properties(dev)
+    ghz = 1.965      # clocks.max.sm of the B200s of this pool; cycles below are quoted at that clock
+    r = dfma_rate(dev)
+    print(f"{props.name}, {props.multi_processor_count} SMs")
+    print(f"DFMA rate, 12 warps/SM x 8 chains: {r / 1e12:.2f} T DFMA/s = {r / props.multi_processor_count / (ghz * 1e9):.1f} lanes/clk/SM at {ghz} GHz")
+    for warps, chains in ((1, 1), (1, 2), (1, 4), (4, 8)):
+        ns = dfma_chain_ns(warps, chains, dev)
+        print(f"DFMA, {warps} warp(s)/SM, {chains} chain(s): {ns * ghz:.2f} cycles per DFMA of a warp")
+    print("per step: 12 warps x (N LDS.128 + 234 DFMA) [+ 92,160 B of bulk copies]; floors: 36 LDS -> 1728 cycles, DFMA 1404 cycles")
+    rows = [("LDS(36) only", 1, 36), ("DFMA only", 2, 36), ("LDS(36) + DFMA", 3, 36), ("bulk copies only", 4, 36),
+            ("LDS(36) + bulk", 5, 36), ("DFMA + bulk", 6, 36), ("LDS(36) + DFMA + bulk", 7, 36),
+            ("LDS(28) + DFMA", 3, 28), ("LDS(24) + DFMA", 3, 24), ("LDS(18) + DFMA", 3, 18), ("LDS(28) + DFMA + bulk", 7, 28)]
+    for name, mode, nl in rows:
+        ms = mix_ms_per_step(mode, nl, dev)
+        print(f"{name:24s} {ms * 1e3:7.3f} us/step = {ms * 1e-3 * ghz * 1e9:6.0f} cycles/step")
+
+
+if __name__ == "__main__":
+    main()
