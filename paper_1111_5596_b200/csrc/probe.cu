@@ -80,6 +80,65 @@ __global__ void __launch_bounds__(416, 1) mix_kernel(double* out, const double2*
     if (t == 123.456) out[0] = t;
 }
 
+// ---- do operand loads and DFMAs of the SAME warp overlap? -------------------------------------------------------
+// The register kernels (plaquette.cu, ape.cu, hop.cu) run 2 warps per sub-partition at 255 registers; their measured
+// times are close to (L1 data-pipe time) + (fp64 pipe time).  This probe isolates the cause: NW warps per SM, per step
+// and warp NL 128-bit loads (SRC 0: LDS from shared memory, SRC 1: LDG that hits L1) and 234 DFMAs on the loaded values;
+// PIPE 0: the loads of a step are issued at its start (a warp alternates between a load phase and an arithmetic phase,
+// only other warps can fill the gaps), PIPE 1: the loads of step s+1 are issued before the arithmetic of step s
+// (register double buffer), so one warp has both pipes busy at once.  MODE bit 0: loads, bit 1: DFMAs.
+template <int MODE, int NL, int SRC, int PIPE, int NW>
+__global__ void __launch_bounds__(NW * 32, 1) overlap_kernel(double* out, const double2* __restrict__ gsrc, int steps, double a, double b) {
+    extern __shared__ __align__(128) unsigned char smem_probe[];
+    double2* tile = reinterpret_cast<double2*>(smem_probe);                 // 96 KB = 192 planes of 32 double2
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const double2* src = SRC ? gsrc + (size_t)blockIdx.x * 6144 : tile;
+    if (!SRC) for (int i = threadIdx.x; i < 6144; i += blockDim.x) tile[i] = make_double2(i * 1e-6, 1.0 - i * 1e-6);
+    __syncthreads();
+    double acc[18];
+#pragma unroll
+    for (int i = 0; i < 18; i++) acc[i] = lane * 1e-9 + i;
+    double2 sink = make_double2(0, 0);
+    auto load = [&](double2 (&m)[NL], int s) {
+#pragma unroll
+        for (int c = 0; c < NL; c++) {
+            const double2* q = src + ((warp * NL + c + s) % 192) * 32 + lane;
+            m[c] = (MODE & 1) ? (SRC ? __ldg(q) : *q) : make_double2(a + c, b - c);
+        }
+    };
+    auto math = [&](const double2 (&m)[NL]) {
+        if (MODE & 2) {
+#pragma unroll
+            for (int r = 0; r < 13; r++)
+#pragma unroll
+                for (int i = 0; i < 18; i++) acc[i] = fma(acc[i], (r & 1) ? m[(i + r) % NL].x : m[(i + r + NL / 2) % NL].y, b);
+        } else {
+#pragma unroll
+            for (int c = 0; c < NL; c++) { sink.x += m[c].x; sink.y += m[c].y; }
+        }
+    };
+    if (PIPE) {
+        double2 m0[NL], m1[NL];
+        load(m0, 0);
+        for (int s = 0; s < steps; s += 2) {
+            load(m1, s + 1);
+            math(m0);
+            load(m0, s + 2);
+            math(m1);
+        }
+    } else {
+        for (int s = 0; s < steps; s++) {
+            double2 m[NL];
+            load(m, s);
+            math(m);
+        }
+    }
+    double t = sink.x + sink.y;
+#pragma unroll
+    for (int i = 0; i < 18; i++) t += acc[i];
+    if (t == 123.456) out[0] = t;
+}
+
 template <int CHAINS>
 __global__ void dfma_chain_kernel(double* out, int iters, double a, double b) {
     double v[CHAINS];
@@ -160,6 +219,45 @@ extern "C" int qdp_probe_mix(int device, void* stream, int mode, int nlds, doubl
             default: e = QDP_MIX(7); break;
         }
 #undef QDP_MIX
+    }
+    if (e == cudaSuccess) *ms_per_step = (double)ms / steps;
+    if (out) cudaFree(out);
+    if (src) cudaFree(src);
+    cudaSetDevice(prev);
+    return (int)e;
+}
+
+template <int MODE, int SRC, int PIPE, int NW>
+cudaError_t run_overlap(cudaStream_t st, int sms, double* out, const double2* src, int steps, float* ms) {
+    const int smem = 98304;
+    cudaError_t e = cudaFuncSetAttribute(overlap_kernel<MODE, 24, SRC, PIPE, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    return time_launches(st, 7, ms, [&] { overlap_kernel<MODE, 24, SRC, PIPE, NW><<<sms, NW * 32, smem, st>>>(out, src, steps, 1.0000001, 1e-9); });
+}
+
+// mode: bit 0 loads (24 x 128 bit per warp and step), bit 1 DFMAs (234 per warp and step); src: 0 shared memory, 1 global
+// memory resident in L1; pipe: 0 load phase then arithmetic phase, 1 loads of the next step issued before the arithmetic
+// of this one; warps: 8 (2 per sub-partition, what the 255-register kernels run).  *ms_per_step = median time / steps.
+extern "C" int qdp_probe_overlap(int device, void* stream, int mode, int src_kind, int pipe, double* ms_per_step) {
+    if (!ms_per_step || mode < 1 || mode > 3 || src_kind < 0 || src_kind > 1 || pipe < 0 || pipe > 1) return (int)cudaErrorInvalidValue;
+    cudaError_t e;
+    int prev = 0, sms = 0;
+    if ((e = cudaGetDevice(&prev)) != cudaSuccess) return (int)e;
+    if ((e = cudaSetDevice(device)) != cudaSuccess) return (int)e;
+    cudaStream_t st = (cudaStream_t)stream;
+    double* out = nullptr;
+    double2* src = nullptr;
+    const int steps = 400;
+    float ms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) e = cudaMalloc(&out, 64);
+    if (e == cudaSuccess) e = cudaMalloc(&src, ((size_t)sms * 6144 + 64) * sizeof(double2));
+    if (e == cudaSuccess) e = cudaMemset(src, 0, ((size_t)sms * 6144 + 64) * sizeof(double2));
+    if (e == cudaSuccess) {
+#define QDP_OV(M) (src_kind == 0 ? (pipe ? run_overlap<M, 0, 1, 8>(st, sms, out, src, steps, &ms) : run_overlap<M, 0, 0, 8>(st, sms, out, src, steps, &ms)) \
+                                 : (pipe ? run_overlap<M, 1, 1, 8>(st, sms, out, src, steps, &ms) : run_overlap<M, 1, 0, 8>(st, sms, out, src, steps, &ms)))
+        e = mode == 1 ? QDP_OV(1) : mode == 2 ? QDP_OV(2) : QDP_OV(3);
+#undef QDP_OV
     }
     if (e == cudaSuccess) *ms_per_step = (double)ms / steps;
     if (out) cudaFree(out);

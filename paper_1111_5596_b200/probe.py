@@ -20,6 +20,7 @@ def _get():
         lib.qdp_probe_dfma.argtypes, lib.qdp_probe_dfma.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, D], ctypes.c_int
         lib.qdp_probe_mix.argtypes, lib.qdp_probe_mix.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
         lib.qdp_probe_dfma_chain.argtypes, lib.qdp_probe_dfma_chain.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
+        lib.qdp_probe_overlap.argtypes, lib.qdp_probe_overlap.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
         _lib = lib
     return _lib
 
@@ -46,6 +47,11 @@ def dfma_chain_ns(warps: int, chains: int, device: int = 0, stream=None) -> floa
     return _call(_get().qdp_probe_dfma_chain, device, stream, warps, chains)
 
 
+def overlap_ms_per_step(mode: int, src: int, pipe: int, device: int = 0, stream=None) -> float:
+    """8 warps/SM, per step and warp 24 128-bit loads (src 0: LDS, 1: LDG hitting L1) and 234 DFMA; see csrc/probe.cu."""
+    return _call(_get().qdp_probe_overlap, device, stream, mode, src, pipe)
+
+
 def main() -> None:
     import torch
     dev = torch.cuda.current_device()
@@ -64,6 +70,12 @@ def main() -> None:
     for name, mode, nl in rows:
         ms = mix_ms_per_step(mode, nl, dev)
         print(f"{name:24s} {ms * 1e3:7.3f} us/step = {ms * 1e-3 * ghz * 1e9:6.0f} cycles/step")
+    print("8 warps/SM (2 per sub-partition), per step and warp 24 x 128-bit loads + 234 DFMA; floors: loads 768 cycles, DFMA 936 cycles")
+    for src, sname in ((0, "LDS"), (1, "LDG, L1 hit")):
+        for name, mode, pipe in (("loads only", 1, 0), ("DFMA only", 2, 0), ("loads, then DFMA (per warp)", 3, 0),
+                                 ("loads of step s+1 before DFMA of step s", 3, 1)):
+            ms = overlap_ms_per_step(mode, src, pipe, dev)
+            print(f"{sname:12s} {name:42s} {ms * 1e3:7.3f} us/step = {ms * 1e-3 * ghz * 1e9:6.0f} cycles/step")
 
 
 if __name__ == "__main__":
