@@ -28,6 +28,7 @@ namespace qdp {
 #define APE_THREADS 128
 #endif
 constexpr int kApeThreads = APE_THREADS;
+
 // A never-taken branch ptxas cannot predicate away: it ends the basic block.  The unrolled
 // directions would otherwise merge into one block of ~5000 instructions in which ptxas hoists
 // the loads of all directions to the top and spills 2-4 KB per thread (measured: 1.96 ms).
@@ -50,6 +51,8 @@ ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out, const typename Vec2
     using T2 = typename Vec2<T>::type;
     constexpr int ND = FOURD ? 4 : 3;        // smeared directions
     constexpr int NS = 2 * (ND - 1);         // staples per link
+    // fp32, 4-D: the products run on (re, im) register pairs (su3.cuh: *_pk; 0.85 -> 0.76 ms on 32^3 x 64)
+    constexpr bool kPk = sizeof(T) == 4 && FOURD;
     const int i = blockIdx.x * kApeThreads + threadIdx.x;
     int p, h;
     if (i >= work_items(g, subset) || !work_site(g, subset, i, p, h)) return;
@@ -90,21 +93,28 @@ ape_kernel(Geom g, typename Vec2<T>::type* __restrict__ out, const typename Vec2
     };
 
     Mat3<T> A = ld_mat_at<T>(ptrA(0, 0)), B = ld_mat_at<T>(ptrB(0, 0));
-#pragma unroll
+    // 4-D: the direction loop stays rolled.  Unrolled, the 24 staples and 4 projections are ~160 KB of straight-line
+    // code, more than the instruction cache holds (32^3 x 64: fp64 2.56 ms unrolled, 1.43 ms unrolled by two,
+    // 1.38 ms rolled; fp32 0.83 -> 0.76 ms).  The spatial step is faster unrolled (fp64 0.73 ms against 0.81 ms rolled).
+    constexpr int kUnrollMu = FOURD ? 1 : ND;
+#pragma unroll kUnrollMu
     for (int mu = 0; mu < ND; mu++) {
         Mat3<T> S = mat_zero<T>();
         Mat3<T> U;
 #pragma unroll
         for (int k = 0; k < NS; k++) {
             Mat3<T> C = ld_mat_at<T>(ptrC(mu, k));
-            Mat3<T> Tm = (k & 1) ? adj_mul(A, B) : mul(A, B);
+            Mat3<T> Tm;
+            if constexpr (kPk) Tm = (k & 1) ? adj_mul_pk(A, B) : mul_pk(A, B);
+            else               Tm = (k & 1) ? adj_mul(A, B) : mul(A, B);
             if (k + 1 < NS) {
                 A = ld_mat_at<T>(ptrA(mu, k + 1));
                 B = ld_mat_at<T>(ptrB(mu, k + 1));
             } else {
                 U = ld_mat_at<T>(site_ptr(u, 36, mu * 9, sb));
             }
-            if (k & 1) mad_mul(S, Tm, C); else mad_mul_adj(S, Tm, C);
+            if constexpr (kPk) { if (k & 1) mad_mul_pk(S, Tm, C); else mad_mul_adj_pk(S, Tm, C); }
+            else               { if (k & 1) mad_mul(S, Tm, C); else mad_mul_adj(S, Tm, C); }
         }
         if (mu + 1 < ND) {   // first operands of the next direction, in flight during the projection
             A = ld_mat_at<T>(ptrA(mu + 1, 0));
