@@ -285,6 +285,9 @@ def run_ours(args) -> dict | None:
     extra_defs = {
         "smear_hop": (lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3), 51,
                       "qdp_smear_hop, t_dir = 3 (row f2): u 27 + psi 12 + chi 12 complex per site"),
+        "ape_4d": (lambda: q.qdp_ape_smear_step(u2, u, 0.5, -1), 72,
+                   "qdp_ape_smear_step, t_dir = -1 (row f2: 4-D APE, 6 staples per link, all four links projected): "
+                   "36 complex read + 36 written per site"),
         "inner_timeslices": (lambda: q.qdp_inner_timeslices(psi, chi), 24,
                              "qdp_inner_timeslices (row f3): 2 x 12 complex per site, includes the host round trip"),
         "reunitarize_gs": (lambda: q.qdp_reunitarize(u2, u, q.QDP_REUNIT_GRAM_SCHMIDT), 60,
