@@ -336,6 +336,42 @@ int qdp_expr_trace_mul(qdp_field* dst, const qdp_field* a, int slot_a, int adj_a
 int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a, const qdp_field* b, int slot_b, int adj_b,
                            int mu, int sign, qdp_subset subset, double out[2]);
 
+/* ---- Row f1, second step: run-time expressions -------------------------------------------------------------------
+ * The paper's scheme itself (the tree parser "generates the CUDA kernel code" of an expression, which is
+ * JIT-compiled and cached so that "each expression is compiled only once"): the expression arrives as text, is parsed
+ * and type-checked on the host, written out as a node type of the expression layer (csrc/expr.cuh), compiled with NVRTC
+ * for sm_100a into ONE kernel and cached by (expression, precision, assignment | sum).  The first use of an expression
+ * costs one compilation (0.2-0.4 s); later uses launch the cached kernel.  libnvrtc is loaded at the first compilation
+ * (QDP_ERR_CUDA with a message if it is missing); nothing is read from the file system.
+ *   expr   := term { '+' term }            term := factor { '*' factor }
+ *   factor := adj(expr) | trace(expr) | real(expr) | imag(expr) | shift(expr, +mu | -mu) | '(' expr ')' | leaf
+ *   leaf   := f<k> [ '[' slot ']' ]        matrix `slot` (a link of a gauge field; default 0) of field argument k = 0..3
+ *           | s<k>                         real scalar argument k = 0..3 (cast to the field precision)
+ * Semantics as in the build-time layer and SURVEY.md 8(c): a value is a 3x3 matrix, a complex number or a real number;
+ * adj = conjugate transpose (conjugate of a complex number), trace: matrix -> complex, real / imag: complex -> real,
+ * shift(e, +mu)(x) = e(x + mu) for the whole sub-expression e (A3), '+' needs equal kinds, '*' is matrix * matrix,
+ * real * anything, anything * real or complex * complex.  Field arguments: QDP_COLOR_MATRIX or QDP_GAUGE of one
+ * lattice and precision.
+ *   qdp_expr_jit_kind:    host only; *kind_out = 0 matrix, 1 complex, 2 real.  field_kinds[k] = qdp_kind of argument k.
+ *   qdp_expr_jit_compile: host only (NVRTC needs no device): compiles the kernel for (expr, prec, sum != 0) into the
+ *                         cache if it is not there; *cubin_bytes (optional) receives the size of its image.
+ *   qdp_expr_jit_assign:  dst[slot_d](x) = expr(x) for x in subset, other sites untouched.  A matrix expression needs a
+ *                         QDP_COLOR_MATRIX (slot_d = 0) or QDP_GAUGE destination, a complex one a QDP_COMPLEX destination
+ *                         (QDP_ERR_KIND).  dst may be an operand unless the expression contains a shift (QDP_ERR_ALIAS).
+ *                         Asynchronous.
+ *   qdp_expr_jit_sum:     out = (re, im) of sum_{x in subset} expr(x) for a real or complex expression (fp64
+ *                         accumulation, fixed order, not normalised).  Synchronous.
+ *   qdp_expr_jit_compilations: number of NVRTC compilations this process has done (cache misses).
+ * Syntax and kind errors are QDP_ERR_ARG with the position in qdp_last_error(). */
+int qdp_expr_jit_kind(const char* expr, const int* field_kinds, int nfields, int nscalars, int* kind_out);
+int qdp_expr_jit_compile(const char* expr, const int* field_kinds, int nfields, int nscalars, qdp_prec prec, int sum,
+                         size_t* cubin_bytes);
+int qdp_expr_jit_assign(qdp_field* dst, int slot_d, const char* expr, const qdp_field* const* fields, int nfields,
+                        const double* scalars, int nscalars, qdp_subset subset);
+int qdp_expr_jit_sum(const char* expr, const qdp_field* const* fields, int nfields, const double* scalars, int nscalars,
+                     qdp_subset subset, double out[2]);
+int64_t qdp_expr_jit_compilations(void);
+
 /* ---- faces for an x3-slab decomposition over several GPUs ----------------------
  * The paper is single-GPU (multi-GPU "future work") and BASELINE.json fixes one GPU, so bench.py runs
  * replicas only; these calls are the device half of the decomposition SURVEY.md 8(e) describes: every rank owns a slab

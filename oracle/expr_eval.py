@@ -1,0 +1,206 @@
+"""ORACLE -- test infrastructure, not the product.
+
+Run-time lattice expressions (second step), evaluated the slow and obvious
+way: every sub-expression becomes a whole-lattice numpy array (exactly the temporaries QDP++ avoids), one node at a time,
+in the order the expression is written.  Shares nothing with ``csrc/jit.cu``: own tokenizer, own recursive descent.
+
+Grammar (the same language the library documents in ``include/qdp_b200.h``):
+
+    expr   := term { '+' term }          term := factor { '*' factor }
+    factor := adj(expr) | trace(expr) | real(expr) | imag(expr) | shift(expr, +mu | -mu) | '(' expr ')' | leaf
+    leaf   := f<k> [ '[' slot ']' ]  |  s<k>
+
+Values: matrix field [V,3,3] complex128, complex field [V] complex128, real field [V] float64 (a scalar argument is a
+constant real field).  adj = conjugate transpose / complex conjugate / identity on reals; trace over the colour indices;
+shift(e, +mu)(x) = e(x + mu) with periodic wrap (reading A3), done by ``oracle.shift`` on the evaluated array; '*' is
+the per-site matrix product, or scaling by a real, or the product of complex numbers; '+' adds values of equal kind.
+"""
+from __future__ import annotations
+
+import re
+
+import numpy as np
+
+from . import shift as _shift, volume as _volume
+
+MAT, CPLX, REAL = 0, 1, 2
+_TOKEN = re.compile(r"\s*(adj|trace|real|imag|shift|f\d|s\d|[()\[\],+\-*]|\d)")
+
+
+class ExprError(ValueError):
+    pass
+
+
+def tokenize(text: str) -> list[str]:
+    out, pos = [], 0
+    text = text.rstrip()
+    while pos < len(text):
+        m = _TOKEN.match(text, pos)
+        if not m:
+            raise ExprError(f"bad input at {text[pos:pos + 12]!r}")
+        out.append(m.group(1))
+        pos = m.end()
+    return out
+
+
+def parse(text: str):
+    """Returns a nested tuple tree: ('f', k, slot) | ('s', k) | ('adj'|'trace'|'real'|'imag', e) | ('shift', e, mu, sign)
+    | ('+', a, b) | ('*', a, b); '+' and '*' associate to the left, '*' binds tighter."""
+    toks = tokenize(text)
+    pos = 0
+
+    def peek():
+        return toks[pos] if pos < len(toks) else None
+
+    def take(want=None):
+        nonlocal pos
+        t = peek()
+        if t is None or (want is not None and t != want):
+            raise ExprError(f"{want!r} expected, got {t!r}")
+        pos += 1
+        return t
+
+    def expr():
+        node = term()
+        while peek() == "+":
+            take()
+            node = ("+", node, term())
+        return node
+
+    def term():
+        node = factor()
+        while peek() == "*":
+            take()
+            node = ("*", node, factor())
+        return node
+
+    def factor():
+        t = take()
+        if t in ("adj", "trace", "real", "imag"):
+            take("(")
+            e = expr()
+            take(")")
+            return (t, e)
+        if t == "shift":
+            take("(")
+            e = expr()
+            take(",")
+            sign = {"+": 1, "-": -1}.get(take())
+            if sign is None:
+                raise ExprError("'+' or '-' expected in shift")
+            mu = int(take())
+            take(")")
+            return ("shift", e, mu, sign)
+        if t == "(":
+            e = expr()
+            take(")")
+            return e
+        if t[0] == "f" and len(t) == 2:
+            slot = 0
+            if peek() == "[":
+                take()
+                slot = int(take())
+                take("]")
+            return ("f", int(t[1]), slot)
+        if t[0] == "s" and len(t) == 2:
+            return ("s", int(t[1]))
+        raise ExprError(f"operand expected, got {t!r}")
+
+    tree = expr()
+    if pos != len(toks):
+        raise ExprError(f"unexpected {toks[pos]!r}")
+    return tree
+
+
+def kind_of(tree, field_slots) -> int:
+    """Value kind of the expression; field_slots[k] = number of matrices per site of field argument k (1 or 4).
+    Raises ExprError for the combinations the language does not define."""
+    op = tree[0]
+    if op == "f":
+        if tree[1] >= len(field_slots) or tree[2] >= field_slots[tree[1]]:
+            raise ExprError("field argument or slot out of range")
+        return MAT
+    if op == "s":
+        return REAL
+    if op in ("adj", "shift"):
+        if op == "shift" and not 0 <= tree[2] <= 3:
+            raise ExprError("direction must be 0..3")
+        return kind_of(tree[1], field_slots)
+    if op == "trace":
+        if kind_of(tree[1], field_slots) != MAT:
+            raise ExprError("trace() takes a matrix")
+        return CPLX
+    if op in ("real", "imag"):
+        if kind_of(tree[1], field_slots) != CPLX:
+            raise ExprError(f"{op}() takes a complex number")
+        return REAL
+    a, b = kind_of(tree[1], field_slots), kind_of(tree[2], field_slots)
+    if op == "+":
+        if a != b:
+            raise ExprError("'+' needs operands of the same kind")
+        return a
+    if a == REAL:
+        return b
+    if b == REAL:
+        return a
+    if a == b:
+        return a
+    raise ExprError("'*' of a matrix and a complex number is not defined")
+
+
+def evaluate(dims, text: str, fields, scalars=()):
+    """The expression at every site.  fields[k]: [V,3,3] (colour matrix) or [V,4,3,3] (gauge) complex arrays.
+    Returns ([V,3,3] | [V] complex128 | [V] float64, kind)."""
+    V = _volume(dims)
+    fields = [np.asarray(f, dtype=np.complex128).reshape(V, -1, 3, 3) for f in fields]
+    tree = parse(text)
+    kind = kind_of(tree, [f.shape[1] for f in fields])
+
+    def ev(t):
+        op = t[0]
+        if op == "f":
+            return fields[t[1]][:, t[2]].copy()
+        if op == "s":
+            return np.full(V, float(scalars[t[1]]))
+        if op == "adj":
+            v = ev(t[1])
+            return np.conj(np.swapaxes(v, 1, 2)) if v.ndim == 3 else np.conj(v)
+        if op == "trace":
+            v = ev(t[1])
+            return v[:, 0, 0] + v[:, 1, 1] + v[:, 2, 2]
+        if op == "real":
+            return np.ascontiguousarray(ev(t[1]).real)
+        if op == "imag":
+            return np.ascontiguousarray(ev(t[1]).imag)
+        if op == "shift":
+            return _shift(dims, np.ascontiguousarray(ev(t[1])), t[2], t[3])
+        a, b = ev(t[1]), ev(t[2])
+        if op == "+":
+            return a + b
+        if a.ndim == 3 and b.ndim == 3:
+            out = np.zeros_like(a)
+            for i in range(3):            # (a b)_ij = sum_k a_ik b_kj, written out
+                for j in range(3):
+                    for k in range(3):
+                        out[:, i, j] += a[:, i, k] * b[:, k, j]
+            return out
+        if a.ndim == 3:
+            return a * b[:, None, None]
+        if b.ndim == 3:
+            return a[:, None, None] * b
+        return a * b
+
+    return ev(tree), kind
+
+
+def total(dims, text: str, fields, scalars=(), mask=None) -> complex:
+    """sum over the sites (of the subset given by the boolean mask) of a real or complex expression, exactly rounded
+    (math.fsum) so that the comparison bar is the GPU's, not this sum's."""
+    import math
+    v, kind = evaluate(dims, text, fields, scalars)
+    if kind == MAT:
+        raise ExprError("a sum needs a real or complex expression")
+    if mask is not None:
+        v = v[mask]
+    v = np.asarray(v, dtype=np.complex128)
+    return complex(math.fsum(v.real), math.fsum(v.imag))

@@ -18,7 +18,7 @@ __all__ = [
     "qdp_lattice_neighbor_table", "qdp_lattice_parity_mask", "qdp_lattice_sync",
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
-    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_project_max_retr", "qdp_baryon_timeslices", "qdp_matmul", "qdp_matvec", "qdp_axpby", "qdp_expr_plaquette", "qdp_expr_staple", "qdp_expr_ape_blend", "qdp_expr_trace_mul", "qdp_expr_sum_trace_mul", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
+    "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_project_max_retr", "qdp_baryon_timeslices", "qdp_matmul", "qdp_matvec", "qdp_axpby", "qdp_expr_plaquette", "qdp_expr_staple", "qdp_expr_ape_blend", "qdp_expr_trace_mul", "qdp_expr_sum_trace_mul", "qdp_expr_jit_kind", "qdp_expr_jit_compile", "qdp_expr_jit_assign", "qdp_expr_jit_sum", "qdp_expr_jit_compilations", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
     "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
     "qdp_field_timeslice_bytes", "qdp_field_get_timeslice", "qdp_field_set_timeslice",
@@ -83,6 +83,11 @@ DECLARED_SYMBOLS = {
     "qdp_expr_ape_blend": ([_P, _P, _I, _D, _I, _I], _I),
     "qdp_expr_trace_mul": ([_P, _P, _I, _I, _P, _I, _I, _I, _I, _I], _I),
     "qdp_expr_sum_trace_mul": ([_P, _I, _I, _P, _I, _I, _I, _I, _I, ctypes.POINTER(_D)], _I),
+    "qdp_expr_jit_kind": ([ctypes.c_char_p, ctypes.POINTER(_I), _I, _I, ctypes.POINTER(_I)], _I),
+    "qdp_expr_jit_compile": ([ctypes.c_char_p, ctypes.POINTER(_I), _I, _I, _I, _I, ctypes.POINTER(_Z)], _I),
+    "qdp_expr_jit_assign": ([_P, _I, ctypes.c_char_p, _PP, _I, ctypes.POINTER(_D), _I, _I], _I),
+    "qdp_expr_jit_sum": ([ctypes.c_char_p, _PP, _I, ctypes.POINTER(_D), _I, _I, ctypes.POINTER(_D)], _I),
+    "qdp_expr_jit_compilations": ([], ctypes.c_int64),
     "qdp_norm2": ([_P, _I, _P], _I),
     "qdp_inner": ([_P, _P, _I, _P], _I),
     "qdp_sum": ([_P, _I, _P], _I),
@@ -343,6 +348,44 @@ def qdp_expr_sum_trace_mul(a: Field, slot_a: int, adj_a: bool, b: Field, slot_b:
     _check(_lib.qdp_expr_sum_trace_mul(a.handle, slot_a, int(bool(adj_a)), b.handle, slot_b, int(bool(adj_b)), mu, sign,
                                        subset, out))
     return complex(out[0], out[1])
+
+
+def qdp_expr_jit_kind(expr: str, field_kinds, nscalars: int = 0) -> int:
+    """Host-only type check of a run-time expression: 0 matrix, 1 complex, 2 real (QdpError on a syntax / kind error)."""
+    kinds = (_I * max(1, len(field_kinds)))(*field_kinds)
+    out = _I()
+    _check(_lib.qdp_expr_jit_kind(expr.encode(), kinds, len(field_kinds), nscalars, ctypes.byref(out)))
+    return out.value
+
+
+def qdp_expr_jit_compile(expr: str, field_kinds, nscalars: int = 0, prec: int = QDP_F64, sum_: bool = False) -> int:
+    """Compile (NVRTC, no device needed) the kernel of the expression into the cache; returns the size of its image."""
+    kinds = (_I * max(1, len(field_kinds)))(*field_kinds)
+    out = _Z()
+    _check(_lib.qdp_expr_jit_compile(expr.encode(), kinds, len(field_kinds), nscalars, prec, int(bool(sum_)), ctypes.byref(out)))
+    return out.value
+
+
+def _jit_args(fields, scalars):
+    fp = (ctypes.c_void_p * len(fields))(*[f.handle for f in fields])
+    sc = (_D * max(1, len(scalars)))(*[float(x) for x in scalars])
+    return fp, sc
+
+
+def qdp_expr_jit_assign(dst: Field, slot_d: int, expr: str, fields, scalars=(), subset: int = QDP_ALL) -> None:
+    fp, sc = _jit_args(fields, scalars)
+    _check(_lib.qdp_expr_jit_assign(dst.handle, slot_d, expr.encode(), fp, len(fields), sc, len(scalars), subset))
+
+
+def qdp_expr_jit_sum(expr: str, fields, scalars=(), subset: int = QDP_ALL) -> complex:
+    fp, sc = _jit_args(fields, scalars)
+    out = (_D * 2)()
+    _check(_lib.qdp_expr_jit_sum(expr.encode(), fp, len(fields), sc, len(scalars), subset, out))
+    return complex(out[0], out[1])
+
+
+def qdp_expr_jit_compilations() -> int:
+    return int(_lib.qdp_expr_jit_compilations())
 
 
 def qdp_reunitarize(u_out: Field, u_in: Field, method: int = QDP_REUNIT_POLAR, subset: int = QDP_ALL) -> None:

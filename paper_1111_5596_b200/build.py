@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqdp_b200.so")
 PROBE_LIB = os.path.join(HERE, "libqdp_probe.so")   # bench-only peak probes (csrc/probe.cu), not part of the C ABI
-SOURCES = ["api.cu", "layout.cu", "shift.cu", "reduce.cu", "hop.cu", "plaquette.cu", "plaquette_tma.cu", "ape.cu", "reunit.cu", "matmul.cu", "expr.cu", "baryon.cu", "pool.cu"]
+SOURCES = ["api.cu", "layout.cu", "shift.cu", "reduce.cu", "hop.cu", "plaquette.cu", "plaquette_tma.cu", "ape.cu", "reunit.cu", "matmul.cu", "expr.cu", "baryon.cu", "pool.cu", "jit.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xptxas", "-v",
@@ -34,6 +34,28 @@ def _deps_mtime() -> float:
     return max(os.path.getmtime(h) for h in hdrs)
 
 
+JIT_HEADERS = ["geom.cuh", "reduce.cuh", "su3.cuh", "expr.cuh"]   # what a run-time expression kernel includes (csrc/jit.cu)
+
+
+def _write_jit_headers(obj_dir: str) -> None:
+    """jit_headers.inc: the headers above as string literals, so that NVRTC needs no file at run time."""
+    parts = []
+    for h in JIT_HEADERS:
+        text = open(os.path.join(CSRC, h)).read()
+        assert ')QDPHDR"' not in text
+        parts.append(f'static const char kJitHdr_{h.split(".")[0]}[] = R"QDPHDR(' + text + ')QDPHDR";\n')
+    names = ", ".join(f'"{h}"' for h in JIT_HEADERS)
+    srcs = ", ".join(f'kJitHdr_{h.split(".")[0]}' for h in JIT_HEADERS)
+    parts.append(f"static const char* const kJitHeaderNames[] = {{{names}}};\n")
+    parts.append(f"static const char* const kJitHeaderSources[] = {{{srcs}}};\n")
+    parts.append(f"static const int kJitHeaderCount = {len(JIT_HEADERS)};\n")
+    new = "".join(parts)
+    path = os.path.join(obj_dir, "jit_headers.inc")
+    if not os.path.exists(path) or open(path).read() != new:
+        with open(path, "w") as f:
+            f.write(new)
+
+
 BC_LIB = os.path.join(HERE, "libqdp_b200_bc.so")    # the same library compiled with -DQDP_BOUNDS_CHECK (su3.cuh: site_ptr_checked)
 
 
@@ -44,6 +66,8 @@ def build(force: bool = False, verbose: bool = False, bounds_check: bool = False
     lib = BC_LIB if bounds_check else LIB
     flags = NVCC_FLAGS + (["-DQDP_BOUNDS_CHECK"] if bounds_check else [])
     os.makedirs(obj_dir, exist_ok=True)
+    _write_jit_headers(obj_dir)
+    flags = flags + ["-I", obj_dir]
     nvcc = _nvcc()
     hdr_t = _deps_mtime()
     jobs = []
@@ -66,7 +90,7 @@ def build(force: bool = False, verbose: bool = False, bounds_check: bool = False
                 raise RuntimeError(f"nvcc failed on {s}")
     objs = [os.path.join(obj_dir, s.replace(".cu", ".o")) for s in SOURCES]
     if jobs or force or not os.path.exists(lib):
-        subprocess.check_call([nvcc, "-shared", "-o", lib, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+        subprocess.check_call([nvcc, "-shared", "-o", lib, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-ldl"])
     if bounds_check:
         return lib
     probe_src = os.path.join(CSRC, "probe.cu")

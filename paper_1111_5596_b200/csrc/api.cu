@@ -8,6 +8,7 @@
 
 #include "../../include/qdp_b200.h"
 #include "internal.h"
+#include "expr.cuh"
 #include "su3.cuh"
 
 using namespace qdp;
@@ -768,6 +769,93 @@ extern "C" int qdp_expr_trace_mul(qdp_field* dst, const qdp_field* a, int slot_a
 extern "C" int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a, const qdp_field* b, int slot_b, int adj_b,
                                       int mu, int sign, qdp_subset subset, double out[2]) {
     return expr_trace_mul_common("qdp_expr_sum_trace_mul", nullptr, a, slot_a, adj_a, b, slot_b, adj_b, mu, sign, subset, out);
+}
+
+// ---- run-time expressions (row f1, second step; jit.cu) -------------------------------------------------------
+static int jit_ncomp_of_kind(int kind) { return kind == QDP_COLOR_MATRIX ? 9 : (kind == QDP_GAUGE ? 36 : 0); }
+
+extern "C" int qdp_expr_jit_kind(const char* expr, const int* field_kinds, int nfields, int nscalars, int* kind_out) {
+    if (!expr || !kind_out || nfields < 0 || nfields > 4 || (nfields && !field_kinds)) return fail(QDP_ERR_ARG, "qdp_expr_jit_kind: bad argument");
+    int ncomp[4] = {0, 0, 0, 0};
+    for (int k = 0; k < nfields; k++)
+        if (!(ncomp[k] = jit_ncomp_of_kind(field_kinds[k]))) return fail(QDP_ERR_KIND, "qdp_expr_jit_kind: field arguments must be colour matrices or gauge fields");
+    JitExpr e;
+    std::string err;
+    if (jit_parse(expr, ncomp, nfields, nscalars, &e, &err) != 0) return fail(QDP_ERR_ARG, "qdp_expr_jit_kind: %s", err.c_str());
+    *kind_out = e.kind;
+    return QDP_OK;
+}
+
+extern "C" int qdp_expr_jit_compile(const char* expr, const int* field_kinds, int nfields, int nscalars, qdp_prec prec, int sum,
+                                    size_t* cubin_bytes) {
+    if (!expr || nfields < 0 || nfields > 4 || (nfields && !field_kinds) || (prec != QDP_F32 && prec != QDP_F64))
+        return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: bad argument");
+    int ncomp[4] = {0, 0, 0, 0};
+    for (int k = 0; k < nfields; k++)
+        if (!(ncomp[k] = jit_ncomp_of_kind(field_kinds[k]))) return fail(QDP_ERR_KIND, "qdp_expr_jit_compile: field arguments must be colour matrices or gauge fields");
+    JitExpr e;
+    std::string err;
+    if (jit_parse(expr, ncomp, nfields, nscalars, &e, &err) != 0) return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: %s", err.c_str());
+    if (sum && e.kind == JIT_MAT) return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: a sum needs a real or complex expression");
+    if (!sum && e.kind == JIT_REAL) return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: an assignment needs a matrix or complex expression");
+    if (jit_compile_only(e, prec == QDP_F64, sum != 0, cubin_bytes, &err) != 0) return fail(QDP_ERR_CUDA, "qdp_expr_jit_compile: %s", err.c_str());
+    return QDP_OK;
+}
+
+extern "C" int64_t qdp_expr_jit_compilations(void) { return jit_compilations(); }
+
+static int jit_common(const char* who, qdp_field* dst, int slot_d, const char* expr, const qdp_field* const* fields, int nfields,
+                      const double* scalars, int nscalars, qdp_subset subset, double* out) {
+    if (!expr || nfields < 1 || nfields > 4 || !fields || nscalars < 0 || nscalars > 4 || (nscalars && !scalars) || !ok_subset(subset) ||
+        (dst && !ok_field(dst)) || (!dst && !out))
+        return fail(QDP_ERR_ARG, "%s: bad argument", who);
+    int ncomp[4] = {0, 0, 0, 0};
+    ex::Args a = {};
+    for (int k = 0; k < nfields; k++) {
+        if (!ok_field(fields[k])) return fail(QDP_ERR_ARG, "%s: field argument %d is not a field", who, k);
+        const int rc = check_pair(who, fields[0], fields[k]);
+        if (rc != QDP_OK) return rc;
+        if (!(ncomp[k] = jit_ncomp_of_kind(fields[k]->kind))) return fail(QDP_ERR_KIND, "%s: field arguments must be colour matrices or gauge fields", who);
+        a.f[k] = fields[k]->data;
+        a.ncomp[k] = ncomp[k];
+    }
+    for (int k = 0; k < nscalars; k++) a.sc[k] = scalars[k];
+    a.mu = -1;
+    JitExpr e;
+    std::string err;
+    if (jit_parse(expr, ncomp, nfields, nscalars, &e, &err) != 0) return fail(QDP_ERR_ARG, "%s: %s", who, err.c_str());
+    qdp_lattice* l = fields[0]->lat;
+    int nd = 0, cd = 0;
+    if (dst) {
+        const int rc = check_pair(who, dst, fields[0]);
+        if (rc != QDP_OK) return rc;
+        if (e.kind == JIT_MAT) {
+            if (dst->kind != QDP_COLOR_MATRIX && dst->kind != QDP_GAUGE) return fail(QDP_ERR_KIND, "%s: a matrix expression needs a colour-matrix or gauge destination", who);
+            if (slot_d < 0 || slot_d >= dst->ncomp / 9) return fail(QDP_ERR_ARG, "%s: destination slot out of range", who);
+            cd = slot_d * 9;
+        } else if (e.kind == JIT_CPLX) {
+            if (dst->kind != QDP_COMPLEX) return fail(QDP_ERR_KIND, "%s: a complex expression needs a QDP_COMPLEX destination", who);
+        } else return fail(QDP_ERR_ARG, "%s: a real expression cannot be assigned (wrap it in a sum)", who);
+        nd = dst->ncomp;
+        if (e.has_shift)
+            for (int k = 0; k < nfields; k++)
+                if ((e.fields_used >> k & 1) && overlaps(dst, fields[k]))
+                    return fail(QDP_ERR_ALIAS, "%s: the destination is an operand of an expression that reads neighbour sites", who);
+    } else if (e.kind == JIT_MAT) return fail(QDP_ERR_ARG, "%s: a sum needs a real or complex expression", who);
+    ENTER(l);
+    cudaError_t ce = dst ? jit_launch_assign(e, fields[0]->prec == QDP_F64, l->geom, a, dst->data, nd, cd, subset, l->stream, &err)
+                         : jit_launch_sum(e, fields[0]->prec == QDP_F64, l->geom, a, subset, reduce_buf(l), l->stream, &err);
+    if (ce != cudaSuccess) return fail(QDP_ERR_CUDA, "%s: %s", who, err.empty() ? cudaGetErrorString(ce) : err.c_str());
+    return dst ? QDP_OK : fetch_result(l, 2, out);
+}
+extern "C" int qdp_expr_jit_assign(qdp_field* dst, int slot_d, const char* expr, const qdp_field* const* fields, int nfields,
+                                   const double* scalars, int nscalars, qdp_subset subset) {
+    if (!dst) return fail(QDP_ERR_ARG, "qdp_expr_jit_assign: bad argument");
+    return jit_common("qdp_expr_jit_assign", dst, slot_d, expr, fields, nfields, scalars, nscalars, subset, nullptr);
+}
+extern "C" int qdp_expr_jit_sum(const char* expr, const qdp_field* const* fields, int nfields, const double* scalars, int nscalars,
+                                qdp_subset subset, double out[2]) {
+    return jit_common("qdp_expr_jit_sum", nullptr, 0, expr, fields, nfields, scalars, nscalars, subset, out);
 }
 
 #ifdef QDP_BOUNDS_CHECK

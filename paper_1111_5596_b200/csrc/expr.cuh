@@ -15,9 +15,12 @@
 // evaluated without forming the product (9 complex / 18 real multiply-adds).  Assignment under a subset:
 // assign_kernel (matrix- or complex-valued expression -> field slot); fused global sums: sum2_kernel.
 #pragma once
+#ifndef __CUDACC_RTC__
 #include <type_traits>
 
 #include "internal.h"
+#endif
+#include "reduce.cuh"
 #include "su3.cuh"
 
 namespace qdp {
@@ -38,7 +41,9 @@ template <class T> struct Env {
 };
 
 struct Node {};
+#ifndef __CUDACC_RTC__
 template <class E> constexpr bool is_node = std::is_base_of<Node, E>::value;
+#endif
 
 // ---- values and their arithmetic ------------------------------------------------------------
 template <class T> __device__ __forceinline__ Mat3<T> v_adj(const Mat3<T>& a) {
@@ -160,7 +165,8 @@ template <class E> struct Imag : Node {
     template <class T> __device__ __forceinline__ static T eval(const Env<T>& e) { return v_imag(E::template eval<T>(e)); }
 };
 
-// ---- the surface syntax -----------------------------------------------------------------------
+// ---- the surface syntax (build-time expressions; jit.cu writes the node types out directly) -----
+#ifndef __CUDACC_RTC__
 template <class A, class B, class = std::enable_if_t<is_node<A> && is_node<B>>>
 constexpr Product<A, B> operator*(A, B) { return {}; }
 template <class A, class B, class = std::enable_if_t<is_node<A> && is_node<B>>>
@@ -171,6 +177,7 @@ template <class E> constexpr Real<E> real(E) { return {}; }
 template <class E> constexpr Imag<E> imag(E) { return {}; }
 template <int MU, int SIGN, class E> constexpr Shifted<E, MU, SIGN> shift(E) { return {}; }
 template <class E> constexpr ShiftedRt<E> shift_rt(E) { return {}; }
+#endif
 
 // ---- kernels ---------------------------------------------------------------------------------------
 template <class T> __device__ __forceinline__ void store_value(typename Vec2<T>::type* p, const Mat3<T>& v) { st_mat_at<T>(p, v); }
@@ -182,12 +189,16 @@ template <class T> __device__ __forceinline__ void store_value(typename Vec2<T>:
 
 // dst[first component cd of nd](x) = E(x) for x in the subset; other sites untouched
 template <class T, class E>
-__global__ void __launch_bounds__(128) assign_kernel(Geom g, Args a, typename Vec2<T>::type* dst, int nd, int cd, int subset) {
+__device__ __forceinline__ void assign_body(const Geom& g, const Args& a, typename Vec2<T>::type* dst, int nd, int cd, int subset) {
     const int i = blockIdx.x * 128 + threadIdx.x;
     int p, h;
     if (i >= work_items(g, subset) || !work_site(g, subset, i, p, h)) return;
     const Env<T> e{g, site_decode(g, p, h), a};
     store_value<T>(site_ptr(dst, nd, cd, e.x.index(g)), E::template eval<T>(e));
+}
+template <class T, class E>
+__global__ void __launch_bounds__(128) assign_kernel(Geom g, Args a, typename Vec2<T>::type* dst, int nd, int cd, int subset) {
+    assign_body<T, E>(g, a, dst, nd, cd, subset);
 }
 
 // result[k] = scale[k] * sum_{x in subset} Ek(x), k = 0, 1: two real-valued expressions, fp64 accumulation, fixed order.
@@ -210,6 +221,30 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 2 : 4) sum2_kernel(Geom 
     warp_grid_reduce<2>(acc, rb, sc);
 }
 
+// result[0, 1] = (re, im) of sum_{x in subset} E(x) for one real- or complex-valued expression, evaluated once per site
+template <class T> __device__ __forceinline__ double part_re(T v) { return (double)v; }
+template <class T> __device__ __forceinline__ double part_im(T) { return 0.0; }
+template <class T> __device__ __forceinline__ double part_re(const Cx<T>& v) { return (double)v.re; }
+template <class T> __device__ __forceinline__ double part_im(const Cx<T>& v) { return (double)v.im; }
+template <class T, class E>
+__device__ __forceinline__ void sumv_body(const Geom& g, const Args& a, int subset, const ReduceBuf& rb) {
+    const int lane = threadIdx.x & 31;
+    const int nwarps = gridDim.x * 4;
+    const int nitems = (work_items(g, subset) + 31) >> 5;
+    double acc[2] = {0.0, 0.0};
+    for (int wi = blockIdx.x * 4 + (threadIdx.x >> 5); wi < nitems; wi += nwarps) {
+        const int i = wi * 32 + lane;
+        int p, h;
+        if (!(i < work_items(g, subset) && work_site(g, subset, i, p, h))) continue;
+        const Env<T> e{g, site_decode(g, p, h), a};
+        const auto v = E::template eval<T>(e);
+        acc[0] += part_re(v);
+        acc[1] += part_im(v);
+    }
+    warp_grid_reduce<2>(acc, rb, nullptr);
+}
+
+#ifndef __CUDACC_RTC__
 template <class T, class E>
 cudaError_t launch_assign(const Geom& g, const Args& a, void* dst, int nd, int cd, int subset, cudaStream_t st) {
     const int items = subset == 0 ? 2 * ((g.Vh + 31) & ~31) : g.Vh;
@@ -227,6 +262,8 @@ cudaError_t launch_sum2(const Geom& g, const Args& a, int subset, const ReduceBu
     g_launch_count++;
     return cudaGetLastError();
 }
+
+#endif   // !__CUDACC_RTC__
 
 }  // namespace ex
 }  // namespace qdp

@@ -21,8 +21,17 @@
 // integer instructions on the decoded coordinates, which is cheaper than the
 // 32 B/site of table traffic it would replace on an HBM-bound path.
 #pragma once
+#ifdef __CUDACC_RTC__
+// Run-time compilation of an expression kernel (jit.cu): NVRTC has the CUDA built-ins but no host headers.
+typedef unsigned int uint32_t;
+typedef unsigned long long uint64_t;
+typedef int int32_t;
+typedef long long int64_t;
+typedef unsigned char uint8_t;
+#else
 #include <cstdint>
 #include <cuda_runtime.h>
+#endif
 
 namespace qdp {
 
@@ -30,6 +39,7 @@ namespace qdp {
 // m = ceil(2^(31+l) / d), l = ceil(log2 d)   (Granlund-Montgomery, N = 31 bits)
 struct FastDiv {
     uint32_t d, m, sh;
+#ifndef __CUDACC_RTC__
     __host__ static FastDiv make(uint32_t d) {
         FastDiv f;
         f.d = d;
@@ -39,6 +49,7 @@ struct FastDiv {
         f.m = (uint32_t)(((1ull << f.sh) + d - 1) / d);
         return f;
     }
+#endif
     __host__ __device__ __forceinline__ uint32_t div(uint32_t n) const {
         return (uint32_t)(((uint64_t)n * m) >> sh);
     }
@@ -56,6 +67,7 @@ struct Geom {
     int slab_ipr;     // 32-site blocks per (x2, x3) line of the (x0, x1) plane = Lh0 * L1 / 32
     int staged;       // 1: use the shared-memory-staged kernels (plaquette_tma.cu, ape_tma.cu) where the lattice allows
 
+#ifndef __CUDACC_RTC__
     __host__ static Geom make(const int* L) {
         Geom g;
         g.L0 = L[0]; g.L1 = L[1]; g.L2 = L[2]; g.L3 = L[3];
@@ -86,6 +98,7 @@ struct Geom {
         }
         return g;
     }
+#endif
 };
 
 // A decoded site.  odd0 = x0 & 1 = (p + x1 + x2 + x3) & 1;  x0 = 2*hx + odd0.

@@ -3,6 +3,8 @@
 #include <atomic>
 #include <cstddef>
 #include <cstdint>
+#include <cstring>
+#include <string>
 #include <cuda_runtime.h>
 
 #include "geom.cuh"
@@ -87,6 +89,26 @@ cudaError_t launch_expr_staple(int prec, const Geom& g, void* dst, const void* u
                                int subset, cudaStream_t st);
 cudaError_t launch_expr_trace_mul(int prec, const Geom& g, void* dst, const void* A, int na, int ia, bool adj_a, const void* B,
                                   int nb, int ib, bool adj_b, int mu, int sign, int subset, const ReduceBuf& rb, cudaStream_t st);
+
+// jit.cu: run-time expressions (text -> node type of expr.cuh -> NVRTC -> cached kernel)
+enum { JIT_MAT = 0, JIT_CPLX = 1, JIT_REAL = 2 };   // value kind of an expression: 3x3 matrix, complex, real
+struct JitExpr {
+    std::string type;       // the expression as a node type of expr.cuh
+    int kind;
+    bool has_shift;         // some operand is read at a neighbour site
+    unsigned fields_used;   // bit k: field argument k occurs
+};
+namespace ex { struct Args; }
+// ncomp[k]: components per site of field argument k (9 or 36).  Returns 0, or -1 with *err set.  No device needed.
+int jit_parse(const char* text, const int* ncomp, int nfields, int nscalars, JitExpr* out, std::string* err);
+std::string jit_source(const JitExpr& e, int prec, bool sum);
+int jit_compile_only(const JitExpr& e, int prec, bool sum, size_t* cubin_bytes, std::string* err);
+long long jit_compilations();
+// a failed compilation returns cudaErrorUnknown with *err set
+cudaError_t jit_launch_assign(const JitExpr& e, int prec, const Geom& g, const ex::Args& a, void* dst, int nd, int cd, int subset,
+                              cudaStream_t st, std::string* err);
+cudaError_t jit_launch_sum(const JitExpr& e, int prec, const Geom& g, const ex::Args& a, int subset, const ReduceBuf& rb,
+                           cudaStream_t st, std::string* err);
 
 // ape.cu
 cudaError_t launch_ape(int prec, const Geom& g, void* u_out, const void* u_in, double alpha, int t_dir,

@@ -7,7 +7,9 @@
 // K results.  No floating-point atomics: the value depends only on the launch
 // shape, so repeated runs are bit-identical.  All accumulation is fp64.
 #pragma once
+#ifndef __CUDACC_RTC__
 #include <cuda_runtime.h>
+#endif
 
 namespace qdp {
 

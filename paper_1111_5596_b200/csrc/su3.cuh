@@ -7,8 +7,10 @@
 // (re, im) adjacent: fp64 -> one double2 = one 128-bit access per thread, a warp moves 512
 // contiguous bytes per component; fp32 -> float2, 256 contiguous bytes per warp.
 #pragma once
+#ifndef __CUDACC_RTC__
 #include <cstdio>
 #include <cuda_runtime.h>
+#endif
 #include "geom.cuh"
 
 namespace qdp {

@@ -1,0 +1,136 @@
+"""Pins of the oracle's run-time expression evaluator (oracle/expr_eval.py, second step), and the
+host half of the library's front end (parser, kind check, NVRTC compilation) which needs no GPU."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from oracle import expr_eval as ee
+
+DIMS = [(4, 4, 4, 4), (4, 2, 6, 4)]
+PLAQ = "real(trace(f0[{m}] * shift(f0[{n}], +{m}) * adj(shift(f0[{m}], +{n})) * adj(f0[{n}])))"
+UPPER = "f0[{n}] * shift(f0[{m}], +{n}) * adj(shift(f0[{n}], +{m}))"
+LOWER = "shift(adj(f0[{n}]) * f0[{m}] * shift(f0[{n}], +{m}), -{n})"
+
+
+def test_parser_precedence_and_associativity():
+    assert ee.parse("f0 + f1 * f2") == ("+", ("f", 0, 0), ("*", ("f", 1, 0), ("f", 2, 0)))
+    assert ee.parse("f0 * f1 * f2") == ("*", ("*", ("f", 0, 0), ("f", 1, 0)), ("f", 2, 0))
+    assert ee.parse("(f0 + f1) * s2") == ("*", ("+", ("f", 0, 0), ("f", 1, 0)), ("s", 2))
+    assert ee.parse("shift(adj(f0[3]), -2)") == ("shift", ("adj", ("f", 0, 3)), 2, -1)
+    for bad in ("f0 +", "f0 * * f1", "shift(f0, 2)", "trace f0", "f0[", "g0", "f0 f1", "(f0"):
+        with pytest.raises(ee.ExprError):
+            ee.parse(bad)
+
+
+def test_kinds():
+    slots = [4, 1]
+    assert ee.kind_of(ee.parse("f0[1] * f1"), slots) == ee.MAT
+    assert ee.kind_of(ee.parse("trace(f0[1] * f1)"), slots) == ee.CPLX
+    assert ee.kind_of(ee.parse("real(trace(f1)) * s0"), slots) == ee.REAL
+    assert ee.kind_of(ee.parse("s0 * f1 * s1"), slots) == ee.MAT
+    assert ee.kind_of(ee.parse("trace(f1) * trace(f1)"), slots) == ee.CPLX
+    for bad in ("f0 + trace(f1)", "trace(trace(f1))", "real(f1)", "f1 * trace(f1)", "f1[1]", "f0[4]", "f2", "shift(f1, +4)"):
+        with pytest.raises(ee.ExprError):
+            ee.kind_of(ee.parse(bad), slots)
+
+
+@pytest.mark.parametrize("dims", DIMS)
+def test_plaquette_expression_is_def2(dims):
+    """sum of real(trace(four links)) over the planes, normalised, is the plaquette of the C oracle (itself pinned on the
+    unit field, abelian closed forms and numpy brute force: tests/test_oracle_plaquette.py)."""
+    hu = synth.gauge_hot(dims, 41)
+    V = synth.volume(dims)
+    sp = sum(ee.total(dims, PLAQ.format(m=m, n=n), [hu]).real for m, n in ((0, 1), (0, 2), (1, 2)))
+    tp = sum(ee.total(dims, PLAQ.format(m=m, n=3), [hu]).real for m in range(3))
+    want = oracle.plaquette(dims, hu)
+    assert abs(sp / (9 * V) - want[1]) < 1e-13 and abs(tp / (9 * V) - want[2]) < 1e-13
+    # per site against the C oracle's own per-site plaquette
+    v, kind = ee.evaluate(dims, PLAQ.format(m=0, n=1), [hu])
+    assert kind == ee.REAL
+    for lex in (0, 7, V - 1):
+        assert abs(v[lex] - oracle.plaquette_site(dims, hu, lex)[0]) < 1e-13
+
+
+@pytest.mark.parametrize("dims", DIMS)
+def test_staple_and_blend_expressions_are_def3(dims):
+    hu = synth.gauge_hot(dims, 42)
+    for mu in range(3):
+        nus = [n for n in range(3) if n != mu]
+        text = " + ".join(UPPER.format(m=mu, n=n) + " + " + LOWER.format(m=mu, n=n) for n in nus)
+        got, kind = ee.evaluate(dims, text, [hu])
+        assert kind == ee.MAT
+        assert np.abs(got - oracle.staple_field(dims, hu, mu, 3)).max() < 1e-13
+        blend, _ = ee.evaluate(dims, f"s0 * f0[{mu}] + s1 * ({text})", [hu], [0.4, 0.6 / 4])
+        assert np.abs(blend - oracle.ape_blend_field(dims, hu, mu, 0.6, 3)).max() < 1e-13
+
+
+@pytest.mark.parametrize("dims", DIMS)
+def test_trace_forms_match_trace_mul(dims):
+    hu, hm = synth.gauge_hot(dims, 43), synth.color_matrix(dims, 44)
+    got, _ = ee.evaluate(dims, "trace(adj(f0[2]) * shift(f1, -1))", [hu, hm])
+    assert np.abs(got - oracle.trace_mul(dims, hu, 2, 1, hm, 0, 0, 1, -1)).max() < 1e-13
+    got, _ = ee.evaluate(dims, "trace(f1 * adj(shift(f0[3], +0)))", [hu, hm])
+    assert np.abs(got - oracle.trace_mul(dims, hm, 0, 0, hu, 3, 1, 0, +1)).max() < 1e-13
+
+
+def test_algebraic_identities():
+    dims = (4, 2, 6, 4)
+    hu, hm = synth.gauge_hot(dims, 45), synth.color_matrix(dims, 46)
+    ev = lambda t, s=(): ee.evaluate(dims, t, [hu, hm], s)[0]
+    assert np.abs(ev("trace(f0[1] * f1)") - ev("trace(f1 * f0[1])")).max() < 1e-13                       # cyclicity
+    assert np.abs(ev("adj(f0[1] * f1)") - ev("adj(f1) * adj(f0[1])")).max() < 1e-13                      # (AB)^dag
+    assert np.array_equal(ev("shift(shift(f1, +2), -2)"), ev("f1"))                                      # shifts invert
+    assert np.array_equal(ev("shift(f0[0] * f1, +3)"), ev("shift(f0[0], +3) * shift(f1, +3)"))           # site-local ops commute with shift
+    assert np.array_equal(ev("shift(shift(f1, +0), +1)"), ev("shift(shift(f1, +1), +0)"))
+    assert np.abs(ev("f0[2] * adj(f0[2])") - np.eye(3)).max() < 1e-13                                     # SU(3) links
+    fro = (np.abs(hm) ** 2).sum(axis=(1, 2))
+    assert np.abs(ev("real(trace(adj(f1) * f1))") - fro).max() < 1e-12 * fro.max()
+    assert np.abs(ev("imag(trace(adj(f1) * f1))")).max() < 1e-13 * fro.max()
+    assert np.abs(ev("s0 * f1 + s1 * f1", (0.25, 0.5)) - 0.75 * hm).max() < 1e-15 * np.abs(hm).max() * 4
+    # brute force at one site: (a b)_ij and the trace, from the definitions
+    x = 5
+    a, b = hu[x, 1], hm[x]
+    want = sum(a[i, k] * b[k, i] for i in range(3) for k in range(3))
+    assert abs(ev("trace(f0[1] * f1)")[x] - want) < 1e-13
+
+
+# ---- the library's host-side front end (no GPU): it must accept and reject what the oracle's language does ------
+VALID = [("f0[1] * f1", ee.MAT), ("trace(f0[1] * f1)", ee.CPLX), ("real(trace(f1)) * s0", ee.REAL), ("s0 * f1 * s1", ee.MAT),
+         ("trace(f1) * trace(adj(f1)) + trace(f0[3])", ee.CPLX), (LOWER.format(m=0, n=2), ee.MAT), ("( f1+adj( f1 ) )*s1", ee.MAT),
+         ("imag(trace(f1)) * real(trace(f0[0]))", ee.REAL), ("trace(f1) * s0", ee.CPLX)]
+INVALID = ["f0 + trace(f1)", "trace(trace(f1))", "real(f1)", "f1 * trace(f1)", "f1[1]", "f0[4]", "f2", "shift(f1, +4)", "f0 +",
+           "shift(f0, 2)", "f0 f1", "(f0", "s2 * f1", "", "f0[0] * ", "adj f1"]
+
+
+def test_library_front_end_agrees_with_the_oracle_language():
+    q = pytest.importorskip("paper_1111_5596_b200")
+    kinds = [q.QDP_GAUGE, q.QDP_COLOR_MATRIX]
+    for text, kind in VALID:
+        assert ee.kind_of(ee.parse(text), [4, 1]) == kind
+        assert q.qdp_expr_jit_kind(text, kinds, 2) == kind, text
+    for text in INVALID:
+        with pytest.raises(q.QdpError):
+            q.qdp_expr_jit_kind(text, kinds, 2)
+        with pytest.raises(ee.ExprError):
+            tree = ee.parse(text)
+            ee.kind_of(tree, [4, 1])
+            if "s2" in text:
+                raise ee.ExprError("scalar argument out of range")   # the oracle takes its scalars from a Python sequence
+
+
+def test_nvrtc_compiles_an_expression_once_without_a_gpu():
+    q = pytest.importorskip("paper_1111_5596_b200")
+    kinds = [q.QDP_GAUGE]
+    text = "trace(f0[0] * adj(shift(f0[1], -2))) * s0"
+    before = q.qdp_expr_jit_compilations()
+    size = q.qdp_expr_jit_compile(text, kinds, 1, q.QDP_F64, sum_=True)
+    assert size > 1000 and q.qdp_expr_jit_compilations() == before + 1
+    assert q.qdp_expr_jit_compile(text, kinds, 1, q.QDP_F64, sum_=True) == size      # cached
+    assert q.qdp_expr_jit_compilations() == before + 1
+    q.qdp_expr_jit_compile("trace( f0[0]*adj(shift(f0[1],-2)) )*s0", kinds, 1, q.QDP_F64, sum_=True)   # same tree, other spelling
+    assert q.qdp_expr_jit_compilations() == before + 1
+    q.qdp_expr_jit_compile(text, kinds, 1, q.QDP_F32, sum_=True)                     # another precision: another kernel
+    assert q.qdp_expr_jit_compilations() == before + 2
+    with pytest.raises(q.QdpError):
+        q.qdp_expr_jit_compile("f0[0]", kinds, 0, q.QDP_F64, sum_=True)              # a matrix cannot be summed
