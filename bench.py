@@ -282,6 +282,11 @@ def run_ours(args) -> dict | None:
     # ---- rows widened beyond the step: timed separately, not part of `value` -------
     # name -> (call, complex numbers moved per site (algorithmic), note)
     cm = q.qdp_field_alloc(lat, q.QDP_COLOR_MATRIX, P)
+    plane = "real(trace(f0[{a}] * shift(f0[{b}], +{a}) * adj(shift(f0[{a}], +{b})) * adj(f0[{b}])))"
+    JIT_PLAQ_S = " + ".join(plane.format(a=a, b=b) for a, b in ((0, 1), (0, 2), (1, 2)))
+    JIT_PLAQ_T = " + ".join(plane.format(a=a, b=3) for a in range(3))
+    JIT_STAPLE = " + ".join(f"(f0[{n}] * shift(f0[0], +{n}) * adj(shift(f0[{n}], +0)) + shift(adj(f0[{n}]) * f0[0] * shift(f0[{n}], +0), -{n}))"
+                            for n in (1, 2))
     extra_defs = {
         "smear_hop": (lambda: q.qdp_smear_hop(chi, a, b, u, psi, 3), 51,
                       "qdp_smear_hop, t_dir = 3 (row f2): u 27 + psi 12 + chi 12 complex per site"),
@@ -300,6 +305,13 @@ def run_ours(args) -> dict | None:
         "expr_plaquette": (lambda: q.qdp_expr_plaquette(u), 36,
                            "qdp_expr_plaquette (row f1): the plaquette written as one expression of the compile-time "
                            "layer, one kernel; compare ops.plaquette (hand-fused)"),
+        "jit_plaquette": (lambda: (q.qdp_expr_jit_sum(JIT_PLAQ_S, [u]), q.qdp_expr_jit_sum(JIT_PLAQ_T, [u])), 72,
+                          "qdp_expr_jit_sum (row f1, run-time expressions): the spatial and the temporal planes of the plaquette "
+                          "as two text expressions compiled with NVRTC on first use (cached afterwards): two kernels, the "
+                          "gauge field is read twice; compare expr_plaquette (nvcc, one kernel) and ops.plaquette"),
+        "jit_staple": (lambda: q.qdp_expr_jit_assign(cm, 0, JIT_STAPLE, [u]), 36,
+                       "qdp_expr_jit_assign (row f1): the spatial staple sum of link 0 as a text expression; the same kernel as "
+                       "expr_staple, through NVRTC"),
         "expr_staple": (lambda: q.qdp_expr_staple(cm, u, 0, 3), 36,
                         "qdp_expr_staple mu = 0, spatial (row f1): the staple sum as one expression; 27 complex read "
                         "(three links) + 9 written per site"),
@@ -313,6 +325,11 @@ def run_ours(args) -> dict | None:
     }
     extra_ms = {}
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_jit = time.perf_counter()      # first use compiles: measured once, outside every timed region
+    n_jit = q.qdp_expr_jit_compilations()
+    extra_defs["jit_plaquette"][0]()
+    extra_defs["jit_staple"][0]()
+    jit_compile = {"expressions": q.qdp_expr_jit_compilations() - n_jit, "seconds": round(time.perf_counter() - t_jit, 3)}
 
     def time_extra(fn):
         for _ in range(3):
@@ -481,6 +498,8 @@ def run_ours(args) -> dict | None:
                                  "frac": round(V * nc * eb / extra_ms[name] / 1e6 / peak, 4),
                                  "note": note + "; not part of the step"}
                           for name, (_, nc, note) in extra_defs.items()},
+            "jit": dict(jit_compile, note="NVRTC compilations on first use of the run-time expressions of extra_ops (jit_*), wall clock "
+                                          "including their first launches; later uses hit the cache"),
             "scalars": {"plaquette": [float(x) for x in results["plaquette"]], "norm2": float(results["norm2"])},
         }
         if world == 1 and not args.no_cpu_baseline:
