@@ -285,6 +285,7 @@ def run_ours(args) -> dict | None:
     plane = "real(trace(f0[{a}] * shift(f0[{b}], +{a}) * adj(shift(f0[{a}], +{b})) * adj(f0[{b}])))"
     JIT_PLAQ_S = " + ".join(plane.format(a=a, b=b) for a, b in ((0, 1), (0, 2), (1, 2)))
     JIT_PLAQ_T = " + ".join(plane.format(a=a, b=3) for a in range(3))
+    JIT_HOP = " + ".join(f"f0[{m}] * shift(f1, +{m}) + shift(adj(f0[{m}]) * f1, -{m})" for m in range(4))
     JIT_STAPLE = " + ".join(f"(f0[{n}] * shift(f0[0], +{n}) * adj(shift(f0[{n}], +0)) + shift(adj(f0[{n}]) * f0[0] * shift(f0[{n}], +0), -{n}))"
                             for n in (1, 2))
     extra_defs = {
@@ -309,6 +310,11 @@ def run_ours(args) -> dict | None:
                           "qdp_expr_jit_sum (row f1, run-time expressions): the spatial and the temporal planes of the plaquette "
                           "as two text expressions compiled with NVRTC on first use (cached afterwards): two kernels, the "
                           "gauge field is read twice; compare expr_plaquette (nvcc, one kernel) and ops.plaquette"),
+        "jit_hop": (lambda: q.qdp_expr_jit_assign(chi, 0, JIT_HOP, [u, psi]), 48,
+                    "qdp_expr_jit_assign (row f1): the hopping term of def. 5 on the full lattice as a text expression with "
+                    "fermion leaves (u 36 + chi 12 complex per site); compare the hand-fused qdp_hop ALL (hop_all)"),
+        "hop_all": (lambda: q.qdp_hop(chi, u, psi, q.QDP_ALL), 48,
+                    "qdp_hop on the full lattice, hand-fused (the step times the halves and the fused axpy form)"),
         "jit_staple": (lambda: q.qdp_expr_jit_assign(cm, 0, JIT_STAPLE, [u]), 36,
                        "qdp_expr_jit_assign (row f1): the spatial staple sum of link 0 as a text expression; the same kernel as "
                        "expr_staple, through NVRTC"),
@@ -329,6 +335,7 @@ def run_ours(args) -> dict | None:
     n_jit = q.qdp_expr_jit_compilations()
     extra_defs["jit_plaquette"][0]()
     extra_defs["jit_staple"][0]()
+    extra_defs["jit_hop"][0]()
     jit_compile = {"expressions": q.qdp_expr_jit_compilations() - n_jit, "seconds": round(time.perf_counter() - t_jit, 3)}
 
     def time_extra(fn):

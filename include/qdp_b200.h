@@ -344,20 +344,25 @@ int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a, const qdp_
  * costs one compilation (0.2-0.4 s); later uses launch the cached kernel.  libnvrtc is loaded at the first compilation
  * (QDP_ERR_CUDA with a message if it is missing); nothing is read from the file system.
  *   expr   := term { '+' term }            term := factor { '*' factor }
- *   factor := adj(expr) | trace(expr) | real(expr) | imag(expr) | shift(expr, +mu | -mu) | '(' expr ')' | leaf
- *   leaf   := f<k> [ '[' slot ']' ]        matrix `slot` (a link of a gauge field; default 0) of field argument k = 0..3
+ *   factor := adj(expr) | trace(expr) | real(expr) | imag(expr) | norm2(expr) | inner(expr, expr)
+ *           | shift(expr, +mu | -mu) | '(' expr ')' | leaf
+ *   leaf   := f<k> [ '[' slot ']' ]        field argument k = 0..3: matrix `slot` of a QDP_COLOR_MATRIX or QDP_GAUGE field
+ *                                          (a link of a gauge field; default 0), or the spinor of a QDP_FERMION field
  *           | s<k>                         real scalar argument k = 0..3 (cast to the field precision)
- * Semantics as in the build-time layer and SURVEY.md 8(c): a value is a 3x3 matrix, a complex number or a real number;
- * adj = conjugate transpose (conjugate of a complex number), trace: matrix -> complex, real / imag: complex -> real,
- * shift(e, +mu)(x) = e(x + mu) for the whole sub-expression e (A3), '+' needs equal kinds, '*' is matrix * matrix,
- * real * anything, anything * real or complex * complex.  Field arguments: QDP_COLOR_MATRIX or QDP_GAUGE of one
- * lattice and precision.
- *   qdp_expr_jit_kind:    host only; *kind_out = 0 matrix, 1 complex, 2 real.  field_kinds[k] = qdp_kind of argument k.
+ * Semantics as in the build-time layer and SURVEY.md 8(c): a value is a 3x3 matrix, a spinor (4 spin x 3 colour), a
+ * complex number or a real number; adj = conjugate transpose (conjugate of a complex number; not defined on spinors),
+ * trace: matrix -> complex, real / imag: complex -> real, norm2: spinor -> real (sum over spin and colour of |.|^2),
+ * inner(a, b): two spinors -> complex (sum of conj(a) b), shift(e, +mu)(x) = e(x + mu) for the whole sub-expression e
+ * (A3), '+' needs equal kinds, '*' is matrix * matrix, matrix * spinor (the matrix acts on the colour index of every spin
+ * component: the product of the hopping term, A11), real * anything, anything * real, complex * complex or complex *
+ * spinor.  All field arguments belong to one lattice and precision.  Example, the hopping term of def. 5:
+ *   "f0[0] * shift(f1, +0) + shift(adj(f0[0]) * f1, -0) + f0[1] * shift(f1, +1) + ..."  with f0 = u, f1 = psi.
+ *   qdp_expr_jit_kind:    host only; *kind_out = 0 matrix, 1 complex, 2 real, 3 spinor.  field_kinds[k] = qdp_kind of argument k.
  *   qdp_expr_jit_compile: host only (NVRTC needs no device): compiles the kernel for (expr, prec, sum != 0) into the
  *                         cache if it is not there; *cubin_bytes (optional) receives the size of its image.
  *   qdp_expr_jit_assign:  dst[slot_d](x) = expr(x) for x in subset, other sites untouched.  A matrix expression needs a
- *                         QDP_COLOR_MATRIX (slot_d = 0) or QDP_GAUGE destination, a complex one a QDP_COMPLEX destination
- *                         (QDP_ERR_KIND).  dst may be an operand unless the expression contains a shift (QDP_ERR_ALIAS).
+ *                         QDP_COLOR_MATRIX (slot_d = 0) or QDP_GAUGE destination, a spinor expression a QDP_FERMION and a
+ *                         complex one a QDP_COMPLEX destination (QDP_ERR_KIND).  dst may be an operand unless the expression contains a shift (QDP_ERR_ALIAS).
  *                         Asynchronous.
  *   qdp_expr_jit_sum:     out = (re, im) of sum_{x in subset} expr(x) for a real or complex expression (fp64
  *                         accumulation, fixed order, not normalised).  Synchronous.

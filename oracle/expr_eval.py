@@ -7,13 +7,17 @@ in the order the expression is written.  Shares nothing with ``csrc/jit.cu``: ow
 Grammar (the same language the library documents in ``include/qdp_b200.h``):
 
     expr   := term { '+' term }          term := factor { '*' factor }
-    factor := adj(expr) | trace(expr) | real(expr) | imag(expr) | shift(expr, +mu | -mu) | '(' expr ')' | leaf
+    factor := adj(expr) | trace(expr) | real(expr) | imag(expr) | norm2(expr) | inner(expr, expr)
+            | shift(expr, +mu | -mu) | '(' expr ')' | leaf
     leaf   := f<k> [ '[' slot ']' ]  |  s<k>
 
-Values: matrix field [V,3,3] complex128, complex field [V] complex128, real field [V] float64 (a scalar argument is a
-constant real field).  adj = conjugate transpose / complex conjugate / identity on reals; trace over the colour indices;
-shift(e, +mu)(x) = e(x + mu) with periodic wrap (reading A3), done by ``oracle.shift`` on the evaluated array; '*' is
-the per-site matrix product, or scaling by a real, or the product of complex numbers; '+' adds values of equal kind.
+Values: matrix field [V,3,3] complex128, spinor field [V,4,3] complex128 (a fermion argument), complex field [V]
+complex128, real field [V] float64 (a scalar argument is a constant real field).  adj = conjugate transpose / complex
+conjugate / identity on reals (not defined on spinors); trace over the colour indices; norm2(psi) = sum over spin and
+colour of |psi|^2, inner(a, b) = sum over spin and colour of conj(a) b; shift(e, +mu)(x) = e(x + mu) with periodic wrap
+(reading A3), done by ``oracle.shift`` on the evaluated array; '*' is the per-site matrix product, a matrix acting on the
+colour index of every spin component of a spinor, scaling by a real or a complex number, or the product of complex
+numbers; '+' adds values of equal kind.
 """
 from __future__ import annotations
 
@@ -23,8 +27,8 @@ import numpy as np
 
 from . import shift as _shift, volume as _volume
 
-MAT, CPLX, REAL = 0, 1, 2
-_TOKEN = re.compile(r"\s*(adj|trace|real|imag|shift|f\d|s\d|[()\[\],+\-*]|\d)")
+MAT, CPLX, REAL, SPINOR = 0, 1, 2, 3
+_TOKEN = re.compile(r"\s*(adj|trace|real|imag|norm2|inner|shift|f\d|s\d|[()\[\],+\-*]|\d)")
 
 
 class ExprError(ValueError):
@@ -44,8 +48,9 @@ def tokenize(text: str) -> list[str]:
 
 
 def parse(text: str):
-    """Returns a nested tuple tree: ('f', k, slot) | ('s', k) | ('adj'|'trace'|'real'|'imag', e) | ('shift', e, mu, sign)
-    | ('+', a, b) | ('*', a, b); '+' and '*' associate to the left, '*' binds tighter."""
+    """Returns a nested tuple tree: ('f', k, slot | None) | ('s', k) | ('adj'|'trace'|'real'|'imag'|'norm2', e) |
+    ('inner', a, b) | ('shift', e, mu, sign) | ('+', a, b) | ('*', a, b); '+' and '*' associate to the left, '*' binds
+    tighter."""
     toks = tokenize(text)
     pos = 0
 
@@ -76,11 +81,18 @@ def parse(text: str):
 
     def factor():
         t = take()
-        if t in ("adj", "trace", "real", "imag"):
+        if t in ("adj", "trace", "real", "imag", "norm2"):
             take("(")
             e = expr()
             take(")")
             return (t, e)
+        if t == "inner":
+            take("(")
+            a = expr()
+            take(",")
+            b = expr()
+            take(")")
+            return ("inner", a, b)
         if t == "shift":
             take("(")
             e = expr()
@@ -96,7 +108,7 @@ def parse(text: str):
             take(")")
             return e
         if t[0] == "f" and len(t) == 2:
-            slot = 0
+            slot = None                      # None: no subscript written
             if peek() == "[":
                 take()
                 slot = int(take())
@@ -113,19 +125,28 @@ def parse(text: str):
 
 
 def kind_of(tree, field_slots) -> int:
-    """Value kind of the expression; field_slots[k] = number of matrices per site of field argument k (1 or 4).
-    Raises ExprError for the combinations the language does not define."""
+    """Value kind of the expression; field_slots[k] = number of matrices per site of field argument k (1 colour matrix,
+    4 gauge field) or 0 for a fermion field.  Raises ExprError for the combinations the language does not define."""
     op = tree[0]
     if op == "f":
-        if tree[1] >= len(field_slots) or tree[2] >= field_slots[tree[1]]:
-            raise ExprError("field argument or slot out of range")
+        if tree[1] >= len(field_slots):
+            raise ExprError("field argument out of range")
+        if field_slots[tree[1]] == 0:
+            if tree[2] is not None:
+                raise ExprError("a fermion field has no slots")
+            return SPINOR
+        if (tree[2] or 0) >= field_slots[tree[1]]:
+            raise ExprError("slot out of range")
         return MAT
     if op == "s":
         return REAL
     if op in ("adj", "shift"):
         if op == "shift" and not 0 <= tree[2] <= 3:
             raise ExprError("direction must be 0..3")
-        return kind_of(tree[1], field_slots)
+        k = kind_of(tree[1], field_slots)
+        if op == "adj" and k == SPINOR:
+            raise ExprError("adj() of a spinor is not defined")
+        return k
     if op == "trace":
         if kind_of(tree[1], field_slots) != MAT:
             raise ExprError("trace() takes a matrix")
@@ -134,7 +155,15 @@ def kind_of(tree, field_slots) -> int:
         if kind_of(tree[1], field_slots) != CPLX:
             raise ExprError(f"{op}() takes a complex number")
         return REAL
+    if op == "norm2":
+        if kind_of(tree[1], field_slots) != SPINOR:
+            raise ExprError("norm2() takes a spinor")
+        return REAL
     a, b = kind_of(tree[1], field_slots), kind_of(tree[2], field_slots)
+    if op == "inner":
+        if a != SPINOR or b != SPINOR:
+            raise ExprError("inner() takes two spinors")
+        return CPLX
     if op == "+":
         if a != b:
             raise ExprError("'+' needs operands of the same kind")
@@ -143,28 +172,38 @@ def kind_of(tree, field_slots) -> int:
         return b
     if b == REAL:
         return a
-    if a == b:
+    if (a, b) in ((MAT, MAT), (CPLX, CPLX)):
         return a
-    raise ExprError("'*' of a matrix and a complex number is not defined")
+    if (a, b) in ((MAT, SPINOR), (CPLX, SPINOR), (SPINOR, CPLX)):
+        return SPINOR
+    raise ExprError("'*' is not defined for these operand kinds")
 
 
 def evaluate(dims, text: str, fields, scalars=()):
-    """The expression at every site.  fields[k]: [V,3,3] (colour matrix) or [V,4,3,3] (gauge) complex arrays.
-    Returns ([V,3,3] | [V] complex128 | [V] float64, kind)."""
+    """The expression at every site.  fields[k]: [V,3,3] (colour matrix), [V,4,3,3] (gauge) or [V,4,3] (fermion) complex
+    arrays.  Returns ([V,3,3] | [V,4,3] | [V] complex128 | [V] float64, kind)."""
     V = _volume(dims)
-    fields = [np.asarray(f, dtype=np.complex128).reshape(V, -1, 3, 3) for f in fields]
+    fields = [np.asarray(f, dtype=np.complex128) for f in fields]
+    is_spinor = [f.ndim == 3 and f.shape[1:] == (4, 3) for f in fields]
+    mats = [None if sp else f.reshape(V, -1, 3, 3) for f, sp in zip(fields, is_spinor)]
     tree = parse(text)
-    kind = kind_of(tree, [f.shape[1] for f in fields])
+    kind = kind_of(tree, [0 if sp else m.shape[1] for m, sp in zip(mats, is_spinor)])
+
+    def is_mat(v):
+        return v.ndim == 3 and v.shape[1:] == (3, 3)
+
+    def is_spin(v):
+        return v.ndim == 3 and v.shape[1:] == (4, 3)
 
     def ev(t):
         op = t[0]
         if op == "f":
-            return fields[t[1]][:, t[2]].copy()
+            return fields[t[1]].copy() if is_spinor[t[1]] else mats[t[1]][:, t[2] or 0].copy()
         if op == "s":
             return np.full(V, float(scalars[t[1]]))
         if op == "adj":
             v = ev(t[1])
-            return np.conj(np.swapaxes(v, 1, 2)) if v.ndim == 3 else np.conj(v)
+            return np.conj(np.swapaxes(v, 1, 2)) if is_mat(v) else np.conj(v)
         if op == "trace":
             v = ev(t[1])
             return v[:, 0, 0] + v[:, 1, 1] + v[:, 2, 2]
@@ -172,17 +211,30 @@ def evaluate(dims, text: str, fields, scalars=()):
             return np.ascontiguousarray(ev(t[1]).real)
         if op == "imag":
             return np.ascontiguousarray(ev(t[1]).imag)
+        if op == "norm2":
+            v = ev(t[1])
+            return (v.real ** 2 + v.imag ** 2).reshape(V, 12).sum(axis=1)
+        if op == "inner":
+            a, b = ev(t[1]), ev(t[2])
+            return (np.conj(a) * b).reshape(V, 12).sum(axis=1)
         if op == "shift":
             return _shift(dims, np.ascontiguousarray(ev(t[1])), t[2], t[3])
         a, b = ev(t[1]), ev(t[2])
         if op == "+":
             return a + b
-        if a.ndim == 3 and b.ndim == 3:
+        if is_mat(a) and is_mat(b):
             out = np.zeros_like(a)
             for i in range(3):            # (a b)_ij = sum_k a_ik b_kj, written out
                 for j in range(3):
                     for k in range(3):
                         out[:, i, j] += a[:, i, k] * b[:, k, j]
+            return out
+        if is_mat(a) and is_spin(b):
+            out = np.zeros_like(b)
+            for sp in range(4):           # (a psi)_{s,i} = sum_k a_ik psi_{s,k}: spin untouched (reading A11)
+                for i in range(3):
+                    for k in range(3):
+                        out[:, sp, i] += a[:, i, k] * b[:, sp, k]
             return out
         if a.ndim == 3:
             return a * b[:, None, None]
@@ -198,7 +250,7 @@ def total(dims, text: str, fields, scalars=(), mask=None) -> complex:
     (math.fsum) so that the comparison bar is the GPU's, not this sum's."""
     import math
     v, kind = evaluate(dims, text, fields, scalars)
-    if kind == MAT:
+    if kind in (MAT, SPINOR):
         raise ExprError("a sum needs a real or complex expression")
     if mask is not None:
         v = v[mask]

@@ -772,13 +772,13 @@ extern "C" int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a,
 }
 
 // ---- run-time expressions (row f1, second step; jit.cu) -------------------------------------------------------
-static int jit_ncomp_of_kind(int kind) { return kind == QDP_COLOR_MATRIX ? 9 : (kind == QDP_GAUGE ? 36 : 0); }
+static int jit_ncomp_of_kind(int kind) { return kind == QDP_COLOR_MATRIX ? 9 : (kind == QDP_GAUGE ? 36 : (kind == QDP_FERMION ? 12 : 0)); }
 
 extern "C" int qdp_expr_jit_kind(const char* expr, const int* field_kinds, int nfields, int nscalars, int* kind_out) {
     if (!expr || !kind_out || nfields < 0 || nfields > 4 || (nfields && !field_kinds)) return fail(QDP_ERR_ARG, "qdp_expr_jit_kind: bad argument");
     int ncomp[4] = {0, 0, 0, 0};
     for (int k = 0; k < nfields; k++)
-        if (!(ncomp[k] = jit_ncomp_of_kind(field_kinds[k]))) return fail(QDP_ERR_KIND, "qdp_expr_jit_kind: field arguments must be colour matrices or gauge fields");
+        if (!(ncomp[k] = jit_ncomp_of_kind(field_kinds[k]))) return fail(QDP_ERR_KIND, "qdp_expr_jit_kind: field arguments must be colour matrices, gauge fields or fermions");
     JitExpr e;
     std::string err;
     if (jit_parse(expr, ncomp, nfields, nscalars, &e, &err) != 0) return fail(QDP_ERR_ARG, "qdp_expr_jit_kind: %s", err.c_str());
@@ -792,11 +792,11 @@ extern "C" int qdp_expr_jit_compile(const char* expr, const int* field_kinds, in
         return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: bad argument");
     int ncomp[4] = {0, 0, 0, 0};
     for (int k = 0; k < nfields; k++)
-        if (!(ncomp[k] = jit_ncomp_of_kind(field_kinds[k]))) return fail(QDP_ERR_KIND, "qdp_expr_jit_compile: field arguments must be colour matrices or gauge fields");
+        if (!(ncomp[k] = jit_ncomp_of_kind(field_kinds[k]))) return fail(QDP_ERR_KIND, "qdp_expr_jit_compile: field arguments must be colour matrices, gauge fields or fermions");
     JitExpr e;
     std::string err;
     if (jit_parse(expr, ncomp, nfields, nscalars, &e, &err) != 0) return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: %s", err.c_str());
-    if (sum && e.kind == JIT_MAT) return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: a sum needs a real or complex expression");
+    if (sum && (e.kind == JIT_MAT || e.kind == JIT_SPINOR)) return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: a sum needs a real or complex expression");
     if (!sum && e.kind == JIT_REAL) return fail(QDP_ERR_ARG, "qdp_expr_jit_compile: an assignment needs a matrix or complex expression");
     if (jit_compile_only(e, prec == QDP_F64, sum != 0, cubin_bytes, &err) != 0) return fail(QDP_ERR_CUDA, "qdp_expr_jit_compile: %s", err.c_str());
     return QDP_OK;
@@ -815,7 +815,7 @@ static int jit_common(const char* who, qdp_field* dst, int slot_d, const char* e
         if (!ok_field(fields[k])) return fail(QDP_ERR_ARG, "%s: field argument %d is not a field", who, k);
         const int rc = check_pair(who, fields[0], fields[k]);
         if (rc != QDP_OK) return rc;
-        if (!(ncomp[k] = jit_ncomp_of_kind(fields[k]->kind))) return fail(QDP_ERR_KIND, "%s: field arguments must be colour matrices or gauge fields", who);
+        if (!(ncomp[k] = jit_ncomp_of_kind(fields[k]->kind))) return fail(QDP_ERR_KIND, "%s: field arguments must be colour matrices, gauge fields or fermions", who);
         a.f[k] = fields[k]->data;
         a.ncomp[k] = ncomp[k];
     }
@@ -835,13 +835,15 @@ static int jit_common(const char* who, qdp_field* dst, int slot_d, const char* e
             cd = slot_d * 9;
         } else if (e.kind == JIT_CPLX) {
             if (dst->kind != QDP_COMPLEX) return fail(QDP_ERR_KIND, "%s: a complex expression needs a QDP_COMPLEX destination", who);
+        } else if (e.kind == JIT_SPINOR) {
+            if (dst->kind != QDP_FERMION) return fail(QDP_ERR_KIND, "%s: a spinor expression needs a QDP_FERMION destination", who);
         } else return fail(QDP_ERR_ARG, "%s: a real expression cannot be assigned (wrap it in a sum)", who);
         nd = dst->ncomp;
         if (e.has_shift)
             for (int k = 0; k < nfields; k++)
                 if ((e.fields_used >> k & 1) && overlaps(dst, fields[k]))
                     return fail(QDP_ERR_ALIAS, "%s: the destination is an operand of an expression that reads neighbour sites", who);
-    } else if (e.kind == JIT_MAT) return fail(QDP_ERR_ARG, "%s: a sum needs a real or complex expression", who);
+    } else if (e.kind == JIT_MAT || e.kind == JIT_SPINOR) return fail(QDP_ERR_ARG, "%s: a sum needs a real or complex expression", who);
     ENTER(l);
     cudaError_t ce = dst ? jit_launch_assign(e, fields[0]->prec == QDP_F64, l->geom, a, dst->data, nd, cd, subset, l->stream, &err)
                          : jit_launch_sum(e, fields[0]->prec == QDP_F64, l->geom, a, subset, reduce_buf(l), l->stream, &err);

@@ -9,7 +9,7 @@
 //
 // is written below as  real(trace(U<MU>() * shift<MU,+1>(U<NU>()) * adj(shift<NU,+1>(U<MU>())) * adj(U<NU>())))
 // and handed to sum2_kernel.  Leaves:  M<ARG,NCOMP,SLOT> (matrix SLOT of field operand ARG), Mrt<ARG> (slot chosen at
-// run time), Sc<K> (real scalar operand K).  Nodes:  a * b, a + b, adj(a), trace(a), real(a), shift<MU,SIGN>(a) and
+// run time), F<ARG> (fermion field operand ARG), Sc<K> (real scalar operand K).  Nodes:  a * b, a + b, adj(a), trace(a), real(a), shift<MU,SIGN>(a) and
 // shift_rt(a) -- a shift moves the evaluation point of its whole sub-expression, so shift<NU,-1>(adj(U<NU>()) *
 // U<MU>() * shift<MU,+1>(U<NU>())) is the lower staple with its two-hop leaf.  trace(a * b) and real(trace(a * b)) are
 // evaluated without forming the product (9 complex / 18 real multiply-adds).  Assignment under a subset:
@@ -78,6 +78,53 @@ template <class T> __device__ __forceinline__ Mat3<T> v_add(const Mat3<T>& a, co
 template <class T> __device__ __forceinline__ Cx<T> v_add(Cx<T> a, Cx<T> b) { return a + b; }
 template <class T> __device__ __forceinline__ T v_add(T a, T b) { return a + b; }
 
+// spin-colour vectors (fermions): a colour matrix rotates the colour index of each spin component (the hopping term's product)
+template <class T> __device__ __forceinline__ Spinor<T> v_mul(const Mat3<T>& u, const Spinor<T>& p) {
+    Spinor<T> r;
+#pragma unroll
+    for (int sp = 0; sp < 4; sp++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            Cx<T> s = u.e[a * 3] * p.e[sp * 3];
+            cmad(s, u.e[a * 3 + 1], p.e[sp * 3 + 1]);
+            cmad(s, u.e[a * 3 + 2], p.e[sp * 3 + 2]);
+            r.e[sp * 3 + a] = s;
+        }
+    return r;
+}
+template <class T> __device__ __forceinline__ Spinor<T> v_mul(T s, const Spinor<T>& p) {
+    Spinor<T> r;
+#pragma unroll
+    for (int i = 0; i < 12; i++) r.e[i] = cx<T>(s * p.e[i].re, s * p.e[i].im);
+    return r;
+}
+template <class T> __device__ __forceinline__ Spinor<T> v_mul(const Spinor<T>& p, T s) { return v_mul(s, p); }
+template <class T> __device__ __forceinline__ Spinor<T> v_mul(Cx<T> z, const Spinor<T>& p) {
+    Spinor<T> r;
+#pragma unroll
+    for (int i = 0; i < 12; i++) r.e[i] = z * p.e[i];
+    return r;
+}
+template <class T> __device__ __forceinline__ Spinor<T> v_add(const Spinor<T>& a, const Spinor<T>& b) {
+    Spinor<T> r;
+#pragma unroll
+    for (int i = 0; i < 12; i++) r.e[i] = a.e[i] + b.e[i];
+    return r;
+}
+// site-local norm and inner product (QDP++ localNorm2 / localInnerProduct): sum over spin and colour
+template <class T> __device__ __forceinline__ T v_norm2(const Spinor<T>& a) {
+    T s = 0;
+#pragma unroll
+    for (int i = 0; i < 12; i++) { s = fma(a.e[i].re, a.e[i].re, s); s = fma(a.e[i].im, a.e[i].im, s); }
+    return s;
+}
+template <class T> __device__ __forceinline__ Cx<T> v_inner(const Spinor<T>& a, const Spinor<T>& b) {
+    Cx<T> s = cx<T>(0, 0);
+#pragma unroll
+    for (int i = 0; i < 12; i++) cmad_conj_a(s, a.e[i], b.e[i]);
+    return s;
+}
+
 template <class T> __device__ __forceinline__ Cx<T> v_trace(const Mat3<T>& a) { return a.e[0] + a.e[4] + a.e[8]; }
 template <class T> __device__ __forceinline__ T v_real(Cx<T> a) { return a.re; }
 template <class T> __device__ __forceinline__ T v_imag(Cx<T> a) { return a.im; }
@@ -95,6 +142,13 @@ template <int ARG> struct Mrt : Node {
         using T2 = typename Vec2<T>::type;
         const Geom& g = e.g;
         return ld_mat_at<T>(site_ptr(static_cast<const T2*>(e.a.f[ARG]), e.a.ncomp[ARG], e.a.slot[ARG] * 9, e.x.index(g)));
+    }
+};
+template <int ARG> struct F : Node {   // fermion field operand ARG
+    template <class T> __device__ __forceinline__ static Spinor<T> eval(const Env<T>& e) {
+        using T2 = typename Vec2<T>::type;
+        const Geom& g = e.g;
+        return ld_spinor_at<T>(site_ptr(static_cast<const T2*>(e.a.f[ARG]), 12, 0, e.x.index(g)));
     }
 };
 template <int K> struct Sc : Node {
@@ -161,6 +215,14 @@ template <class A, class B> struct Real<Trace<Product<A, B>>> : Node {
     }
 };
 
+template <class E> struct Norm2 : Node {
+    template <class T> __device__ __forceinline__ static T eval(const Env<T>& e) { return v_norm2(E::template eval<T>(e)); }
+};
+template <class A, class B> struct Inner : Node {
+    template <class T> __device__ __forceinline__ static Cx<T> eval(const Env<T>& e) {
+        return v_inner(A::template eval<T>(e), B::template eval<T>(e));
+    }
+};
 template <class E> struct Imag : Node {
     template <class T> __device__ __forceinline__ static T eval(const Env<T>& e) { return v_imag(E::template eval<T>(e)); }
 };
@@ -181,6 +243,14 @@ template <class E> constexpr ShiftedRt<E> shift_rt(E) { return {}; }
 
 // ---- kernels ---------------------------------------------------------------------------------------
 template <class T> __device__ __forceinline__ void store_value(typename Vec2<T>::type* p, const Mat3<T>& v) { st_mat_at<T>(p, v); }
+template <class T> __device__ __forceinline__ void store_value(typename Vec2<T>::type* p, const Spinor<T>& v) {
+#pragma unroll
+    for (int c = 0; c < 12; c++) {
+        typename Vec2<T>::type o;
+        o.x = v.e[c].re; o.y = v.e[c].im;
+        p[c * kLane] = o;
+    }
+}
 template <class T> __device__ __forceinline__ void store_value(typename Vec2<T>::type* p, const Cx<T>& v) {
     typename Vec2<T>::type o;
     o.x = v.re; o.y = v.im;

@@ -91,7 +91,7 @@ cudaError_t launch_expr_trace_mul(int prec, const Geom& g, void* dst, const void
                                   int nb, int ib, bool adj_b, int mu, int sign, int subset, const ReduceBuf& rb, cudaStream_t st);
 
 // jit.cu: run-time expressions (text -> node type of expr.cuh -> NVRTC -> cached kernel)
-enum { JIT_MAT = 0, JIT_CPLX = 1, JIT_REAL = 2 };   // value kind of an expression: 3x3 matrix, complex, real
+enum { JIT_MAT = 0, JIT_CPLX = 1, JIT_REAL = 2, JIT_SPINOR = 3 };   // value kind of an expression: 3x3 matrix, complex, real, spin-colour vector
 struct JitExpr {
     std::string type;       // the expression as a node type of expr.cuh
     int kind;
@@ -99,7 +99,7 @@ struct JitExpr {
     unsigned fields_used;   // bit k: field argument k occurs
 };
 namespace ex { struct Args; }
-// ncomp[k]: components per site of field argument k (9 or 36).  Returns 0, or -1 with *err set.  No device needed.
+// ncomp[k]: components per site of field argument k (9, 36 or 12).  Returns 0, or -1 with *err set.  No device needed.
 int jit_parse(const char* text, const int* ncomp, int nfields, int nscalars, JitExpr* out, std::string* err);
 std::string jit_source(const JitExpr& e, int prec, bool sum);
 int jit_compile_only(const JitExpr& e, int prec, bool sum, size_t* cubin_bytes, std::string* err);

@@ -8,12 +8,16 @@
 //   expr   := term { '+' term }
 //   term   := factor { '*' factor }
 //   factor := 'adj' '(' expr ')' | 'trace' '(' expr ')' | 'real' '(' expr ')' | 'imag' '(' expr ')'
+//           | 'norm2' '(' expr ')' | 'inner' '(' expr ',' expr ')'
 //           | 'shift' '(' expr ',' ('+'|'-') DIGIT ')' | '(' expr ')' | leaf
-//   leaf   := 'f' DIGIT [ '[' DIGIT ']' ]     matrix [slot] of field argument DIGIT (slot: link of a gauge field, default 0)
+//   leaf   := 'f' DIGIT [ '[' DIGIT ']' ]     field argument DIGIT: matrix [slot] of a colour-matrix or gauge field (slot:
+//                                             link of a gauge field, default 0), or the spinor of a fermion field
 //           | 's' DIGIT                       real scalar argument DIGIT
-// Value kinds: matrix (3x3 complex), complex, real.  f -> matrix, s -> real, adj keeps the kind, trace: matrix ->
-// complex, real/imag: complex -> real, shift keeps the kind (shift(e, +mu)(x) = e(x + mu), A3), '+' needs equal kinds,
-// '*': matrix*matrix, real*anything, anything*real, complex*complex.
+// Value kinds: matrix (3x3 complex), complex, real, spinor (4 spin x 3 colour).  s -> real, adj keeps the kind (not
+// defined on spinors), trace: matrix -> complex, real/imag: complex -> real, norm2: spinor -> real, inner: two spinors ->
+// complex (the first conjugated), shift keeps the kind (shift(e, +mu)(x) = e(x + mu), A3), '+' needs equal kinds,
+// '*': matrix*matrix, matrix*spinor (colour rotation of every spin component), real*anything, anything*real,
+// complex*complex, complex*spinor.
 //
 // NVRTC is loaded with dlopen at the first compilation (the library does not link it), the headers the generated
 // translation unit includes are embedded in this object at build time (build.py -> jit_headers.inc), and the cubin is
@@ -73,14 +77,15 @@ struct Parser {
         while (eat('*')) {
             Parsed r;
             if (!factor(r)) return false;
-            if (out.kind == JIT_MAT && r.kind == JIT_MAT) { out.type = "Product<" + out.type + ", " + r.type + " >"; }
+            if (out.kind == JIT_MAT && (r.kind == JIT_MAT || r.kind == JIT_SPINOR)) { out.type = "Product<" + out.type + ", " + r.type + " >"; out.kind = r.kind; }
             else if (out.kind == JIT_REAL) { out.type = "Product<" + out.type + ", " + r.type + " >"; out.kind = r.kind; }
             else if (r.kind == JIT_REAL) {
-                // real factors go first (expr.cuh has v_mul(real, complex) but not the mirror image)
-                out.type = out.kind == JIT_MAT ? "Product<" + out.type + ", " + r.type + " >" : "Product<" + r.type + ", " + out.type + " >";
+                // real factors go first where expr.cuh has no mirror image of v_mul(real, x)
+                out.type = out.kind == JIT_CPLX ? "Product<" + r.type + ", " + out.type + " >" : "Product<" + out.type + ", " + r.type + " >";
             }
-            else if (out.kind == JIT_CPLX && r.kind == JIT_CPLX) { out.type = "Product<" + out.type + ", " + r.type + " >"; }
-            else return fail("'*' of a matrix and a complex number is not defined");
+            else if (out.kind == JIT_CPLX && (r.kind == JIT_CPLX || r.kind == JIT_SPINOR)) { out.type = "Product<" + out.type + ", " + r.type + " >"; out.kind = r.kind; }
+            else if (out.kind == JIT_SPINOR && r.kind == JIT_CPLX) { out.type = "Product<" + r.type + ", " + out.type + " >"; }
+            else return fail("'*' is not defined for these operand kinds");
         }
         return true;
     }
@@ -94,7 +99,24 @@ struct Parser {
         return true;
     }
     bool factor(Parsed& out) {
-        if (word("adj")) return unary("Adjoint", out, -1, -1, "");
+        if (word("adj")) {
+            if (!unary("Adjoint", out, -1, -1, "")) return false;
+            if (out.kind == JIT_SPINOR) return fail("adj() of a spinor is not defined");
+            return true;
+        }
+        if (word("norm2")) return unary("Norm2", out, JIT_SPINOR, JIT_REAL, "norm2() takes a spinor");
+        if (word("inner")) {
+            Parsed b;
+            if (!eat('(')) return fail("'(' expected");
+            if (!expr(out)) return false;
+            if (!eat(',')) return fail("',' expected");
+            if (!expr(b)) return false;
+            if (!eat(')')) return fail("')' expected");
+            if (out.kind != JIT_SPINOR || b.kind != JIT_SPINOR) return fail("inner() takes two spinors");
+            out.type = "Inner<" + out.type + ", " + b.type + " >";
+            out.kind = JIT_CPLX;
+            return true;
+        }
         if (word("trace")) return unary("Trace", out, JIT_MAT, JIT_CPLX, "trace() takes a matrix");
         if (word("real")) return unary("Real", out, JIT_CPLX, JIT_REAL, "real() takes a complex number");
         if (word("imag")) return unary("Imag", out, JIT_CPLX, JIT_REAL, "imag() takes a complex number");
@@ -124,8 +146,15 @@ struct Parser {
             int k = 0, slot = 0;
             if (!digit(k)) return false;
             if (k >= nfields) return fail("field argument out of range");
+            if (ncomp[k] == 12) {
+                if (*s == '[') return fail("a fermion field has no slots");
+                out.type = "F<" + std::to_string(k) + ">";
+                out.kind = JIT_SPINOR;
+                fields_used |= 1u << k;
+                return true;
+            }
             if (*s == '[') { s++; if (!digit(slot)) return false; if (!eat(']')) return fail("']' expected"); }
-            if (ncomp[k] != 9 && ncomp[k] != 36) return fail("field arguments must be colour matrices or gauge fields");
+            if (ncomp[k] != 9 && ncomp[k] != 36) return fail("field arguments must be colour matrices, gauge fields or fermions");
             if (slot >= ncomp[k] / 9) return fail("slot out of range");
             out.type = "M<" + std::to_string(k) + ", " + std::to_string(ncomp[k]) + ", " + std::to_string(slot) + ">";
             out.kind = JIT_MAT;

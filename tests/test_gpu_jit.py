@@ -144,3 +144,51 @@ def test_jit_cache_errors_and_aliasing(qdp):
     psi = qdp.field_from_host(lat, 2, synth.spinor(dims, 3))
     with pytest.raises(qdp.QdpError):      # fermions are not matrix operands
         qdp.qdp_expr_jit_assign(dst, 0, "f0", [psi])
+
+
+HOP = " + ".join(f"f0[{m}] * shift(f1, +{m}) + shift(adj(f0[{m}]) * f1, -{m})" for m in range(4))
+
+
+@pytest.mark.parametrize("dims", SMALL + [C2])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_jit_spinor_expressions(qdp, dims, prec):
+    """Fermion leaves: the hopping term (def. 5) and a psi + b hop(psi) (def. 6) written as text, their fused norm2 and
+    innerProduct, against the oracle's evaluator and against the hand-fused kernels."""
+    hu = synth.round_to(synth.gauge_hot(dims, _seed(dims) + 211), prec)
+    hp = synth.round_to(synth.spinor(dims, _seed(dims) + 212), prec)
+    lat = qdp.qdp_lattice_create(dims)
+    u, psi = qdp.field_from_host(lat, 1, hu), qdp.field_from_host(lat, 2, hp)
+    V = synth.volume(dims)
+    mask = oracle.parity_mask(dims)
+    h64 = [hu.astype(np.complex128), hp.astype(np.complex128)]
+    sc = _scalars((0.3, -0.7), prec)
+    axpy = f"s0 * f1 + s1 * ({HOP})"
+    want_hop, kind = ee.evaluate(dims, HOP, h64)
+    assert kind == ee.SPINOR
+    want_axpy, _ = ee.evaluate(dims, axpy, h64, sc)
+    sentinel = np.full((V, 4, 3), 3.0 + 1.0j, hp.dtype)
+    for subset in (0, 1, 2):
+        sel = np.ones(V, bool) if subset == 0 else (mask == (subset - 1))
+        for text, want, s in ((HOP, want_hop, ()), (axpy, want_axpy, (0.3, -0.7))):
+            chi = qdp.field_from_host(lat, 2, sentinel)
+            qdp.qdp_expr_jit_assign(chi, 0, text, [u, psi], s, subset)
+            got = qdp.field_to_host(chi)
+            assert np.array_equal(got[~sel], sentinel[~sel])
+            assert site_rel_err(got[sel], want[sel]).max() <= TOL_SITE[prec], (text[:30], subset)
+        n2 = qdp.qdp_expr_jit_sum(f"norm2({HOP})", [u, psi], (), subset)
+        w = ee.total(dims, f"norm2({HOP})", h64, (), sel)
+        assert abs(n2 - w) <= TOL_SUM[prec] * abs(w) and n2.imag == 0.0
+        ip = qdp.qdp_expr_jit_sum(f"inner(f1, {HOP})", [u, psi], (), subset)
+        wi = ee.total(dims, f"inner(f1, {HOP})", h64, (), sel)
+        assert abs(ip - wi) <= TOL_SUM[prec] * 8 * float((np.abs(h64[1][sel]) ** 2).sum())
+    # the hand-fused kernel evaluates the same definition
+    a, b = qdp.qdp_field_alloc(lat, 2, u.prec), qdp.qdp_field_alloc(lat, 2, u.prec)
+    qdp.qdp_expr_jit_assign(a, 0, HOP, [u, psi])
+    qdp.qdp_hop(b, u, psi)
+    assert site_rel_err(qdp.field_to_host(a), qdp.field_to_host(b)).max() <= (1e-13 if prec == "f64" else 1e-5)
+    # destination kinds
+    m = qdp.qdp_field_alloc(lat, 0, u.prec)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_expr_jit_assign(m, 0, HOP, [u, psi])
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_expr_jit_sum(HOP, [u, psi])

@@ -14,9 +14,10 @@ LOWER = "shift(adj(f0[{n}]) * f0[{m}] * shift(f0[{n}], +{m}), -{n})"
 
 
 def test_parser_precedence_and_associativity():
-    assert ee.parse("f0 + f1 * f2") == ("+", ("f", 0, 0), ("*", ("f", 1, 0), ("f", 2, 0)))
-    assert ee.parse("f0 * f1 * f2") == ("*", ("*", ("f", 0, 0), ("f", 1, 0)), ("f", 2, 0))
-    assert ee.parse("(f0 + f1) * s2") == ("*", ("+", ("f", 0, 0), ("f", 1, 0)), ("s", 2))
+    assert ee.parse("f0 + f1 * f2") == ("+", ("f", 0, None), ("*", ("f", 1, None), ("f", 2, None)))
+    assert ee.parse("f0 * f1 * f2") == ("*", ("*", ("f", 0, None), ("f", 1, None)), ("f", 2, None))
+    assert ee.parse("(f0 + f1) * s2") == ("*", ("+", ("f", 0, None), ("f", 1, None)), ("s", 2))
+    assert ee.parse("inner(f2, f0[1] * f2)") == ("inner", ("f", 2, None), ("*", ("f", 0, 1), ("f", 2, None)))
     assert ee.parse("shift(adj(f0[3]), -2)") == ("shift", ("adj", ("f", 0, 3)), 2, -1)
     for bad in ("f0 +", "f0 * * f1", "shift(f0, 2)", "trace f0", "f0[", "g0", "f0 f1", "(f0"):
         with pytest.raises(ee.ExprError):
@@ -31,6 +32,14 @@ def test_kinds():
     assert ee.kind_of(ee.parse("s0 * f1 * s1"), slots) == ee.MAT
     assert ee.kind_of(ee.parse("trace(f1) * trace(f1)"), slots) == ee.CPLX
     for bad in ("f0 + trace(f1)", "trace(trace(f1))", "real(f1)", "f1 * trace(f1)", "f1[1]", "f0[4]", "f2", "shift(f1, +4)"):
+        with pytest.raises(ee.ExprError):
+            ee.kind_of(ee.parse(bad), slots)
+    slots = [4, 1, 0]      # gauge, colour matrix, fermion
+    assert ee.kind_of(ee.parse("f0[1] * shift(f2, +1)"), slots) == ee.SPINOR
+    assert ee.kind_of(ee.parse("s0 * f2 + f1 * f2 * s1 + trace(f1) * f2 + f2 * trace(f1)"), slots) == ee.SPINOR
+    assert ee.kind_of(ee.parse("norm2(f1 * f2)"), slots) == ee.REAL
+    assert ee.kind_of(ee.parse("inner(f2, f0[3] * f2)"), slots) == ee.CPLX
+    for bad in ("f2 * f1", "f2 * f2", "adj(f2)", "trace(f2)", "f2[0]", "norm2(f1)", "inner(f2, f1)", "f2 + f1", "inner(f2)"):
         with pytest.raises(ee.ExprError):
             ee.kind_of(ee.parse(bad), slots)
 
@@ -95,6 +104,32 @@ def test_algebraic_identities():
     assert abs(ev("trace(f0[1] * f1)")[x] - want) < 1e-13
 
 
+HOP = " + ".join(f"f0[{m}] * shift(f1, +{m}) + shift(adj(f0[{m}]) * f1, -{m})" for m in range(4))
+
+
+@pytest.mark.parametrize("dims", DIMS)
+def test_spinor_expressions_are_def5_and_def6(dims):
+    """The hopping term, the fused a psi + b hop(psi), norm2 and innerProduct written as expressions equal the C oracle's
+    functions (pinned on numpy brute force, plane waves, gauge covariance: tests/test_oracle_hop.py, _reductions.py)."""
+    hu, hp = synth.gauge_hot(dims, 47), synth.spinor(dims, 48)
+    chi, kind = ee.evaluate(dims, HOP, [hu, hp])
+    assert kind == ee.SPINOR
+    want = oracle.hop(dims, hu, hp)
+    assert np.abs(chi - want).max() < 1e-13 * np.abs(want).max()
+    axpy, _ = ee.evaluate(dims, f"s0 * f1 + s1 * ({HOP})", [hu, hp], (0.3, -0.7))
+    w2 = oracle.axpy_hop(dims, 0.3, -0.7, hu, hp)
+    assert np.abs(axpy - w2).max() < 1e-13 * np.abs(w2).max()
+    n2 = ee.total(dims, f"norm2({HOP})", [hu, hp])
+    assert abs(n2.real - oracle.norm2(dims, want)) < 1e-12 * n2.real and n2.imag == 0.0
+    ip = ee.total(dims, f"inner(f1, {HOP})", [hu, hp])
+    assert abs(ip - oracle.inner(dims, hp, want)) < 1e-12 * abs(n2)
+    # the colour rotation leaves the spin index alone: a one-hot spinor stays in its spin component
+    one = np.zeros_like(hp)
+    one[:, 2, 1] = 1.0
+    v, _ = ee.evaluate(dims, "f0[3] * f1", [hu, one])
+    assert np.abs(v[:, [0, 1, 3]]).max() == 0.0 and np.abs(v[:, 2] - hu[:, 3, :, 1]).max() < 1e-15
+
+
 # ---- the library's host-side front end (no GPU): it must accept and reject what the oracle's language does ------
 VALID = [("f0[1] * f1", ee.MAT), ("trace(f0[1] * f1)", ee.CPLX), ("real(trace(f1)) * s0", ee.REAL), ("s0 * f1 * s1", ee.MAT),
          ("trace(f1) * trace(adj(f1)) + trace(f0[3])", ee.CPLX), (LOWER.format(m=0, n=2), ee.MAT), ("( f1+adj( f1 ) )*s1", ee.MAT),
@@ -117,6 +152,16 @@ def test_library_front_end_agrees_with_the_oracle_language():
             ee.kind_of(tree, [4, 1])
             if "s2" in text:
                 raise ee.ExprError("scalar argument out of range")   # the oracle takes its scalars from a Python sequence
+    kinds = [q.QDP_GAUGE, q.QDP_COLOR_MATRIX, q.QDP_FERMION]
+    for text, kind in [("f0[1] * shift(f2, +1)", ee.SPINOR), ("s0 * f2 + f1 * f2 * s1 + trace(f1) * f2 + f2 * trace(f1)", ee.SPINOR),
+                       ("norm2(f1 * f2)", ee.REAL), ("inner(f2, f0[3] * f2)", ee.CPLX), (HOP.replace("f1", "f2"), ee.SPINOR)]:
+        assert ee.kind_of(ee.parse(text), [4, 1, 0]) == kind
+        assert q.qdp_expr_jit_kind(text, kinds, 2) == kind, text
+    for text in ("f2 * f1", "f2 * f2", "adj(f2)", "trace(f2)", "f2[0]", "norm2(f1)", "inner(f2, f1)", "f2 + f1", "inner(f2)"):
+        with pytest.raises(q.QdpError):
+            q.qdp_expr_jit_kind(text, kinds, 2)
+        with pytest.raises(ee.ExprError):
+            ee.kind_of(ee.parse(text), [4, 1, 0])
 
 
 def test_nvrtc_compiles_an_expression_once_without_a_gpu():
