@@ -593,7 +593,7 @@ def main():
     ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--e2e-pipes", type=int, default=3, help="lattices (host threads) pipelined in the e2e leg")
+    ap.add_argument("--e2e-pipes", type=int, default=2, help="lattices (host threads) pipelined in the e2e leg")
     ap.add_argument("--cpu-fraction", type=int, default=1, help="cpu_baseline runs on V/fraction sites (1: one whole pass, ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
