@@ -253,8 +253,12 @@ static int jit_get(const JitExpr& e, int prec, bool sum, bool load, Compiled** o
             *err = "nvrtcCreateProgram failed";
             return -1;
         }
+#ifdef QDP_BOUNDS_CHECK   // the bounds-checked build validates the site addresses of its run-time kernels too
+        const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "-DQDP_BOUNDS_CHECK"};
+#else
         const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo"};
-        const nvrtcResult rc = g_nvrtc.compile(prog, 3, opts);
+#endif
+        const nvrtcResult rc = g_nvrtc.compile(prog, (int)(sizeof(opts) / sizeof(opts[0])), opts);
         if (rc != NVRTC_SUCCESS) {
             size_t n = 0;
             g_nvrtc.log_size(prog, &n);

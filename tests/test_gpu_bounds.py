@@ -32,8 +32,10 @@ def test_small_lattice_suite_under_the_bounds_checked_build():
     r = subprocess.run([sys.executable, "-c", SELFTEST], capture_output=True, text=True, env=env, cwd=ROOT, timeout=600)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "libqdp_b200_bc.so" in r.stdout and r.stdout.count("QDP_BOUNDS") == 3, r.stdout
-    # every op, subset, kind and precision on the tiny, ragged and anisotropic lattices (C2 left out: time)
-    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join("tests", "test_gpu_parity.py"), "-x", "-q", "-s", "-m", "gpu",
+    # every op, subset, kind and precision on the tiny, ragged and anisotropic lattices (C2 left out: time); the run-time
+    # expression kernels are compiled by NVRTC with the same check
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join("tests", "test_gpu_parity.py"), os.path.join("tests", "test_gpu_jit.py"),
+                        "-x", "-q", "-s", "-m", "gpu",
                         "-k", "not dims5", "-p", "no:cacheprovider"],
                        capture_output=True, text=True, env=env, cwd=ROOT, timeout=3000)
     out = r.stdout + r.stderr
