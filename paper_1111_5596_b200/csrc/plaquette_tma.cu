@@ -24,7 +24,14 @@ namespace qdp {
 
 constexpr int kPtConsumers = 12;                     // 2 parities x 6 planes
 constexpr int kPtThreads = (kPtConsumers + 1) * 32;  // + the producer warp
-constexpr int kPtOwnSlots = 3, kPtHaloSlots = 2;
+// ring depths: fp64 3 + 2 slots = one step of lookahead in 221 KB; fp32 slots are half as large, so 6 + 4 slots give three
+// steps of lookahead in the same shared memory (a step is consumed in ~0.5 us in fp32, less than the latency of its copies)
+#ifndef PT_OWN_F32
+#define PT_OWN_F32 6
+#endif
+#ifndef PT_HALO_F32
+#define PT_HALO_F32 4
+#endif
 
 struct PlaqTmaGeo {
     int P;          // block pairs per (x0, x1) plane = Lh0 * L1 / 32
@@ -39,6 +46,7 @@ template <class T> struct PlaqTmaSmem {
     static constexpr int kGauge = 4 * kLink;
     static constexpr uint32_t kLinkBytes = kLink * sizeof(T2);
     static constexpr uint32_t kGaugeBytes = 4 * kLinkBytes;
+    static constexpr int kPtOwnSlots = sizeof(T) == 8 ? 3 : PT_OWN_F32, kPtHaloSlots = sizeof(T) == 8 ? 2 : PT_HALO_F32;
     T2 own[kPtOwnSlots][2][kGauge];                  // [slot][parity]
     T2 halo2[kPtHaloSlots][2][3 * kLink];            // links 0, 1, 3 of the plane at x2+1
     T2 halo3[kPtHaloSlots][2][3 * kLink];            // links 0, 1, 2 of the plane at x3+1
@@ -90,7 +98,7 @@ __device__ __forceinline__ double plaq_tma_consume(PlaqTmaSmem<T>& sm, const Pla
         const int x2 = q % pg.L2, x3 = q / pg.L2;
         for (int j = 0; j < pg.P; j++) {
             const int it0 = own_base + j, it1 = it0 + 1;
-            const int s0 = it0 % kPtOwnSlots, s1 = it1 % kPtOwnSlots, hs = halo_item % kPtHaloSlots;
+            const int s0 = it0 % S::kPtOwnSlots, s1 = it1 % S::kPtOwnSlots, hs = halo_item % S::kPtHaloSlots;
             // geometry of site (p, 32 j + lane) of this plane
             const int o = 32 * j + lane;
             const int x1 = o >> pg.lg, hx = o & (pg.Lh0 - 1);
@@ -114,9 +122,9 @@ __device__ __forceinline__ double plaq_tma_consume(PlaqTmaSmem<T>& sm, const Pla
             const T2* pB = nb(mu, nu);               // U_nu(x+mu)
             const T2* pA2 = here + nu * S::kLink;    // U_nu(x)
             const T2* pB2 = nb(nu, mu);              // U_mu(x+nu)
-            mbar_wait(&sm.own_full[s0], (it0 / kPtOwnSlots) & 1);
-            mbar_wait(&sm.own_full[s1], (it1 / kPtOwnSlots) & 1);
-            mbar_wait(&sm.halo_full[hs], (halo_item / kPtHaloSlots) & 1);
+            mbar_wait(&sm.own_full[s0], (it0 / S::kPtOwnSlots) & 1);
+            mbar_wait(&sm.own_full[s1], (it1 / S::kPtOwnSlots) & 1);
+            mbar_wait(&sm.halo_full[hs], (halo_item / S::kPtHaloSlots) & 1);
             const Mat3<T> A = lds_mat<T>(pA);
             const Mat3<T> B = lds_mat<T>(pB);
             const Mat3<T> Pm = mul(A, B);
@@ -145,8 +153,8 @@ plaquette_tma_kernel(PlaqTmaGeo pg, const typename Vec2<T>::type* __restrict__ u
     S& sm = *reinterpret_cast<S*>(smem_pt);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int i = 0; i < kPtOwnSlots; i++) { mbar_init(&sm.own_full[i], 1); mbar_init(&sm.own_empty[i], kPtConsumers); }
-        for (int i = 0; i < kPtHaloSlots; i++) { mbar_init(&sm.halo_full[i], 1); mbar_init(&sm.halo_empty[i], kPtConsumers); }
+        for (int i = 0; i < S::kPtOwnSlots; i++) { mbar_init(&sm.own_full[i], 1); mbar_init(&sm.own_empty[i], kPtConsumers); }
+        for (int i = 0; i < S::kPtHaloSlots; i++) { mbar_init(&sm.halo_full[i], 1); mbar_init(&sm.halo_empty[i], kPtConsumers); }
         mbar_fence_init();
     }
     __syncthreads();
@@ -161,8 +169,8 @@ plaquette_tma_kernel(PlaqTmaGeo pg, const typename Vec2<T>::type* __restrict__ u
                 const int q3 = x2 + pg.L2 * (x3 + 1 == pg.L3 ? 0 : x3 + 1);
                 for (int j = 0; j <= pg.P; j++) {
                     {
-                        const int s = own_item % kPtOwnSlots;
-                        mbar_wait(&sm.own_empty[s], ((own_item / kPtOwnSlots) & 1) ^ 1);
+                        const int s = own_item % S::kPtOwnSlots;
+                        mbar_wait(&sm.own_empty[s], ((own_item / S::kPtOwnSlots) & 1) ^ 1);
                         mbar_arrive_expect_tx(&sm.own_full[s], 2 * S::kGaugeBytes);
                         const int jb = j == pg.P ? 0 : j;   // the x1 wrap: the plane's first pair again
 #ifdef QDP_BOUNDS_CHECK
@@ -175,8 +183,8 @@ plaquette_tma_kernel(PlaqTmaGeo pg, const typename Vec2<T>::type* __restrict__ u
                         own_item++;
                     }
                     if (j >= 1) {
-                        const int s = halo_item % kPtHaloSlots;
-                        mbar_wait(&sm.halo_empty[s], ((halo_item / kPtHaloSlots) & 1) ^ 1);
+                        const int s = halo_item % S::kPtHaloSlots;
+                        mbar_wait(&sm.halo_empty[s], ((halo_item / S::kPtHaloSlots) & 1) ^ 1);
                         mbar_arrive_expect_tx(&sm.halo_full[s], 12 * S::kLinkBytes);
                         for (int p = 0; p < 2; p++) {
                             const T2* b2 = u + (size_t)(p * pg.nblk_half + q2 * pg.P + (j - 1)) * S::kGauge;
