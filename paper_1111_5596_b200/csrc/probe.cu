@@ -139,6 +139,27 @@ __global__ void __launch_bounds__(NW * 32, 1) overlap_kernel(double* out, const 
     if (t == 123.456) out[0] = t;
 }
 
+// ---- bulk copies from L2 into shared memory: per-SM ingest rate against the number of active SMs ------------------
+// One lane per block keeps two 92,160-byte slots filled with `ncopies` cp.async.bulk copies per step from an L2-resident
+// buffer, issuing step s+1 before it waits for step s.  With few blocks the rate is what one SM can ingest; with one
+// block on every SM it is what the L2 can deliver to all of them (profiles/r2_microbench.md).
+__global__ void __launch_bounds__(32, 1) bulk_rate_kernel(const double2* __restrict__ src, int steps, int ncopies, int bytes_each) {
+    extern __shared__ __align__(128) unsigned char smem_probe[];
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_probe + 200704);
+    if (threadIdx.x == 0) { qdp::mbar_init(&bar[0], 1); qdp::mbar_init(&bar[1], 1); qdp::mbar_fence_init(); }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    const char* base = reinterpret_cast<const char*>(src) + (size_t)blockIdx.x * ncopies * bytes_each;
+    for (int s = 0; s < steps + 1; s++) {
+        if (s < steps) {
+            qdp::mbar_arrive_expect_tx(&bar[s & 1], ncopies * bytes_each);
+            for (int c = 0; c < ncopies; c++)
+                qdp::bulk_g2s(smem_probe + (s & 1) * 100352 + c * bytes_each, base + (size_t)c * bytes_each, bytes_each, &bar[s & 1]);
+        }
+        if (s >= 1) qdp::mbar_wait(&bar[(s - 1) & 1], ((s - 1) >> 1) & 1);
+    }
+}
+
 template <int CHAINS>
 __global__ void dfma_chain_kernel(double* out, int iters, double a, double b) {
     double v[CHAINS];
@@ -261,6 +282,31 @@ extern "C" int qdp_probe_overlap(int device, void* stream, int mode, int src_kin
     }
     if (e == cudaSuccess) *ms_per_step = (double)ms / steps;
     if (out) cudaFree(out);
+    if (src) cudaFree(src);
+    cudaSetDevice(prev);
+    return (int)e;
+}
+
+// blocks: active SMs (1 .. SM count); ncopies: copies per 92,160-byte step (5 -> 18,432 B each, 20 -> 4,608 B each).
+// *bytes_per_s = bytes copied per second by all blocks together.
+extern "C" int qdp_probe_bulk_rate(int device, void* stream, int blocks, int ncopies, double* bytes_per_s) {
+    if (!bytes_per_s || blocks < 1 || (ncopies != 5 && ncopies != 20)) return (int)cudaErrorInvalidValue;
+    cudaError_t e;
+    int prev = 0, sms = 0;
+    if ((e = cudaGetDevice(&prev)) != cudaSuccess) return (int)e;
+    if ((e = cudaSetDevice(device)) != cudaSuccess) return (int)e;
+    cudaStream_t st = (cudaStream_t)stream;
+    double2* src = nullptr;
+    const int steps = 400, smem = 200704 + 64;
+    float ms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess && blocks > sms) e = cudaErrorInvalidValue;
+    if (e == cudaSuccess) e = cudaMalloc(&src, (size_t)sms * 92160 + 1024);
+    if (e == cudaSuccess) e = cudaMemset(src, 0, (size_t)sms * 92160);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bulk_rate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess)
+        e = time_launches(st, 7, &ms, [&] { bulk_rate_kernel<<<blocks, 32, smem, st>>>(src, steps, ncopies, 92160 / ncopies); });
+    if (e == cudaSuccess) *bytes_per_s = (double)blocks * steps * 92160 / (ms * 1e-3);
     if (src) cudaFree(src);
     cudaSetDevice(prev);
     return (int)e;

@@ -20,6 +20,7 @@ def _get():
         lib.qdp_probe_dfma.argtypes, lib.qdp_probe_dfma.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, D], ctypes.c_int
         lib.qdp_probe_mix.argtypes, lib.qdp_probe_mix.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
         lib.qdp_probe_dfma_chain.argtypes, lib.qdp_probe_dfma_chain.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
+        lib.qdp_probe_bulk_rate.argtypes, lib.qdp_probe_bulk_rate.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
         lib.qdp_probe_overlap.argtypes, lib.qdp_probe_overlap.restype = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, D], ctypes.c_int
         _lib = lib
     return _lib
@@ -52,6 +53,11 @@ def overlap_ms_per_step(mode: int, src: int, pipe: int, device: int = 0, stream=
     return _call(_get().qdp_probe_overlap, device, stream, mode, src, pipe)
 
 
+def bulk_bytes_per_s(blocks: int, ncopies: int = 5, device: int = 0, stream=None) -> float:
+    """cp.async.bulk from an L2-resident buffer into shared memory, `blocks` active SMs; see csrc/probe.cu."""
+    return _call(_get().qdp_probe_bulk_rate, device, stream, blocks, ncopies)
+
+
 def main() -> None:
     import torch
     dev = torch.cuda.current_device()
@@ -76,6 +82,13 @@ def main() -> None:
                                  ("loads of step s+1 before DFMA of step s", 3, 1)):
             ms = overlap_ms_per_step(mode, src, pipe, dev)
             print(f"{sname:12s} {name:42s} {ms * 1e3:7.3f} us/step = {ms * 1e-3 * ghz * 1e9:6.0f} cycles/step")
+
+    print("cp.async.bulk from L2 into shared memory, 92,160 B per step and SM, two steps in flight")
+    nsm = props.multi_processor_count
+    for ncopies in (5, 20):
+        for blocks in (8, nsm // 4, nsm // 2, nsm):
+            r = bulk_bytes_per_s(blocks, ncopies, dev)
+            print(f"{ncopies:2d} copies of {92160 // ncopies:5d} B, {blocks:3d} SMs: {r / 1e12:6.2f} TB/s in total = {r / blocks / (ghz * 1e9):6.1f} B/clk/SM")
 
 
 if __name__ == "__main__":
