@@ -169,7 +169,12 @@ def test_nvrtc_compiles_an_expression_once_without_a_gpu():
     kinds = [q.QDP_GAUGE]
     text = "trace(f0[0] * adj(shift(f0[1], -2))) * s0"
     before = q.qdp_expr_jit_compilations()
-    size = q.qdp_expr_jit_compile(text, kinds, 1, q.QDP_F64, sum_=True)
+    try:
+        size = q.qdp_expr_jit_compile(text, kinds, 1, q.QDP_F64, sum_=True)
+    except q.QdpError as exc:
+        if "libnvrtc" in str(exc):
+            pytest.skip("no libnvrtc on this machine")
+        raise
     assert size > 1000 and q.qdp_expr_jit_compilations() == before + 1
     assert q.qdp_expr_jit_compile(text, kinds, 1, q.QDP_F64, sum_=True) == size      # cached
     assert q.qdp_expr_jit_compilations() == before + 1
