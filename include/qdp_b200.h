@@ -267,6 +267,39 @@ int qdp_norm2(const qdp_field* f, qdp_subset subset, double* out);
 int qdp_inner(const qdp_field* a, const qdp_field* b, qdp_subset subset, double out[2]);
 int qdp_sum(const qdp_field* f, qdp_subset subset, double* out);
 
+/* qdp_sum for callers that cannot allocate device memory (def. 6, the same sum as qdp_sum).
+ *
+ * Some callers hold raw device pointers and a stream and are not allowed a cudaMalloc: a plug-in
+ * inside a framework whose own allocator has claimed the whole GPU, a latency-bound loop that
+ * cannot take the device-wide synchronisation cudaMalloc/cudaFree imply, or code that simply has
+ * no qdp_lattice (creating one allocates scratch, staging and pinned memory).  This entry point
+ * needs no handle and allocates nothing, on the device or through any library routine: its
+ * per-block partial sums go to a fixed 36,864-byte __device__ array compiled into the library
+ * (held by every GPU that loads it, until the process exits).
+ *
+ *   dims        host, the four extents (even, >= 2), as for qdp_lattice_create
+ *   ncomp       complex components per site, 1 <= ncomp <= 36 (QDP_COMPLEX 1, QDP_COLOR_MATRIX 9,
+ *               QDP_FERMION 12, QDP_GAUGE 36).  More than 36 does not fit the fixed scratch:
+ *               QDP_ERR_ARG, message names the limit
+ *   field_dev   device, on the CURRENT device, a field in the library's device layout (the memory
+ *               behind qdp_field_wrap / qdp_cache_acquire), read only; bytes must equal
+ *               qdp_field_bytes of that lattice, kind and precision, else QDP_ERR_ARG
+ *   out_dev     device-accessible (device or mapped pinned host memory), 2 * ncomp doubles:
+ *               out_dev[2c], out_dev[2c+1] = (re, im) of sum_{x in subset} f_c(x), fp64, the same
+ *               fixed summation order as qdp_sum (bit-identical results); caller-owned
+ *   cuda_stream a cudaStream_t (NULL = legacy default stream).  Asynchronous: synchronise that
+ *               stream (or order later work on it) before reading out_dev
+ *
+ * All calls on a device share the one scratch array, which keeps the previous call's contents;
+ * nothing in it needs clearing (each call overwrites every slot it later reads).  Calls that
+ * overlap on the GPU -- different streams without ordering between them -- race on it and return
+ * garbage; calls on one stream are safe.  The first call on each device also looks up the array's
+ * device address (cudaGetSymbolAddress; may load the library's device code): make that first call
+ * outside any stream capture.  Errors: QDP_ERR_ARG / QDP_ERR_DIMS before any launch, QDP_ERR_CUDA
+ * for a failed look-up or launch; nothing is written on error. */
+int qdp_sum_noalloc(const int dims[4], int ncomp, qdp_prec prec, const void* field_dev, size_t bytes,
+                    qdp_subset subset, double* out_dev, void* cuda_stream);
+
 /* dst = a*x + b*y on the subset, real a, b cast to the field precision, any kind (all three
  * fields of the same kind and precision): the residual and solution-reconstruction expressions
  * around the solver (r = b - A x, x += alpha p).  Element-wise, so dst may be x or y.

@@ -19,7 +19,7 @@ __all__ = [
     "qdp_field_alloc", "qdp_field_wrap", "qdp_field_free", "qdp_field_bytes",
     "qdp_field_upload", "qdp_field_download", "qdp_field_copy",
     "qdp_shift", "qdp_plaquette", "qdp_ape_smear_step", "qdp_hop", "qdp_axpy_hop", "qdp_smear_hop", "qdp_inner_timeslices", "qdp_inner_timeslices_gamma", "qdp_reunitarize", "qdp_project_max_retr", "qdp_baryon_timeslices", "qdp_matmul", "qdp_matvec", "qdp_axpby", "qdp_expr_plaquette", "qdp_expr_staple", "qdp_expr_ape_blend", "qdp_expr_trace_mul", "qdp_expr_sum_trace_mul", "qdp_expr_jit_kind", "qdp_expr_jit_compile", "qdp_expr_jit_assign", "qdp_expr_jit_sum", "qdp_expr_jit_compilations", "QDP_REUNIT_POLAR", "QDP_REUNIT_GRAM_SCHMIDT",
-    "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_kernel_launch_count", "qdp_last_error",
+    "qdp_norm2", "qdp_inner", "qdp_sum", "qdp_sum_noalloc", "qdp_kernel_launch_count", "qdp_last_error",
     "qdp_set_allocator", "field_from_host", "field_to_host",
     "qdp_field_timeslice_bytes", "qdp_field_get_timeslice", "qdp_field_set_timeslice",
     "Pool", "Cached", "qdp_pool_create", "qdp_pool_destroy", "qdp_pool_alloc", "qdp_pool_free", "qdp_pool_stats",
@@ -91,6 +91,7 @@ DECLARED_SYMBOLS = {
     "qdp_norm2": ([_P, _I, _P], _I),
     "qdp_inner": ([_P, _P, _I, _P], _I),
     "qdp_sum": ([_P, _I, _P], _I),
+    "qdp_sum_noalloc": ([ctypes.POINTER(ctypes.c_int), _I, _I, _P, _Z, _I, _P, _P], _I),
     "qdp_lattice_sync": ([_P], _I),
     "qdp_kernel_launch_count": ([], ctypes.c_int64),
     "qdp_last_error": ([], ctypes.c_char_p),
@@ -472,6 +473,15 @@ def qdp_sum(f: Field, subset: int = QDP_ALL) -> np.ndarray:
     out = np.empty(2 * _NCOMP[f.kind])
     _check(_lib.qdp_sum(f.handle, subset, out.ctypes.data))
     return (out[0::2] + 1j * out[1::2]).reshape(_SHAPE[f.kind])
+
+
+def qdp_sum_noalloc(dims, ncomp: int, prec: int, field_dev: int, nbytes: int, subset: int, out_dev: int,
+                    cuda_stream: int | None = None) -> None:
+    """qdp_sum without a lattice handle and without any allocation, for callers that may not call cudaMalloc
+    (include/qdp_b200.h).  field_dev / out_dev are raw device addresses on the current device (out_dev: 2 * ncomp
+    doubles); the call is asynchronous on cuda_stream.  Calls that overlap on the GPU race on the shared scratch."""
+    _check(_lib.qdp_sum_noalloc((ctypes.c_int * 4)(*[int(d) for d in dims]), int(ncomp), int(prec), field_dev,
+                                int(nbytes), int(subset), out_dev, cuda_stream))
 
 
 def qdp_field_timeslice_bytes(f: Field) -> int:

@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqdp_b200.so")
 PROBE_LIB = os.path.join(HERE, "libqdp_probe.so")   # bench-only peak probes (csrc/probe.cu), not part of the C ABI
-SOURCES = ["api.cu", "layout.cu", "shift.cu", "reduce.cu", "hop.cu", "plaquette.cu", "plaquette_tma.cu", "ape.cu", "reunit.cu", "matmul.cu", "expr.cu", "baryon.cu", "pool.cu", "jit.cu"]
+SOURCES = ["api.cu", "layout.cu", "shift.cu", "reduce.cu", "hop.cu", "plaquette.cu", "plaquette_tma.cu", "ape.cu", "reunit.cu", "matmul.cu", "expr.cu", "baryon.cu", "pool.cu", "jit.cu", "noalloc.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xptxas", "-v",
