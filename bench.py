@@ -40,10 +40,10 @@ UNIT = "site-updates/s"
 OPS_PER_STEP = 7          # shift, plaquette, ape, hop(even+odd), inner, axpy_hop+norm2, norm2
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
 # fp64 instructions per site of the fused kernels as implemented (SASS, straight-line code: every instruction
-# executes once per site; profiles/r2_sass.md): (DFMA, DMUL, DADD).  The "alu" view of the roofline divides the
+# executes once per site; profiles/r3_sass.md, counted with cuobjdump): (DFMA, DMUL, DADD).  The "alu" view of the roofline divides the
 # resulting flop rate by the DFMA rate measured in the same run (paper_1111_5596_b200/csrc/probe.cu).
 FP64_INSTR_PER_SITE = {
-    "ape": (3300, 491, 92),          # 24 3x3 complex products, blend, three SU(3) projections
+    "ape": (3310, 493, 89),          # 24 3x3 complex products, blend, three SU(3) projections
     "plaquette": (1188, 219, 18),    # 12 products + 6 traces
 }
 
@@ -306,15 +306,17 @@ def run_ours(args) -> dict | None:
         "expr_plaquette": (lambda: q.qdp_expr_plaquette(u), 36,
                            "qdp_expr_plaquette (row f1): the plaquette written as one expression of the compile-time "
                            "layer, one kernel; compare ops.plaquette (hand-fused)"),
-        "jit_plaquette": (lambda: (q.qdp_expr_jit_sum(JIT_PLAQ_S, [u]), q.qdp_expr_jit_sum(JIT_PLAQ_T, [u])), 72,
+        "jit_plaquette": (lambda: (q.qdp_expr_jit_sum(JIT_PLAQ_S, [u]), q.qdp_expr_jit_sum(JIT_PLAQ_T, [u])), 36,
                           "qdp_expr_jit_sum (row f1, run-time expressions): the spatial and the temporal planes of the plaquette "
-                          "as two text expressions compiled with NVRTC on first use (cached afterwards): two kernels, the "
-                          "gauge field is read twice; compare expr_plaquette (nvcc, one kernel) and ops.plaquette"),
-        "jit_hop": (lambda: q.qdp_expr_jit_assign(chi, 0, JIT_HOP, [u, psi]), 48,
+                          "as two text expressions compiled with NVRTC on first use (cached afterwards): two kernels, so the "
+                          "gauge field is really read twice, but the algorithmic bytes are those of the plaquette (36 complex "
+                          "per site) and the fraction is charged for the second read; compare expr_plaquette and ops.plaquette"),
+        "jit_hop": (lambda: q.qdp_expr_jit_assign(chi, 0, JIT_HOP, [u, psi]), 60,
                     "qdp_expr_jit_assign (row f1): the hopping term of def. 5 on the full lattice as a text expression with "
-                    "fermion leaves (u 36 + chi 12 complex per site); compare the hand-fused qdp_hop ALL (hop_all)"),
-        "hop_all": (lambda: q.qdp_hop(chi, u, psi, q.QDP_ALL), 48,
-                    "qdp_hop on the full lattice, hand-fused (the step times the halves and the fused axpy form)"),
+                    "fermion leaves (u 36 + psi 12 + chi 12 complex per site, SURVEY.md 8(d): 960 B in fp64); compare the hand-fused qdp_hop ALL (hop_all)"),
+        "hop_all": (lambda: q.qdp_hop(chi, u, psi, q.QDP_ALL), 60,
+                    "qdp_hop on the full lattice, hand-fused (the step times the halves and the fused axpy form): "
+                    "u 36 + psi 12 + chi 12 complex per site"),
         "jit_staple": (lambda: q.qdp_expr_jit_assign(cm, 0, JIT_STAPLE, [u]), 36,
                        "qdp_expr_jit_assign (row f1): the spatial staple sum of link 0 as a text expression; the same kernel as "
                        "expr_staple, through NVRTC"),
@@ -324,8 +326,10 @@ def run_ours(args) -> dict | None:
         "project_max_retr": (lambda: q.qdp_project_max_retr(u2, u, 3), 72,
                              "qdp_project_max_retr, 3 sweeps (row f2): 36 complex read + 36 written per site"),
         "baryon_timeslices": (lambda: q.qdp_baryon_timeslices([psi, chi, sh], [chi, sh, psi], [sh, psi, chi], 5), 36,
-                              "qdp_baryon_timeslices, nsrc = 3 (row f3): here 3 distinct spinor fields stand in for the 9 "
-                              "propagator columns (36 complex per site algorithmic), includes the host round trip"),
+                              "qdp_baryon_timeslices, nsrc = 3 (row f3): the call takes nine field arguments (108 complex per site "
+                              "when they are nine different propagator columns); this row passes 3 distinct spinor fields three "
+                              "times each, so the bytes that must move, and are counted, are 36 complex per site; includes the "
+                              "host round trip"),
         "plaquette_staged": (None, 36, "qdp_plaquette with qdp_lattice_set_staged(1): cp.async.bulk + mbarrier "
                                        "shared-memory rings (plaquette_tma.cu); compare ops.plaquette"),
     }
@@ -442,9 +446,11 @@ def run_ours(args) -> dict | None:
     other = {}
     if world == 1 and not args.no_other_configs and args.config == "C4" and prec == "f64":
         peak_o, _ = measured_peak()
-        for cfg, pr in (("C4", "f32"), ("C3", "f64"), ("C3", "f32")):
+        # C5 (48^3 x 96, 6.1 GB fp64 gauge field) is BASELINE.json's "bandwidth at scale" configuration: few steps, its
+        # host-side generation and upload dominate the ~20 s each precision adds to the run
+        for cfg, pr in (("C4", "f32"), ("C3", "f64"), ("C3", "f32"), ("C5", "f64"), ("C5", "f32")):
             wo = Workload(q, torch, cfg, pr, local, synth.BASE_SEED + 3)
-            ko = max(3, min(K, 10))
+            ko = max(3, min(K, 10)) if cfg != "C5" else 3
             tot, per_op, _ = wo.timed(ko, 3)
             other[f"{cfg}/{pr}"] = {"ms_per_step": round(tot / ko, 5), "steps": ko,
                                     "site_updates_per_s": OPS_PER_STEP * wo.V * ko / (tot * 1e-3),
@@ -597,7 +603,7 @@ def main():
     ap.add_argument("--cpu-fraction", type=int, default=1, help="cpu_baseline runs on V/fraction sites (1: one whole pass, ~15 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
-    ap.add_argument("--no-other-configs", action="store_true", help="skip the C4 f32 / C3 f64 / C3 f32 per-op block")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the C4 f32 / C3 / C5 per-op block")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     out = run_reference(args) if args.impl == "reference" else run_ours(args)

@@ -40,7 +40,10 @@
  *     subset's sites.  Neighbours are read from wherever they are.
  *   - Kernels are enqueued on the lattice's stream (default: the legacy default
  *     stream).  Field->field calls are asynchronous with respect to the host;
- *     calls that return host scalars synchronise that stream before returning.
+ *     calls that return host scalars return only when the result is complete: the
+ *     reducing kernel writes it to mapped pinned host memory followed by a
+ *     completion number, which the call polls (everything enqueued on that stream
+ *     before it has finished by then; qdp_sum synchronises the stream instead).
  *   - Neighbour-reading operations are out of place: passing the destination as
  *     a neighbour-read source returns QDP_ERR_ALIAS.
  *   - There is no CPU fallback anywhere: a missing device is an error.
@@ -221,7 +224,9 @@ int qdp_matvec(qdp_field* chi, const qdp_field* a, int slot_a, int adj_a, const 
  * u_out == u_in is allowed.  Arithmetic in fp64 for both precisions.  Asynchronous.
  * Conditioning: Proj is invariant under V -> c V (c > 0) and is evaluated on V / |V|_F, then
  * polished by Newton-Schulz steps until V^dag V = 1 to ~50 ulp; the result is accurate to about
- * cond(V) * 2^-52 per matrix for cond(V) up to ~1e5 (singular V: undefined, no error is raised). */
+ * cond(V) * 2^-52 per matrix for cond(V) up to ~1e5 (singular V of non-zero norm: undefined, no
+ * error is raised).  Under QDP_REUNIT_POLAR a matrix that is exactly zero, or has an infinite or
+ * NaN entry, has no polar factor and is copied to u_out unchanged (never turned into NaNs). */
 enum { QDP_REUNIT_POLAR = 0, QDP_REUNIT_GRAM_SCHMIDT = 1 };
 int qdp_reunitarize(qdp_field* u_out, const qdp_field* u_in, int method, qdp_subset subset);
 

@@ -580,9 +580,9 @@ def qdp_cache_release(c: Cached) -> None:
 
 
 def qdp_cache_unregister(c: Cached) -> None:
-    h, c.handle = c.handle, None
-    if h:
-        _check(_lib.qdp_cache_unregister(h))
+    if c.handle:
+        _check(_lib.qdp_cache_unregister(c.handle))     # a refused call ("still acquired") keeps the handle, so it can be retried
+        c.handle = None
 
 
 def qdp_cache_is_resident(c: Cached) -> bool:

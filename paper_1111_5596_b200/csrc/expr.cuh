@@ -185,33 +185,42 @@ template <class A, class B> struct Sum : Node {
 template <class E> struct Trace : Node {
     template <class T> __device__ __forceinline__ static Cx<T> eval(const Env<T>& e) { return v_trace(E::template eval<T>(e)); }
 };
-// trace(a * b) = sum_ij a_ij b_ji: no product is formed
+// trace(a * b) = sum_ij a_ij b_ji: no product is formed when both factors are matrices; any other pair the
+// language allows under a trace (real scalar * matrix, either order) takes the plain route
+template <class T> __device__ __forceinline__ Cx<T> v_trace_mul(const Mat3<T>& a, const Mat3<T>& b) {
+    Cx<T> s = cx<T>(0, 0);
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) cmad(s, a.e[i * 3 + j], b.e[j * 3 + i]);
+    return s;
+}
+template <class T> __device__ __forceinline__ Cx<T> v_trace_mul(T s, const Mat3<T>& b) { return v_mul(s, v_trace(b)); }
+template <class T> __device__ __forceinline__ Cx<T> v_trace_mul(const Mat3<T>& a, T s) { return v_mul(s, v_trace(a)); }
 template <class A, class B> struct Trace<Product<A, B>> : Node {
     template <class T> __device__ __forceinline__ static Cx<T> eval(const Env<T>& e) {
-        const Mat3<T> a = A::template eval<T>(e), b = B::template eval<T>(e);
-        Cx<T> s = cx<T>(0, 0);
-#pragma unroll
-        for (int i = 0; i < 3; i++)
-#pragma unroll
-            for (int j = 0; j < 3; j++) cmad(s, a.e[i * 3 + j], b.e[j * 3 + i]);
-        return s;
+        return v_trace_mul(A::template eval<T>(e), B::template eval<T>(e));
     }
 };
 template <class E> struct Real : Node {
     template <class T> __device__ __forceinline__ static T eval(const Env<T>& e) { return v_real(E::template eval<T>(e)); }
 };
-// real(trace(a * b)) = sum_ij Re(a_ij b_ji): 18 multiply-adds
+// real(trace(a * b)) = sum_ij Re(a_ij b_ji): 18 multiply-adds for two matrices
+template <class T> __device__ __forceinline__ T v_real_trace_mul(const Mat3<T>& a, const Mat3<T>& b) {
+    T s0 = 0, s1 = 0, s2 = 0;
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        s0 = fma(a.e[j].re, b.e[j * 3].re, s0);         s0 = fma(-a.e[j].im, b.e[j * 3].im, s0);
+        s1 = fma(a.e[3 + j].re, b.e[j * 3 + 1].re, s1); s1 = fma(-a.e[3 + j].im, b.e[j * 3 + 1].im, s1);
+        s2 = fma(a.e[6 + j].re, b.e[j * 3 + 2].re, s2); s2 = fma(-a.e[6 + j].im, b.e[j * 3 + 2].im, s2);
+    }
+    return s0 + s1 + s2;
+}
+template <class T> __device__ __forceinline__ T v_real_trace_mul(T s, const Mat3<T>& b) { return s * v_trace(b).re; }
+template <class T> __device__ __forceinline__ T v_real_trace_mul(const Mat3<T>& a, T s) { return s * v_trace(a).re; }
 template <class A, class B> struct Real<Trace<Product<A, B>>> : Node {
     template <class T> __device__ __forceinline__ static T eval(const Env<T>& e) {
-        const Mat3<T> a = A::template eval<T>(e), b = B::template eval<T>(e);
-        T s0 = 0, s1 = 0, s2 = 0;
-#pragma unroll
-        for (int j = 0; j < 3; j++) {
-            s0 = fma(a.e[j].re, b.e[j * 3].re, s0);         s0 = fma(-a.e[j].im, b.e[j * 3].im, s0);
-            s1 = fma(a.e[3 + j].re, b.e[j * 3 + 1].re, s1); s1 = fma(-a.e[3 + j].im, b.e[j * 3 + 1].im, s1);
-            s2 = fma(a.e[6 + j].re, b.e[j * 3 + 2].re, s2); s2 = fma(-a.e[6 + j].im, b.e[j * 3 + 2].im, s2);
-        }
-        return s0 + s1 + s2;
+        return v_real_trace_mul(A::template eval<T>(e), B::template eval<T>(e));
     }
 };
 

@@ -65,7 +65,7 @@ struct Geom {
     // L2-aware sweep order of the neighbour-reading kernels (sweep_block below); slab_c2 = 0: linear
     int slab_c2;      // x2 extent of a slab (a divisor of L2)
     int slab_ipr;     // 32-site blocks per (x2, x3) line of the (x0, x1) plane = Lh0 * L1 / 32
-    int staged;       // 1: use the shared-memory-staged kernels (plaquette_tma.cu, ape_tma.cu) where the lattice allows
+    int staged;       // 1: use the shared-memory-staged kernels (plaquette_tma.cu) where the lattice allows
 
 #ifndef __CUDACC_RTC__
     __host__ static Geom make(const int* L) {

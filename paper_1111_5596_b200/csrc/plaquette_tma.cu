@@ -230,11 +230,11 @@ static cudaError_t launch_plaquette_tma_t(const Geom& g, const void* u, const Re
     pg.nplanes = g.L2 * g.L3;
     pg.nblk_half = g.Vhp >> 5;
     const int smem = (int)sizeof(PlaqTmaSmem<T>);
-    static bool attr_set = false;
-    if (!attr_set) {
+    // the opt-in is a per-device property of the function: set it on whichever device is current (cheap, and safe
+    // from several host threads, unlike a process-wide flag)
+    {
         cudaError_t e = cudaFuncSetAttribute(plaquette_tma_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     const int grid = pg.nplanes < sms ? pg.nplanes : sms;
     const double n = (double)g.V;

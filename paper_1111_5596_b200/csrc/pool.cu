@@ -140,6 +140,8 @@ extern "C" int qdp_pool_create(int device, size_t bytes, qdp_pool** out) {
 extern "C" int qdp_pool_destroy(qdp_pool* p) {
     if (!ok_pool(p)) return qdp::set_error(QDP_ERR_ARG, "qdp_pool_destroy: not a pool");
     if (!p->lru_.empty()) return qdp::set_error(QDP_ERR_ARG, "qdp_pool_destroy: cached objects still registered");
+    // blocks handed out by qdp_pool_alloc / qdp_pool_hook_alloc (fields, a lattice's scratch) would dangle after the cudaFree below
+    if (!p->used_.empty()) return qdp::set_error(QDP_ERR_ARG, "qdp_pool_destroy: blocks of this pool are still allocated (free the fields and lattices that live in it first)");
     if (p->device >= 0) {
         int prev = 0;
         cudaGetDevice(&prev);

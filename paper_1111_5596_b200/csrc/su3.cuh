@@ -457,6 +457,10 @@ __device__ __forceinline__ Mat3<double> proj_su3_general(Mat3<double> V) {
     double n2 = 0;
 #pragma unroll
     for (int c = 0; c < 9; c++) n2 = fma(V.e[c].re, V.e[c].re, fma(V.e[c].im, V.e[c].im, n2));
+    // The zero matrix has no polar factor, and a matrix with an infinite or NaN entry no meaningful one: such a
+    // matrix is returned as it came (inf * 0 below would otherwise turn a zero link into NaNs), so the caller can
+    // still see what was wrong with it.  Documented with qdp_reunitarize in qdp_b200.h.
+    if (!(n2 > 0.0) || !(n2 <= 1.7976931348623157e308)) return V;
     const double sc = 1.7320508075688772 / sqrt(n2);
 #pragma unroll
     for (int c = 0; c < 9; c++) V.e[c] = cx<double>(V.e[c].re * sc, V.e[c].im * sc);

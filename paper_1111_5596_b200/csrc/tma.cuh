@@ -1,5 +1,5 @@
 // tma.cuh -- sm_100a bulk-copy (TMA engine, `cp.async.bulk`) and mbarrier primitives used by the
-// shared-memory-staged kernels (plaquette_tma.cu, ape_tma.cu).  Thin inline-PTX wrappers only.
+// shared-memory-staged kernels (plaquette_tma.cu).  Thin inline-PTX wrappers only.
 //
 // Pattern ("staged kernels"): one producer lane arms a "full" mbarrier with the
 // byte count of a ring slot (arrive.expect_tx) and issues the bulk copies global -> shared that

@@ -89,6 +89,10 @@ def slab_shift(q, dst, src, mu: int, sign: int, subset: int, comm, scratch=None)
     q.qdp_field_get_timeslice(src, plan["send_slice"], send.data_ptr(), nbytes)
     q.qdp_lattice_sync(lat)                    # the face must be complete before the communication library reads it
     comm.sendrecv(send, plan["send_to"], recv, plan["recv_from"])
+    # The communication (NCCL's kernels, or the loopback copy) runs on torch's current stream, and req.wait() only
+    # orders that stream, not the host.  The unpack kernel goes to the lattice's own stream, which may be a
+    # non-blocking one that has no implicit ordering with it: wait here until `recv` is really written.
+    torch.cuda.current_stream(torch.device("cuda", lat.device)).synchronize()
     q.qdp_field_set_timeslice(dst, plan["fix_slice"], recv.data_ptr(), nbytes, subset)
     return scratch
 

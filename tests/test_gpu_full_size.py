@@ -77,21 +77,27 @@ def _check_step(qdp, dims, prec, seed, n_ape_steps=1, warm=False):
     assert np.abs(g @ np.conj(np.swapaxes(g, 1, 2)) - np.eye(3)).max() <= unit_bar
     assert np.abs(np.linalg.det(g) - 1).max() <= unit_bar
 
-    # ---- further APE steps (ping-pong, A16): plaquette rises, links stay in SU(3); the last step is compared
-    # with the oracle on the sampled sites, restarted from the downloaded field of the step before it
+    # ---- further APE steps (ping-pong, A16): the plaquette triple is recorded after EVERY step and compared with the
+    # oracle's plaquette of the downloaded device field of that step (whole-lattice sum, nothing chained); the spatial
+    # plaquette rises, links stay in SU(3); the last step is also compared link by link with the oracle on the sampled
+    # sites, restarted from the downloaded field of the step before it
     if n_ape_steps > 1:
         bufs = [u2, qdp.qdp_field_alloc(lat, 1, _prec_id(prec))]
         prev = qdp.qdp_plaquette(bufs[0])[1]
+        triples = []
+        field = _as64(got_u)                      # the device field after the first step, downloaded above
         for k in range(n_ape_steps - 1):
-            last = k == n_ape_steps - 2
-            if last:
-                before = _as64(qdp.field_to_host(bufs[0]))
+            before = field
             qdp.qdp_ape_smear_step(bufs[1], bufs[0], 0.5, 3)
             bufs.reverse()
-            cur = qdp.qdp_plaquette(bufs[0])[1]
-            assert cur > prev
-            prev = cur
-        got_last = qdp.field_to_host(bufs[0])
+            triple = qdp.qdp_plaquette(bufs[0])
+            triples.append(triple)
+            field = _as64(qdp.field_to_host(bufs[0]))
+            assert np.abs(triple - oracle.plaquette(dims, field)).max() <= bar, ("plaquette after APE step", k + 2)
+            assert triple[1] > prev
+            prev = triple[1]
+        assert len(triples) == n_ape_steps - 1 and np.all(np.isfinite(np.array(triples)))
+        got_last = field
         for mu in range(3):
             want = np.stack([oracle.ape_site(dims, before, int(s), mu, 0.5, 3) for s in sites])
             fixed, n_centre = z3_fix(_as64(got_last[sites, mu]), want)
@@ -161,8 +167,9 @@ def test_c4_bench_configuration_fp64(qdp):
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_c3_sweep_and_normalised_iteration(qdp, prec):
     """BASELINE.json:configs[2]: chi = a psi + b hop(psi), norm2 after every step, 50 iterations
-    (A14/A15: normalised, the 1/sqrt(n_k) folded into the scalars).  The first 3 steps are checked
-    against the oracle on the whole lattice, the remaining ones by the recorded norms."""
+    (A14/A15: normalised, the 1/sqrt(n_k) folded into the scalars).  The field and the recorded n_k are
+    compared with the oracle on the whole lattice at every step of the first spinor in fp64 and at a spread of
+    steps otherwise (each time from the device field of the step before), the rest by the norm bound."""
     dims = synth.CONFIGS["C3"]
     seed = synth.BASE_SEED + 2
     _check_step(qdp, dims, prec, seed, warm=True)
@@ -174,7 +181,12 @@ def test_c3_sweep_and_normalised_iteration(qdp, prec):
     for ispinor in range(1, 5):          # reading A14: four independent spinor fields, the same (a, b)
         hp = synth.round_to(synth.spinor(dims, seed, ispinor), prec)
         bufs = [qdp.field_from_host(lat, 2, hp), qdp.qdp_field_alloc(lat, 2, _prec_id(prec))]
-        ref = _as64(hp)
+        # steps whose field and recorded n_k are compared with the oracle (about 1.2 s of oracle time each): the whole
+        # 50-step sequence for the first spinor in fp64, a spread of it otherwise
+        if ispinor == 1:
+            checked = set(range(50)) if prec == "f64" else {0, 1, 2, 9, 19, 29, 39, 49}
+        else:
+            checked = {0, 49}
         scale = 1.0
         norms = []
         for k in range(50):
@@ -184,12 +196,11 @@ def test_c3_sweep_and_normalised_iteration(qdp, prec):
             n_k = qdp.qdp_axpy_hop(bufs[1], ak, bk, u, bufs[0], 0, want_norm2=True)
             bufs.reverse()
             norms.append(n_k)
-            if k < (3 if ispinor == 1 else 1):
-                ref = oracle.axpy_hop(dims, ak, bk, u64, ref)
+            if k in checked:
+                ref = oracle.axpy_hop(dims, ak, bk, u64, _as64(qdp.field_to_host(bufs[1])))   # from the device field of the step before: per-step error, no drift
                 got = _as64(qdp.field_to_host(bufs[0]))
-                assert site_rel_err(got, ref).max() <= (k + 1) * TOL_SITE[prec], (ispinor, k)
-                assert abs(n_k - oracle.norm2(dims, ref)) <= TOL_SUM[prec] * n_k
-                ref = got          # continue the oracle from the device field: per-step error, not drift
+                assert site_rel_err(got, ref).max() <= TOL_SITE[prec], (ispinor, k)
+                assert abs(n_k - oracle.norm2(dims, ref)) <= TOL_SUM[prec] * n_k, (ispinor, k)
             scale = 1.0 / np.sqrt(n_k)
         norms = np.array(norms)
         assert np.all(np.isfinite(norms)) and np.all(norms > 0)

@@ -40,6 +40,32 @@ def test_loopback_shift_equals_the_periodic_shift_and_faces_round_trip(qdp, dims
         qdp.qdp_field_get_timeslice(src, 0, buf.data_ptr(), nbytes - 16)
 
 
+def test_loopback_shift_on_a_non_default_lattice_stream(qdp):
+    """The lattice's kernels run on a non-blocking stream of their own while the communication runs on torch's current
+    stream: slab_shift has to order the two itself (there is no implicit null-stream ordering to hide a missing wait).
+    A large face and a busy current stream make a missing wait visible."""
+    import torch
+    dims = (16, 16, 16, 4)
+    lat = qdp.qdp_lattice_create(dims)
+    own = torch.cuda.Stream()
+    qdp.qdp_lattice_set_stream(lat, own.cuda_stream)
+    hu = synth.gauge_hot(dims, 1403)
+    src = qdp.field_from_host(lat, qdp.QDP_GAUGE, hu)
+    comm = slab.LoopbackComm()
+    busy = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
+    scratch = None
+    for sign in (+1, -1):
+        sentinel = np.full_like(hu, 3.0 - 1.0j)
+        dst = qdp.field_from_host(lat, qdp.QDP_GAUGE, sentinel)
+        qdp.qdp_lattice_sync(lat)
+        for _ in range(8):
+            busy.fill_(1)                                 # work queued on torch's current stream ahead of the copy
+        scratch = slab.slab_shift(qdp, dst, src, 3, sign, 0, comm, scratch)
+        assert np.array_equal(qdp.field_to_host(dst), oracle.shift(dims, hu, 3, sign, 0, dst=sentinel)), sign
+    qdp.qdp_lattice_sync(lat)
+    qdp.qdp_lattice_set_stream(lat, None)
+
+
 @pytest.mark.parametrize("gdims", [(4, 4, 4, 8), (8, 8, 8, 16), (4, 2, 6, 8)])
 @pytest.mark.parametrize("kind", ["fermion", "gauge"])
 def test_two_emulated_ranks_reproduce_the_global_shift(qdp, gdims, kind):

@@ -133,7 +133,8 @@ def test_spinor_expressions_are_def5_and_def6(dims):
 # ---- the library's host-side front end (no GPU): it must accept and reject what the oracle's language does ------
 VALID = [("f0[1] * f1", ee.MAT), ("trace(f0[1] * f1)", ee.CPLX), ("real(trace(f1)) * s0", ee.REAL), ("s0 * f1 * s1", ee.MAT),
          ("trace(f1) * trace(adj(f1)) + trace(f0[3])", ee.CPLX), (LOWER.format(m=0, n=2), ee.MAT), ("( f1+adj( f1 ) )*s1", ee.MAT),
-         ("imag(trace(f1)) * real(trace(f0[0]))", ee.REAL), ("trace(f1) * s0", ee.CPLX)]
+         ("imag(trace(f1)) * real(trace(f0[0]))", ee.REAL), ("trace(f1) * s0", ee.CPLX),
+         ("trace(s0 * f1)", ee.CPLX), ("real(trace(f1 * s0))", ee.REAL), ("trace((s0 * f1) * f0[1])", ee.CPLX)]
 INVALID = ["f0 + trace(f1)", "trace(trace(f1))", "real(f1)", "f1 * trace(f1)", "f1[1]", "f0[4]", "f2", "shift(f1, +4)", "f0 +",
            "shift(f0, 2)", "f0 f1", "(f0", "s2 * f1", "", "f0[0] * ", "adj f1"]
 
@@ -184,3 +185,7 @@ def test_nvrtc_compiles_an_expression_once_without_a_gpu():
     assert q.qdp_expr_jit_compilations() == before + 2
     with pytest.raises(q.QdpError):
         q.qdp_expr_jit_compile("f0[0]", kinds, 0, q.QDP_F64, sum_=True)              # a matrix cannot be summed
+    # every shape the front end accepts must also get through the compiler: a real scalar directly under a trace
+    for shape in ("trace(s0 * f0[0])", "real(trace(f0[0] * s0))", "trace((s0 * f0[0]) * f0[1])"):
+        for prec in (q.QDP_F64, q.QDP_F32):
+            assert q.qdp_expr_jit_compile(shape, kinds, 1, prec, sum_=True) > 1000, shape

@@ -153,3 +153,24 @@ def test_cpp_pool_textbook_lru(qdp):
     for o in objs.values():
         qdp.qdp_cache_unregister(o)
     qdp.qdp_pool_destroy(pool)
+
+
+def test_destroy_and_unregister_refuse_while_memory_is_in_use(qdp):
+    """A pool with a live block is not destroyed (the block would dangle), and an unregister that is refused because the
+    object is still acquired keeps the Python handle so that it can be retried."""
+    pool = qdp.qdp_pool_create(-1, 16 * 1024)
+    ptr = qdp.qdp_pool_alloc(pool, 1024)
+    with pytest.raises(qdp.QdpError) as e:
+        qdp.qdp_pool_destroy(pool)
+    assert "still allocated" in str(e.value) and pool.handle
+    qdp.qdp_pool_free(pool, ptr)
+    obj = qdp.qdp_cache_register(pool, None, 4096)
+    qdp.qdp_cache_acquire(obj)
+    with pytest.raises(qdp.QdpError):
+        qdp.qdp_cache_unregister(obj)
+    assert obj.handle
+    qdp.qdp_cache_release(obj)
+    qdp.qdp_cache_unregister(obj)
+    assert obj.handle is None
+    qdp.qdp_pool_destroy(pool)
+    assert pool.handle is None
