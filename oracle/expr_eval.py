@@ -6,10 +6,10 @@ in the order the expression is written.  Shares nothing with ``csrc/jit.cu``: ow
 
 Grammar (the same language the library documents in ``include/qdp_b200.h``):
 
-    expr   := term { '+' term }          term := factor { '*' factor }
-    factor := adj(expr) | trace(expr) | real(expr) | imag(expr) | norm2(expr) | inner(expr, expr)
+    expr   := term { ('+' | '-') term }  term := factor { '*' factor }
+    factor := '-' factor | adj(expr) | trace(expr) | real(expr) | imag(expr) | norm2(expr) | inner(expr, expr)
             | shift(expr, +mu | -mu) | '(' expr ')' | leaf
-    leaf   := f<k> [ '[' slot ']' ]  |  s<k>
+    leaf   := f<k> [ '[' slot ']' ]  |  s<k>  |  number        (number: decimal literal, e.g. 2, 0.5, 1.5e-3)
 
 Values: matrix field [V,3,3] complex128, spinor field [V,4,3] complex128 (a fermion argument), complex field [V]
 complex128, real field [V] float64 (a scalar argument is a constant real field).  adj = conjugate transpose / complex
@@ -17,7 +17,8 @@ conjugate / identity on reals (not defined on spinors); trace over the colour in
 colour of |psi|^2, inner(a, b) = sum over spin and colour of conj(a) b; shift(e, +mu)(x) = e(x + mu) with periodic wrap
 (reading A3), done by ``oracle.shift`` on the evaluated array; '*' is the per-site matrix product, a matrix acting on the
 colour index of every spin component of a spinor, scaling by a real or a complex number, or the product of complex
-numbers; '+' adds values of equal kind.
+numbers; '+' adds and '-' subtracts values of equal kind, a leading '-' negates a value of any kind (it binds tighter than
+'*': -a * b = (-a) * b), a number is a constant real field like a scalar argument.
 """
 from __future__ import annotations
 
@@ -28,7 +29,8 @@ import numpy as np
 from . import shift as _shift, volume as _volume
 
 MAT, CPLX, REAL, SPINOR = 0, 1, 2, 3
-_TOKEN = re.compile(r"\s*(adj|trace|real|imag|norm2|inner|shift|f\d|s\d|[()\[\],+\-*]|\d)")
+_NUMBER = r"(?:\d+\.\d*|\.\d+|\d+)(?:[eE][+-]?\d+)?"
+_TOKEN = re.compile(r"\s*(adj|trace|real|imag|norm2|inner|shift|f\d|s\d|[()\[\],+\-*]|" + _NUMBER + ")")
 
 
 class ExprError(ValueError):
@@ -49,8 +51,8 @@ def tokenize(text: str) -> list[str]:
 
 def parse(text: str):
     """Returns a nested tuple tree: ('f', k, slot | None) | ('s', k) | ('adj'|'trace'|'real'|'imag'|'norm2', e) |
-    ('inner', a, b) | ('shift', e, mu, sign) | ('+', a, b) | ('*', a, b); '+' and '*' associate to the left, '*' binds
-    tighter."""
+    ('inner', a, b) | ('shift', e, mu, sign) | ('+', a, b) | ('-', a, b) | ('*', a, b) | ('neg', e) | ('num', value);
+    '+', '-' and '*' associate to the left, '*' binds tighter, the unary minus tighter still."""
     toks = tokenize(text)
     pos = 0
 
@@ -67,9 +69,9 @@ def parse(text: str):
 
     def expr():
         node = term()
-        while peek() == "+":
-            take()
-            node = ("+", node, term())
+        while peek() in ("+", "-"):
+            op = take()
+            node = (op, node, term())
         return node
 
     def term():
@@ -79,8 +81,16 @@ def parse(text: str):
             node = ("*", node, factor())
         return node
 
+    def small_int(what):
+        t = take()
+        if not (len(t) == 1 and t.isdigit()):
+            raise ExprError(f"{what}: one digit expected, got {t!r}")
+        return int(t)
+
     def factor():
         t = take()
+        if t == "-":
+            return ("neg", factor())
         if t in ("adj", "trace", "real", "imag", "norm2"):
             take("(")
             e = expr()
@@ -100,7 +110,7 @@ def parse(text: str):
             sign = {"+": 1, "-": -1}.get(take())
             if sign is None:
                 raise ExprError("'+' or '-' expected in shift")
-            mu = int(take())
+            mu = small_int("direction")
             take(")")
             return ("shift", e, mu, sign)
         if t == "(":
@@ -111,11 +121,13 @@ def parse(text: str):
             slot = None                      # None: no subscript written
             if peek() == "[":
                 take()
-                slot = int(take())
+                slot = small_int("slot")
                 take("]")
             return ("f", int(t[1]), slot)
         if t[0] == "s" and len(t) == 2:
             return ("s", int(t[1]))
+        if t[0].isdigit() or t[0] == ".":
+            return ("num", float(t))
         raise ExprError(f"operand expected, got {t!r}")
 
     tree = expr()
@@ -138,8 +150,10 @@ def kind_of(tree, field_slots) -> int:
         if (tree[2] or 0) >= field_slots[tree[1]]:
             raise ExprError("slot out of range")
         return MAT
-    if op == "s":
+    if op in ("s", "num"):
         return REAL
+    if op == "neg":
+        return kind_of(tree[1], field_slots)
     if op in ("adj", "shift"):
         if op == "shift" and not 0 <= tree[2] <= 3:
             raise ExprError("direction must be 0..3")
@@ -164,9 +178,9 @@ def kind_of(tree, field_slots) -> int:
         if a != SPINOR or b != SPINOR:
             raise ExprError("inner() takes two spinors")
         return CPLX
-    if op == "+":
+    if op in ("+", "-"):
         if a != b:
-            raise ExprError("'+' needs operands of the same kind")
+            raise ExprError(f"'{op}' needs operands of the same kind")
         return a
     if a == REAL:
         return b
@@ -201,6 +215,10 @@ def evaluate(dims, text: str, fields, scalars=()):
             return fields[t[1]].copy() if is_spinor[t[1]] else mats[t[1]][:, t[2] or 0].copy()
         if op == "s":
             return np.full(V, float(scalars[t[1]]))
+        if op == "num":
+            return np.full(V, t[1])
+        if op == "neg":
+            return -ev(t[1])
         if op == "adj":
             v = ev(t[1])
             return np.conj(np.swapaxes(v, 1, 2)) if is_mat(v) else np.conj(v)
@@ -222,6 +240,8 @@ def evaluate(dims, text: str, fields, scalars=()):
         a, b = ev(t[1]), ev(t[2])
         if op == "+":
             return a + b
+        if op == "-":
+            return a - b
         if is_mat(a) and is_mat(b):
             out = np.zeros_like(a)
             for i in range(3):            # (a b)_ij = sum_k a_ik b_kj, written out

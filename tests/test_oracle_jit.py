@@ -104,6 +104,58 @@ def test_algebraic_identities():
     assert abs(ev("trace(f0[1] * f1)")[x] - want) < 1e-13
 
 
+def test_minus_and_numbers_parse_and_type():
+    """Binary '-' (left-associative, same level as '+'), the unary minus (binds tighter than '*') and decimal literals."""
+    f0, f1, f2 = ("f", 0, None), ("f", 1, None), ("f", 2, None)
+    assert ee.parse("f0 - f1 - f2") == ("-", ("-", f0, f1), f2)
+    assert ee.parse("f0 - f1 + f2") == ("+", ("-", f0, f1), f2)
+    assert ee.parse("f0 - f1 * f2") == ("-", f0, ("*", f1, f2))
+    assert ee.parse("-f0 * f1") == ("*", ("neg", f0), f1)
+    assert ee.parse("f0 - -f1") == ("-", f0, ("neg", f1))
+    assert ee.parse("2 * f0") == ("*", ("num", 2.0), f0)
+    assert ee.parse("f0[1] * 1.5e-3") == ("*", ("f", 0, 1), ("num", 0.0015))
+    assert ee.parse(".5 + 10.") == ("+", ("num", 0.5), ("num", 10.0))
+    assert ee.parse("shift(f0 - 2 * f1, -3)") == ("shift", ("-", f0, ("*", ("num", 2.0), f1)), 3, -1)
+    for bad in ("f0 -", "- ", "f0[10]", "shift(f0, +12)", "1.5.2", "2 f0", "f0 - * f1", "1e"):
+        with pytest.raises(ee.ExprError):
+            ee.parse(bad)
+    slots = [4, 1, 0]
+    assert ee.kind_of(ee.parse("f0[1] - f1"), slots) == ee.MAT
+    assert ee.kind_of(ee.parse("-f2"), slots) == ee.SPINOR
+    assert ee.kind_of(ee.parse("f2 - 0.5 * f1 * f2"), slots) == ee.SPINOR
+    assert ee.kind_of(ee.parse("0.5"), slots) == ee.REAL
+    assert ee.kind_of(ee.parse("-real(trace(f1)) - 3"), slots) == ee.REAL
+    for bad in ("f0 - trace(f1)", "trace(f1) - 2", "f2 - f1", "f1 - 1"):
+        with pytest.raises(ee.ExprError):
+            ee.kind_of(ee.parse(bad), slots)
+
+
+def test_minus_and_numbers_evaluate_to_numpy_arithmetic():
+    """Pinned on numpy written out here (elementwise subtraction, negation and scaling need nothing of the evaluator but the
+    leaves) and on what the algebra fixes."""
+    dims = (4, 2, 6, 4)
+    hu, hm, hp = synth.gauge_hot(dims, 49), synth.color_matrix(dims, 50), synth.spinor(dims, 51)
+    ev = lambda t, s=(): ee.evaluate(dims, t, [hu, hm, hp], s)[0]
+    assert np.array_equal(ev("f0[1] - f1"), hu[:, 1] - hm)
+    assert np.array_equal(ev("-f1"), -hm)
+    assert np.array_equal(ev("-f2"), -hp)
+    assert np.array_equal(ev("2.5 * f1"), 2.5 * hm)
+    assert np.array_equal(ev("f0[0] - f1 * 0.5"), hu[:, 0] - hm * 0.5)
+    assert np.array_equal(ev("f1 - f0[2] - f0[3]"), (hm - hu[:, 2]) - hu[:, 3])              # left-associative
+    assert np.array_equal(ev("-f1 * f0[1]"), ev("(-f1) * f0[1]"))
+    assert not ev("f1 - f1").any() and not ev("f2 - f2").any()
+    assert np.array_equal(ev("f1 - s0 * f0[1]", (0.75,)), ev("f1 + s0 * f0[1]", (-0.75,)))       # a - c b = a + (-c) b
+    assert np.array_equal(ev("f1 - 0.75 * f0[1]"), ev("f1 - s0 * f0[1]", (0.75,)))              # a literal is a scalar argument
+    assert np.array_equal(ev("real(trace(f1 - adj(f1)))"), np.zeros(synth.volume(dims)))         # anti-Hermitian part: imaginary trace
+    assert np.array_equal(ev("trace(f1) - trace(f1) * 2"), -(hm[:, 0, 0] + hm[:, 1, 1] + hm[:, 2, 2]))
+    # the residual of PAPER.md:96, r = b - A x, against the C oracle's hop
+    r = ev("f2 - 0.3 * (" + HOP_F2 + ")")
+    want = hp - 0.3 * oracle.hop(dims, hu, hp)
+    assert np.abs(r - want).max() < 1e-13 * np.abs(want).max()
+    assert abs(ee.total(dims, "norm2(f2 - f2 * 0.5)", [hu, hm, hp]).real - 0.25 * oracle.norm2(dims, hp)) < 1e-12 * oracle.norm2(dims, hp)
+
+
+HOP_F2 = " + ".join(f"f0[{m}] * shift(f2, +{m}) + shift(adj(f0[{m}]) * f2, -{m})" for m in range(4))
 HOP = " + ".join(f"f0[{m}] * shift(f1, +{m}) + shift(adj(f0[{m}]) * f1, -{m})" for m in range(4))
 
 
