@@ -381,17 +381,20 @@ int qdp_expr_sum_trace_mul(const qdp_field* a, int slot_a, int adj_a, const qdp_
  * for sm_100a into ONE kernel and cached by (expression, precision, assignment | sum).  The first use of an expression
  * costs one compilation (0.2-0.4 s); later uses launch the cached kernel.  libnvrtc is loaded at the first compilation
  * (QDP_ERR_CUDA with a message if it is missing); nothing is read from the file system.
- *   expr   := term { '+' term }            term := factor { '*' factor }
- *   factor := adj(expr) | trace(expr) | real(expr) | imag(expr) | norm2(expr) | inner(expr, expr)
+ *   expr   := term { ('+' | '-') term }    term := factor { '*' factor }
+ *   factor := '-' factor | adj(expr) | trace(expr) | real(expr) | imag(expr) | norm2(expr) | inner(expr, expr)
  *           | shift(expr, +mu | -mu) | '(' expr ')' | leaf
  *   leaf   := f<k> [ '[' slot ']' ]        field argument k = 0..3: matrix `slot` of a QDP_COLOR_MATRIX or QDP_GAUGE field
  *                                          (a link of a gauge field; default 0), or the spinor of a QDP_FERMION field
  *           | s<k>                         real scalar argument k = 0..3 (cast to the field precision)
+ *           | number                       decimal literal (2, 0.5, 1.5e-3): a real constant; unlike a scalar argument it
+ *                                          is part of the compiled expression, so another value is another kernel
  * Semantics as in the build-time layer and SURVEY.md 8(c): a value is a 3x3 matrix, a spinor (4 spin x 3 colour), a
  * complex number or a real number; adj = conjugate transpose (conjugate of a complex number; not defined on spinors),
  * trace: matrix -> complex, real / imag: complex -> real, norm2: spinor -> real (sum over spin and colour of |.|^2),
  * inner(a, b): two spinors -> complex (sum of conj(a) b), shift(e, +mu)(x) = e(x + mu) for the whole sub-expression e
- * (A3), '+' needs equal kinds, '*' is matrix * matrix, matrix * spinor (the matrix acts on the colour index of every spin
+ * (A3), '+' and '-' need equal kinds (a - b is the elementwise difference: the residual r = b - A x of PAPER.md:96 is
+ * "f1 - s0 * (...)"), a leading '-' negates a value of any kind and binds tighter than '*', '*' is matrix * matrix, matrix * spinor (the matrix acts on the colour index of every spin
  * component: the product of the hopping term, A11), real * anything, anything * real, complex * complex or complex *
  * spinor.  All field arguments belong to one lattice and precision.  Example, the hopping term of def. 5:
  *   "f0[0] * shift(f1, +0) + shift(adj(f0[0]) * f1, -0) + f0[1] * shift(f1, +1) + ..."  with f0 = u, f1 = psi.

@@ -125,6 +125,21 @@ template <class T> __device__ __forceinline__ Cx<T> v_inner(const Spinor<T>& a, 
     return s;
 }
 
+template <class T> __device__ __forceinline__ Mat3<T> v_neg(const Mat3<T>& a) {
+    Mat3<T> r;
+#pragma unroll
+    for (int i = 0; i < 9; i++) r.e[i] = cx<T>(-a.e[i].re, -a.e[i].im);
+    return r;
+}
+template <class T> __device__ __forceinline__ Spinor<T> v_neg(const Spinor<T>& a) {
+    Spinor<T> r;
+#pragma unroll
+    for (int i = 0; i < 12; i++) r.e[i] = cx<T>(-a.e[i].re, -a.e[i].im);
+    return r;
+}
+template <class T> __device__ __forceinline__ Cx<T> v_neg(Cx<T> a) { return cx<T>(-a.re, -a.im); }
+template <class T> __device__ __forceinline__ T v_neg(T a) { return -a; }
+
 template <class T> __device__ __forceinline__ Cx<T> v_trace(const Mat3<T>& a) { return a.e[0] + a.e[4] + a.e[8]; }
 template <class T> __device__ __forceinline__ T v_real(Cx<T> a) { return a.re; }
 template <class T> __device__ __forceinline__ T v_imag(Cx<T> a) { return a.im; }
@@ -181,6 +196,19 @@ template <class A, class B> struct Sum : Node {
     template <class T> __device__ __forceinline__ static auto eval(const Env<T>& e) {
         return v_add(A::template eval<T>(e), B::template eval<T>(e));
     }
+};
+// -e, and a - b = a + (-b) (exactly the IEEE difference)
+template <class E> struct Neg : Node {
+    template <class T> __device__ __forceinline__ static auto eval(const Env<T>& e) { return v_neg(E::template eval<T>(e)); }
+};
+template <class A, class B> struct Diff : Node {
+    template <class T> __device__ __forceinline__ static auto eval(const Env<T>& e) {
+        return v_add(A::template eval<T>(e), v_neg(B::template eval<T>(e)));
+    }
+};
+// a real literal, carried in the type as the bit pattern of the double (cast to the field precision like a scalar argument)
+template <unsigned long long BITS> struct Lit : Node {
+    template <class T> __device__ __forceinline__ static T eval(const Env<T>&) { return (T)__longlong_as_double((long long)BITS); }
 };
 template <class E> struct Trace : Node {
     template <class T> __device__ __forceinline__ static Cx<T> eval(const Env<T>& e) { return v_trace(E::template eval<T>(e)); }
@@ -242,6 +270,9 @@ template <class A, class B, class = std::enable_if_t<is_node<A> && is_node<B>>>
 constexpr Product<A, B> operator*(A, B) { return {}; }
 template <class A, class B, class = std::enable_if_t<is_node<A> && is_node<B>>>
 constexpr Sum<A, B> operator+(A, B) { return {}; }
+template <class A, class B, class = std::enable_if_t<is_node<A> && is_node<B>>>
+constexpr Diff<A, B> operator-(A, B) { return {}; }
+template <class E, class = std::enable_if_t<is_node<E>>> constexpr Neg<E> operator-(E) { return {}; }
 template <class E> constexpr Adjoint<E> adj(E) { return {}; }
 template <class E> constexpr Trace<E> trace(E) { return {}; }
 template <class E> constexpr Real<E> real(E) { return {}; }

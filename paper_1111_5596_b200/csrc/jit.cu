@@ -5,17 +5,19 @@
 // once"), with the paper's PETE tree replaced by a small grammar and its code generator by the
 // template layer the build-time expressions already use.  Host code only: the kernels come out of NVRTC.
 //
-//   expr   := term { '+' term }
+//   expr   := term { ('+'|'-') term }
 //   term   := factor { '*' factor }
-//   factor := 'adj' '(' expr ')' | 'trace' '(' expr ')' | 'real' '(' expr ')' | 'imag' '(' expr ')'
+//   factor := '-' factor | 'adj' '(' expr ')' | 'trace' '(' expr ')' | 'real' '(' expr ')' | 'imag' '(' expr ')'
 //           | 'norm2' '(' expr ')' | 'inner' '(' expr ',' expr ')'
 //           | 'shift' '(' expr ',' ('+'|'-') DIGIT ')' | '(' expr ')' | leaf
 //   leaf   := 'f' DIGIT [ '[' DIGIT ']' ]     field argument DIGIT: matrix [slot] of a colour-matrix or gauge field (slot:
 //                                             link of a gauge field, default 0), or the spinor of a fermion field
 //           | 's' DIGIT                       real scalar argument DIGIT
+//           | NUMBER                          decimal literal (2, 0.5, 1.5e-3): a real constant, part of the expression's type
 // Value kinds: matrix (3x3 complex), complex, real, spinor (4 spin x 3 colour).  s -> real, adj keeps the kind (not
 // defined on spinors), trace: matrix -> complex, real/imag: complex -> real, norm2: spinor -> real, inner: two spinors ->
-// complex (the first conjugated), shift keeps the kind (shift(e, +mu)(x) = e(x + mu), A3), '+' needs equal kinds,
+// complex (the first conjugated), shift keeps the kind (shift(e, +mu)(x) = e(x + mu), A3), '+' and '-' need equal kinds,
+// the unary minus keeps the kind and binds tighter than '*',
 // '*': matrix*matrix, matrix*spinor (colour rotation of every spin component), real*anything, anything*real,
 // complex*complex, complex*spinor.
 //
@@ -64,13 +66,14 @@ struct Parser {
 
     bool expr(Parsed& out) {
         if (!term(out)) return false;
-        while (eat('+')) {
+        for (;;) {
+            const bool plus = eat('+');
+            if (!plus && !eat('-')) return true;
             Parsed r;
             if (!term(r)) return false;
-            if (r.kind != out.kind) return fail("'+' needs operands of the same kind (matrix, complex or real)");
-            out.type = "Sum<" + out.type + ", " + r.type + " >";
+            if (r.kind != out.kind) return fail("'+' and '-' need operands of the same kind (matrix, spinor, complex or real)");
+            out.type = std::string(plus ? "Sum<" : "Diff<") + out.type + ", " + r.type + " >";
         }
-        return true;
     }
     bool term(Parsed& out) {
         if (!factor(out)) return false;
@@ -99,6 +102,11 @@ struct Parser {
         return true;
     }
     bool factor(Parsed& out) {
+        if (eat('-')) {
+            if (!factor(out)) return false;
+            out.type = "Neg<" + out.type + " >";
+            return true;
+        }
         if (word("adj")) {
             if (!unary("Adjoint", out, -1, -1, "")) return false;
             if (out.kind == JIT_SPINOR) return fail("adj() of a spinor is not defined");
@@ -167,6 +175,29 @@ struct Parser {
             if (!digit(k)) return false;
             if (k >= nscalars) return fail("scalar argument out of range");
             out.type = "Sc<" + std::to_string(k) + ">";
+            out.kind = JIT_REAL;
+            return true;
+        }
+        if ((*s >= '0' && *s <= '9') || (*s == '.' && s[1] >= '0' && s[1] <= '9')) {
+            // digits [. digits] [e [+-] digits]; scanned here so that the accepted spellings do not depend on strtod's
+            // extras (hex floats, "inf", locale)
+            const char* b = s;
+            while (*s >= '0' && *s <= '9') s++;
+            if (*s == '.') { s++; while (*s >= '0' && *s <= '9') s++; }
+            if (*s == 'e' || *s == 'E') {
+                const char* m = s + 1;
+                if (*m == '+' || *m == '-') m++;
+                if (*m < '0' || *m > '9') return fail("digits expected in the exponent");
+                while (*m >= '0' && *m <= '9') m++;
+                s = m;
+            }
+            if ((*s >= 'a' && *s <= 'z') || (*s >= 'A' && *s <= 'Z') || *s == '.') return fail("malformed number");
+            const double v = strtod(std::string(b, s).c_str(), nullptr);
+            unsigned long long bits;
+            memcpy(&bits, &v, sizeof bits);
+            char buf[40];
+            snprintf(buf, sizeof buf, "Lit<0x%016llxull>", bits);
+            out.type = buf;
             out.kind = JIT_REAL;
             return true;
         }

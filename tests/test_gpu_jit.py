@@ -24,6 +24,9 @@ ASSIGN = [
     ("s0 * trace(f1) * trace(adj(f0[2])) + trace(f1 * f1)", (0.3,)),
     ("trace(s0 * f1)", (0.7,)),                                                  # a real scalar directly under the trace
     ("trace((s0 * f1) * f0[2]) + trace(f0[1] * s1)", (1.3, -0.6)),
+    ("f0[1] - f1 * 0.5", ()),                                                    # '-', literals, unary minus
+    ("-f1 * f0[2] - (f1 - adj(f1)) * s0 - - shift(f0[3], -1)", (0.25,)),
+    ("trace(f1 - adj(f1)) * -1.5e-1 - trace(f0[0])", ()),
 ]
 SUMS = [
     (PLAQ01, ()),
@@ -31,6 +34,8 @@ SUMS = [
     ("imag(trace(f1)) * real(trace(f0[0]))", ()),
     ("real(trace(adj(f1) * f1))", ()),
     ("real(trace(f1 * s0)) + real(trace(s1 * f0[2]))", (-0.4, 1.1)),
+    ("3 - real(trace(f0[0] * shift(f0[1], +0) * adj(shift(f0[0], +1)) * adj(f0[1])))", ()),   # 3 - Re tr (plaquette): the Wilson action density
+    ("-imag(trace(f1)) - 0.125 * real(trace(f0[2] - f1))", ()),
 ]
 
 
@@ -169,10 +174,12 @@ def test_jit_spinor_expressions(qdp, dims, prec):
     want_hop, kind = ee.evaluate(dims, HOP, h64)
     assert kind == ee.SPINOR
     want_axpy, _ = ee.evaluate(dims, axpy, h64, sc)
+    resid = f"f1 - s0 * ({HOP}) - 0.5 * -f1"          # the residual form b - A x of PAPER.md:96, with '-' and a literal
+    want_resid, _ = ee.evaluate(dims, resid, h64, _scalars((0.3,), prec))
     sentinel = np.full((V, 4, 3), 3.0 + 1.0j, hp.dtype)
     for subset in (0, 1, 2):
         sel = np.ones(V, bool) if subset == 0 else (mask == (subset - 1))
-        for text, want, s in ((HOP, want_hop, ()), (axpy, want_axpy, (0.3, -0.7))):
+        for text, want, s in ((HOP, want_hop, ()), (axpy, want_axpy, (0.3, -0.7)), (resid, want_resid, (0.3,))):
             chi = qdp.field_from_host(lat, 2, sentinel)
             qdp.qdp_expr_jit_assign(chi, 0, text, [u, psi], s, subset)
             got = qdp.field_to_host(chi)

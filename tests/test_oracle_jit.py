@@ -186,9 +186,12 @@ def test_spinor_expressions_are_def5_and_def6(dims):
 VALID = [("f0[1] * f1", ee.MAT), ("trace(f0[1] * f1)", ee.CPLX), ("real(trace(f1)) * s0", ee.REAL), ("s0 * f1 * s1", ee.MAT),
          ("trace(f1) * trace(adj(f1)) + trace(f0[3])", ee.CPLX), (LOWER.format(m=0, n=2), ee.MAT), ("( f1+adj( f1 ) )*s1", ee.MAT),
          ("imag(trace(f1)) * real(trace(f0[0]))", ee.REAL), ("trace(f1) * s0", ee.CPLX),
-         ("trace(s0 * f1)", ee.CPLX), ("real(trace(f1 * s0))", ee.REAL), ("trace((s0 * f1) * f0[1])", ee.CPLX)]
+         ("trace(s0 * f1)", ee.CPLX), ("real(trace(f1 * s0))", ee.REAL), ("trace((s0 * f1) * f0[1])", ee.CPLX),
+         ("f0[1] - f1", ee.MAT), ("-f1 * f0[2] - 0.5 * f1", ee.MAT), ("real(trace(f1)) - 2.5e-1", ee.REAL), ("- - f1", ee.MAT),
+         ("trace(f1 - adj(f1)) * -1", ee.CPLX), ("shift(f0[0] - 2 * f1, -3)", ee.MAT)]
 INVALID = ["f0 + trace(f1)", "trace(trace(f1))", "real(f1)", "f1 * trace(f1)", "f1[1]", "f0[4]", "f2", "shift(f1, +4)", "f0 +",
-           "shift(f0, 2)", "f0 f1", "(f0", "s2 * f1", "", "f0[0] * ", "adj f1"]
+           "shift(f0, 2)", "f0 f1", "(f0", "s2 * f1", "", "f0[0] * ", "adj f1", "f0 -", "f1 - 1", "trace(f1) - 2", "1.5.2", "2 f1",
+           "f0[10]", "shift(f1, +12)", "1e"]
 
 
 def test_library_front_end_agrees_with_the_oracle_language():
@@ -207,10 +210,11 @@ def test_library_front_end_agrees_with_the_oracle_language():
                 raise ee.ExprError("scalar argument out of range")   # the oracle takes its scalars from a Python sequence
     kinds = [q.QDP_GAUGE, q.QDP_COLOR_MATRIX, q.QDP_FERMION]
     for text, kind in [("f0[1] * shift(f2, +1)", ee.SPINOR), ("s0 * f2 + f1 * f2 * s1 + trace(f1) * f2 + f2 * trace(f1)", ee.SPINOR),
-                       ("norm2(f1 * f2)", ee.REAL), ("inner(f2, f0[3] * f2)", ee.CPLX), (HOP.replace("f1", "f2"), ee.SPINOR)]:
+                       ("norm2(f1 * f2)", ee.REAL), ("inner(f2, f0[3] * f2)", ee.CPLX), (HOP.replace("f1", "f2"), ee.SPINOR),
+                       ("f2 - 0.3 * (" + HOP_F2 + ")", ee.SPINOR), ("-f2", ee.SPINOR), ("norm2(f2 - f1 * f2)", ee.REAL)]:
         assert ee.kind_of(ee.parse(text), [4, 1, 0]) == kind
         assert q.qdp_expr_jit_kind(text, kinds, 2) == kind, text
-    for text in ("f2 * f1", "f2 * f2", "adj(f2)", "trace(f2)", "f2[0]", "norm2(f1)", "inner(f2, f1)", "f2 + f1", "inner(f2)"):
+    for text in ("f2 * f1", "f2 * f2", "adj(f2)", "trace(f2)", "f2[0]", "norm2(f1)", "inner(f2, f1)", "f2 + f1", "inner(f2)", "f2 - f1", "f2 - 1"):
         with pytest.raises(q.QdpError):
             q.qdp_expr_jit_kind(text, kinds, 2)
         with pytest.raises(ee.ExprError):
@@ -238,6 +242,7 @@ def test_nvrtc_compiles_an_expression_once_without_a_gpu():
     with pytest.raises(q.QdpError):
         q.qdp_expr_jit_compile("f0[0]", kinds, 0, q.QDP_F64, sum_=True)              # a matrix cannot be summed
     # every shape the front end accepts must also get through the compiler: a real scalar directly under a trace
-    for shape in ("trace(s0 * f0[0])", "real(trace(f0[0] * s0))", "trace((s0 * f0[0]) * f0[1])"):
+    for shape in ("trace(s0 * f0[0])", "real(trace(f0[0] * s0))", "trace((s0 * f0[0]) * f0[1])",
+                  "real(trace(-f0[0] - 0.5 * f0[1])) - 2", "trace(f0[0]) * -1.5e-1"):
         for prec in (q.QDP_F64, q.QDP_F32):
             assert q.qdp_expr_jit_compile(shape, kinds, 1, prec, sum_=True) > 1000, shape
