@@ -7,8 +7,12 @@ What the decomposition changes, and nothing else:
     neighbouring rank's boundary slice -- ONE face exchange per shift (qdp_field_get_timeslice -> send/recv ->
     qdp_field_set_timeslice).  Shifts along x0, x1, x2 are purely local.
   * global sums: all-reduce of the local doubles.
-The fused neighbour-reading kernels (hop, plaquette, APE) read x3 neighbours inside their kernel and would need ghost
-slices; bench.py therefore runs replicas only (BASELINE.json: one GPU), and this module covers shift and the reductions.
+The fused neighbour-reading kernels (hop, plaquette) read their x3 neighbours inside the kernel and wrap inside the slab,
+so on a slab they are evaluated the way the paper evaluates everything -- expression by expression, each shift along x3
+one halo exchange (slab_hop, slab_plaquette below): the parts that never leave a time-slice stay fused (the spatial
+hops, the spatial plaquette, the whole spatial APE step), the x3 terms are built from slab_shift and the site-local
+products.  That is several passes instead of one: it is the functional multi-GPU path, not a tuned one; bench.py runs
+replicas only (BASELINE.json: one GPU).
 
 `comm` is a small adapter over torch.distributed (or LoopbackComm for one rank); every function here is argument
 marshalling and message ordering -- the data movement on the device is the two kernels of csrc/layout.cu."""
@@ -105,3 +109,55 @@ def slab_inner(q, a, b, subset: int, comm) -> complex:
     z = q.qdp_inner(a, b, subset)
     re, im = comm.allreduce_sum([z.real, z.imag])
     return complex(re, im)
+
+
+def _opposite(subset: int) -> int:
+    return (0, 2, 1)[subset]
+
+
+def slab_ape_smear_step(q, u_out, u_in, alpha: float, subset: int = 0):
+    """The spatial APE step (t_dir = 3) on a slab: its staples never leave the time-slice, so the fused kernel is already
+    the global answer and nothing is exchanged.  (The 4-D step reads x3 neighbours and is not offered on slabs.)"""
+    q.qdp_ape_smear_step(u_out, u_in, alpha, 3, subset)
+
+
+def slab_hop(q, chi, u, psi, subset: int, comm, work=None):
+    """chi(x) = sum_mu [U_mu(x) psi(x+mu) + U_mu^dag(x-mu) psi(x-mu)] of the GLOBAL lattice on the sites of `subset`;
+    chi, u, psi: this rank's slab fields.  Spatial directions: one fused local kernel.  x3: psi(x+3) by slab_shift then the
+    colour rotation; (U_3^dag psi) formed at the source sites (the other parity) then moved by slab_shift.  Two face
+    exchanges of one spinor time-slice each.  `work`: two spinor fields of the slab (allocated if None), returned."""
+    lat = psi.lat
+    if work is None:
+        work = (q.qdp_field_alloc(lat, q.QDP_FERMION, psi.prec), q.qdp_field_alloc(lat, q.QDP_FERMION, psi.prec))
+    t1, t2 = work
+    q.qdp_smear_hop(chi, 0.0, 1.0, u, psi, 3, subset)                 # mu = 0, 1, 2
+    slab_shift(q, t1, psi, 3, +1, subset, comm)                       # t1(x) = psi(x + 3)
+    q.qdp_matvec(t2, u, 3, False, t1, -1, 1, subset)                  # U_3(x) psi(x + 3)
+    q.qdp_axpby(chi, 1.0, chi, 1.0, t2, subset)
+    q.qdp_matvec(t1, u, 3, True, psi, -1, 1, _opposite(subset))       # (U_3^dag psi)(y) at the source sites y = x - 3
+    slab_shift(q, t2, t1, 3, -1, subset, comm)                        # t2(x) = (U_3^dag psi)(x - 3)
+    q.qdp_axpby(chi, 1.0, chi, 1.0, t2, subset)
+    return work
+
+
+def slab_plaquette(q, u, comm, work=None):
+    """[all, spatial, temporal] plaquette of the GLOBAL lattice, normalised as qdp_plaquette.  The spatial planes never
+    leave a time-slice: the fused kernel's spatial sum is exact on a slab.  The three temporal planes need U_mu(x + 3): one
+    slab_shift of the gauge field (one face exchange), then per plane P = U_mu(x) U_3(x+mu), Q = U_3(x) U_mu(x+3) and
+    sum_x Re tr(P Q^dag).  `work`: (gauge field, colour matrix, colour matrix) of the slab, returned as the second value."""
+    import numpy as np
+    lat = u.lat
+    if work is None:
+        work = (q.qdp_field_alloc(lat, q.QDP_GAUGE, u.prec), q.qdp_field_alloc(lat, q.QDP_COLOR_MATRIX, u.prec),
+                q.qdp_field_alloc(lat, q.QDP_COLOR_MATRIX, u.prec))
+    us, P, Q = work
+    v_local = lat.volume
+    spatial = float(q.qdp_plaquette(u)[1]) * 9.0 * v_local            # back to the plain sum over this slab
+    slab_shift(q, us, u, 3, +1, 0, comm)                              # us(x) = u(x + 3)
+    temporal = 0.0
+    for mu in range(3):
+        q.qdp_matmul(P, 0, u, mu, False, u, 3, False, mu, +1)
+        q.qdp_matmul(Q, 0, u, 3, False, us, mu, False, -1, 1)
+        temporal += q.qdp_expr_sum_trace_mul(P, 0, False, Q, 0, True).real
+    sp, tp, vol = comm.allreduce_sum([spatial, temporal, float(v_local)])
+    return np.array([(sp + tp) / (18.0 * vol), sp / (9.0 * vol), tp / (9.0 * vol)]), work

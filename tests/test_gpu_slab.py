@@ -98,3 +98,85 @@ def test_two_emulated_ranks_reproduce_the_global_shift(qdp, gdims, kind):
                 assert np.array_equal(got, want[r * Lt * n:(r + 1) * Lt * n]), (sign, subset, r)
     total = sum(qdp.qdp_norm2(s) for s in srcs)
     assert abs(total - oracle.norm2(gdims, full)) <= 1e-12 * total
+
+
+class _ThreadComm:
+    """Two ranks of one process, one host thread each, every rank driving a lattice of its own on the one GPU.  A face
+    travels as a device tensor through a queue; only host threads wait for one another, never a kernel."""
+
+    def __init__(self, rank, world, boxes, barrier, sums):
+        self.rank, self.world, self.boxes, self.barrier, self.sums = rank, world, boxes, barrier, sums
+
+    def sendrecv(self, send, send_to, recv, recv_from):
+        import torch
+        torch.cuda.current_stream().synchronize()
+        self.boxes[send_to][self.rank].put(send.clone())
+        recv.copy_(self.boxes[self.rank][recv_from].get(timeout=60))
+        torch.cuda.current_stream().synchronize()
+
+    def allreduce_sum(self, values):
+        self.sums[self.rank] = list(values)
+        self.barrier.wait(timeout=60)
+        out = [sum(self.sums[r][i] for r in range(self.world)) for i in range(len(values))]
+        self.barrier.wait(timeout=60)
+        return out
+
+
+@pytest.mark.parametrize("gdims", [(4, 4, 4, 8), (4, 2, 6, 4), (8, 8, 8, 16)])
+def test_two_thread_ranks_hop_plaquette_and_ape_on_slabs(qdp, gdims):
+    """slab_hop, slab_plaquette and the spatial APE step on two x3 slabs reproduce the oracle's results on the global
+    lattice (hop: every subset, per-site bar; plaquette: the bar for sums; APE: the per-link bar)."""
+    import queue
+    import threading
+    from parity import TOL_SITE, links, site_rel_err, z3_fix
+    world = 2
+    ldims = slab.local_dims(gdims, world)
+    n, Lt = gdims[0] * gdims[1] * gdims[2], ldims[3]
+    hu, hp = synth.gauge_hot(gdims, 1404), synth.spinor(gdims, 1405)
+    want_hop = oracle.hop(gdims, hu, hp)
+    want_plaq = oracle.plaquette(gdims, hu)
+    want_ape = oracle.ape_smear_step(gdims, hu, 0.5, 3)
+    mask = oracle.parity_mask(gdims)
+    boxes = [[queue.Queue() for _ in range(world)] for _ in range(world)]
+    barrier, sums, results, errors = threading.Barrier(world), [None] * world, [None] * world, []
+
+    def run(rank):
+        try:
+            comm = _ThreadComm(rank, world, boxes, barrier, sums)
+            lo, hi = rank * Lt * n, (rank + 1) * Lt * n
+            lat = qdp.qdp_lattice_create(ldims)
+            u = qdp.field_from_host(lat, qdp.QDP_GAUGE, hu[lo:hi].copy())
+            psi = qdp.field_from_host(lat, qdp.QDP_FERMION, hp[lo:hi].copy())
+            out = {}
+            work = None
+            for subset in (0, 1, 2):
+                sentinel = np.full_like(hp[lo:hi], 7.0 - 3.0j)
+                chi = qdp.field_from_host(lat, qdp.QDP_FERMION, sentinel)
+                work = slab.slab_hop(qdp, chi, u, psi, subset, comm, work)
+                out["hop", subset] = qdp.field_to_host(chi)
+            out["plaq"], _ = slab.slab_plaquette(qdp, u, comm)
+            u2 = qdp.qdp_field_alloc(lat, qdp.QDP_GAUGE, qdp.QDP_F64)
+            slab.slab_ape_smear_step(qdp, u2, u, 0.5)
+            out["ape"] = qdp.field_to_host(u2)
+            results[rank] = out
+        except BaseException as exc:      # surfaces in the main thread; the other rank then times out on its queue
+            errors.append((rank, exc))
+            barrier.abort()
+
+    threads = [threading.Thread(target=run, args=(r,)) for r in range(world)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+    assert not errors, errors
+    for rank in range(world):
+        lo, hi = rank * Lt * n, (rank + 1) * Lt * n
+        out = results[rank]
+        for subset in (0, 1, 2):
+            sel = np.ones(hi - lo, bool) if subset == 0 else (mask[lo:hi] == (subset - 1))
+            got = out["hop", subset]
+            assert np.all(got[~sel] == 7.0 - 3.0j), (rank, subset)                       # other sites untouched
+            assert site_rel_err(got[sel], want_hop[lo:hi][sel]).max() <= TOL_SITE["f64"], (rank, subset)
+        assert np.abs(out["plaq"] - want_plaq).max() <= 1e-10, (rank, out["plaq"], want_plaq)
+        fixed, n_centre = z3_fix(links(out["ape"].astype(np.complex128)), links(want_ape[lo:hi]))
+        assert n_centre == 0 and site_rel_err(fixed, links(want_ape[lo:hi])).max() <= TOL_SITE["f64"], rank
